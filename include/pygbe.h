@@ -1,0 +1,175 @@
+/*
+ * pygbe.h -- C ABI of libpygbe: the treecode-accelerated boundary-element matrix-vector product of the
+ * linearised Poisson-Boltzmann equation (PyGBe, arXiv:1309.4018) and the ring around it (right-hand
+ * side, restarted GMRES, reaction potential / solvation energy), hand-written CUDA for sm_100a.
+ *
+ * Citations are PAPER.md:<line> (+ section / equation).  "Reading Ax" refers to DESIGN.md.
+ *
+ * Conventions
+ *   Units        Angstrom, elementary charges, energies in kJ/mol
+ *                (C0 = qe^2 N_A 1e7 / eps0 = 17459.1429 kJ A /(mol e^2), reading A17).
+ *   Surfaces     closed triangulated surfaces; triangles counter-clockwise seen from region_out, so the
+ *                unit normal points region_in -> region_out (reading A3).  Every surface separates
+ *                exactly two regions.  Disjoint closed components with identical (region_in,
+ *                region_out) may be passed as one surface.
+ *   Regions      region r has permittivity eps[r] and inverse Debye length kappa[r] (1/Angstrom);
+ *                kappa[r] == 0 selects the Laplace kernel 1/(4 pi r), otherwise the Yukawa kernel
+ *                exp(-kappa r)/(4 pi r) (eq. 2).
+ *   Unknowns     surfaces in creation order; for surface s with N_s panels (caller's triangle order)
+ *                x = [ phi_s (N_s) ; dphi/dn_s (N_s) ], the derivative taken on the region_in side
+ *                along the normal (eq. 10 unknown [phi_1 ; dphi_1/dn]).
+ *   Rows         y = [ equation of region_in(s) collocated on s (N_s) ; equation of region_out(s) (N_s) ].
+ *                Row of region Omega collocated on panel i of surface T (eq. 9/10, PAPER.md:98-108;
+ *                several surfaces: PAPER.md:121-133, reading A4):
+ *                   1/2 phi_T,i - sum_{S in dOmega} sigma_S [ c_S (V_TS dphi_S)_i - (K_TS phi_S)_i ]
+ *                sigma_S = +1, c_S = 1 when Omega = region_in(S); sigma_S = -1,
+ *                c_S = eps[region_in(S)]/eps[region_out(S)] when Omega = region_out(S).
+ *                Green's functions carry 1/(4 pi); the right-hand side is sum_k q_k G(x_i,r_k)/eps.
+ *   Memory       pointers marked HOST are host memory, read during the call and never retained;
+ *                pointers marked DEVICE are device memory on the handle's device, owned by the caller
+ *                (e.g. torch tensors), fp64, pygbe_num_unknowns() long.  The library allocates its own
+ *                internal device memory (reported by pygbe_stats) and frees it in pygbe_destroy.
+ *   Stream       all work of a handle is issued on the stream given in pygbe_options (a cudaStream_t,
+ *                e.g. torch.cuda.current_stream().cuda_stream; NULL = legacy default stream).  Calls
+ *                taking DEVICE pointers are asynchronous unless stated; one handle is not re-entrant.
+ *   Errors       every call returns PYGBE_OK (0) or a negative code; nothing throws or aborts across
+ *                the ABI; pygbe_last_error() gives a thread-local message.  A failed pygbe_create
+ *                leaves *out = NULL.
+ */
+#ifndef PYGBE_H
+#define PYGBE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PYGBE_OK        0
+#define PYGBE_EINVAL   (-1)  /* null pointer, bad size, unsupported K / P, theta < 0, bad region ids,  */
+                             /* open / inconsistently oriented mesh, zero-area triangle               */
+#define PYGBE_ENOMEM   (-2)  /* device or host allocation failed                                       */
+#define PYGBE_ECUDA    (-3)  /* a CUDA call or kernel failed                                           */
+#define PYGBE_ENOCONV  (-4)  /* GMRES reached max_iter; x and the residual are still returned          */
+
+#define PYGBE_PRECISION_FP64  0  /* every kernel in fp64                                               */
+#define PYGBE_PRECISION_MIXED 1  /* P2P / M2P arithmetic in fp32 (cell-local coordinates), fp64        */
+                                 /* accumulation, fp64 near-field corrections, fp64 GMRES              */
+
+typedef struct pygbe_handle pygbe_handle; /* opaque, owned by the library */
+
+/* One closed surface ("flat triangular panels"). HOST pointers. */
+typedef struct {
+    const double  *vertices;   int64_t n_vertices;   /* [n_vertices][3], Angstrom                    */
+    const int32_t *triangles;  int64_t n_triangles;  /* [n_triangles][3], 0-based vertex ids         */
+    int32_t region_in, region_out;
+} pygbe_surface;
+
+/* Point charges (eq. 1). HOST pointers; region == NULL puts all charges in region 0. */
+typedef struct {
+    const double  *xyz;    /* [n][3] Angstrom */
+    const double  *q;      /* [n] units of e  */
+    const int32_t *region; /* [n] or NULL     */
+    int64_t n;
+} pygbe_charges;
+
+/* Options; zero-initialise and set what you need (0 selects the default given in brackets). */
+typedef struct {
+    int32_t K_fine;     /* Gauss points in the near-singular region [19]  (Tables 4, 6)  */
+    double  thres;      /* near-singular radius in units of L = sqrt(2 A_j) [2.0] (Table 6; A7);       */
+                        /* negative disables the near-singular rule (self panels are still analytic)   */
+    int32_t N_k;        /* Gauss-Legendre points per side of the semi-analytic self integral [5]       */
+    int32_t ncrit;      /* max source panels per octree leaf (NCRIT of PAPER.md:155, in panels) [auto] */
+    int32_t precision;  /* PYGBE_PRECISION_* [FP64]                                                    */
+    int32_t device;     /* CUDA device ordinal [0]                                                     */
+    void   *stream;     /* cudaStream_t [NULL]                                                         */
+    int32_t check_mesh; /* 1: verify closedness / orientation on the host in create [0]                */
+    int32_t reserved[7];
+} pygbe_options;
+
+/* Counters and timings filled by pygbe_stats. */
+typedef struct {
+    int64_t n_panels, n_unknowns, n_regions, n_surfaces, n_charges;
+    int64_t n_points;            /* Gauss points summed over regions (a point bounding 2 regions x2)   */
+    int64_t n_cells, n_leaves, n_groups, tree_depth;
+    int64_t p2p_pairs;           /* (target, Gauss point) pairs evaluated directly per matvec          */
+    int64_t m2p_evals;           /* (target, accepted cell) Taylor evaluations per matvec              */
+    int64_t direct_equiv;        /* sum_regions N_targets x N_points: interactions of the dense matvec */
+    int64_t near_nnz;            /* entries of the singular / near-singular correction (a8)            */
+    int64_t device_bytes;        /* internal device memory held by the handle                          */
+    int64_t n_matvec;            /* matvecs executed so far                                            */
+    int64_t kernels_per_matvec;  /* kernel launches one pygbe_matvec issues                            */
+    int64_t kernel_launches;     /* all kernel launches issued by this handle so far                   */
+    double  create_ms, last_solve_ms;
+    int32_t last_iters;
+    int32_t P, K, precision;
+    double  theta;
+} pygbe_stats_t;
+
+/*
+ * Build everything that depends on geometry only ("compute the tree structure and
+ * interaction list only once"): panel geometry and Gauss points (a1), Morton-sorted octree per region
+ * (a2), traversal with the multipole-acceptance criterion theta > r_b / r_tb (eq. 15, PAPER.md:155-159;
+ * reading A8: r_b = cell edge, r_tb = distance to the cell centre) into M2P / P2P lists (a5), and the
+ * singular / near-singular corrections (a8).
+ *   K      Gauss points per panel, one of 1, 3, 4, 7
+ *   P      order of the Cartesian Taylor expansion, 1..12        (eq. 13-14)
+ *   theta  MAC parameter, >= 0; theta == 0 never accepts a cell, i.e. direct O(N^2) summation
+ * Synchronous.  All HOST inputs are copied.
+ */
+int pygbe_create(const pygbe_surface *surfaces, int32_t n_surfaces, const pygbe_charges *charges,
+                 const double *eps, const double *kappa, int32_t n_regions,
+                 int32_t K, int32_t P, double theta, const pygbe_options *opt, pygbe_handle **out);
+
+void pygbe_destroy(pygbe_handle *h);
+
+/* 2 * total number of panels; < 0 on a NULL handle. */
+int64_t pygbe_num_unknowns(const pygbe_handle *h);
+
+/* y = A x: one evaluation of the treecode: P2M (eq. 14), upward pass, M2P with the
+ * Laplace / Yukawa recurrences, P2P, near-field corrections, block combination (eq. 10).
+ * x_dev, y_dev: DEVICE, must not alias.  Asynchronous on the handle's stream. */
+int pygbe_matvec(pygbe_handle *h, const double *x_dev, double *y_dev);
+
+/* Same with HOST buffers: copies x to the device, runs the matvec, copies y back, synchronises. */
+int pygbe_matvec_host(pygbe_handle *h, const double *x_host, double *y_host);
+
+/* b = right-hand side, eq. (9)/(11) with the 1/(4 pi) of eq. (9) (reading A2).
+ * b_dev: DEVICE.  Asynchronous. */
+int pygbe_rhs(pygbe_handle *h, double *b_dev);
+
+/* Restarted GMRES, x0 = 0, no preconditioner, stop at ||b - A x||/||b|| <= tol
+ * (reading A16).  The whole iteration runs on the device; the host only polls a convergence flag.
+ * x_dev: DEVICE, receives the solution.  iters, rel_resid: HOST, may be NULL.  Synchronous.
+ * Returns PYGBE_ENOCONV if max_iter matvecs did not reach tol. */
+int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t max_iter, double *x_dev,
+                int32_t *iters, double *rel_resid);
+
+/* HOST-buffer convenience: solve and copy x back (x_host may be NULL), then evaluate the energies. */
+int pygbe_solve_host(pygbe_handle *h, double tol, int32_t restart, int32_t max_iter, double *x_host,
+                     int32_t *iters, double *rel_resid, double *E_solv_kJ_per_mol,
+                     double *E_coul_kJ_per_mol);
+
+/* Reaction potential at the charges (eq. 4) and dG_solv = 1/2 sum q_k phi_reac(r_k)
+ * (eq. 6); Coulomb energy of the charges (eq. 8).
+ * x_dev: DEVICE.  Outputs HOST, either may be NULL.  Synchronous. */
+int pygbe_energy(pygbe_handle *h, const double *x_dev, double *E_solv_kJ_per_mol,
+                 double *E_coul_kJ_per_mol);
+
+/* phi_reac at every charge, in the caller's charge order (units e/Angstrom, i.e. before C0).
+ * phi_dev: DEVICE [n_charges].  Asynchronous. */
+int pygbe_reaction_potential(pygbe_handle *h, const double *x_dev, double *phi_dev);
+
+int pygbe_stats(const pygbe_handle *h, pygbe_stats_t *out);
+
+/* Thread-local message of the last failing call ("" if none). */
+const char *pygbe_last_error(void);
+
+/* Library / build identification, e.g. "pygbe-b200 0.1 sm_100a". */
+const char *pygbe_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PYGBE_H */

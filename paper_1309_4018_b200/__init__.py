@@ -1,0 +1,221 @@
+"""paper_1309_4018_b200 -- B200-native treecode BEM matvec / GMRES for the Poisson-Boltzmann equation.
+
+Thin Python binding of the C ABI in include/pygbe.h (same names, argument marshalling only).  All
+arithmetic runs in the CUDA kernels of libpygbe.so; PyTorch is used for device memory and streams.
+There is no CPU fallback: importing works without a GPU (so that the build and the symbol table can
+be checked), but any compute call without the library or a device raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpygbe.so")
+HEADER_PATH = os.path.join(_HERE, "..", "include", "pygbe.h")
+
+PYGBE_OK, PYGBE_EINVAL, PYGBE_ENOMEM, PYGBE_ECUDA, PYGBE_ENOCONV = 0, -1, -2, -3, -4
+PRECISION_FP64, PRECISION_MIXED = 0, 1
+
+
+class PygbeError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"pygbe error {code}: {msg}")
+        self.code = code
+
+
+class pygbe_surface(C.Structure):
+    _fields_ = [("vertices", C.POINTER(C.c_double)), ("n_vertices", C.c_int64),
+                ("triangles", C.POINTER(C.c_int32)), ("n_triangles", C.c_int64),
+                ("region_in", C.c_int32), ("region_out", C.c_int32)]
+
+
+class pygbe_charges(C.Structure):
+    _fields_ = [("xyz", C.POINTER(C.c_double)), ("q", C.POINTER(C.c_double)),
+                ("region", C.POINTER(C.c_int32)), ("n", C.c_int64)]
+
+
+class pygbe_options(C.Structure):
+    _fields_ = [("K_fine", C.c_int32), ("thres", C.c_double), ("N_k", C.c_int32), ("ncrit", C.c_int32),
+                ("precision", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p),
+                ("check_mesh", C.c_int32), ("reserved", C.c_int32 * 7)]
+
+
+class pygbe_stats_t(C.Structure):
+    _fields_ = [(n, C.c_int64) for n in (
+        "n_panels", "n_unknowns", "n_regions", "n_surfaces", "n_charges", "n_points", "n_cells", "n_leaves",
+        "n_groups", "tree_depth", "p2p_pairs", "m2p_evals", "direct_equiv", "near_nnz", "device_bytes",
+        "n_matvec", "kernels_per_matvec", "kernel_launches")] + [
+        ("create_ms", C.c_double), ("last_solve_ms", C.c_double), ("last_iters", C.c_int32),
+        ("P", C.c_int32), ("K", C.c_int32), ("precision", C.c_int32), ("theta", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libpygbe.so (built in-tree by paper_1309_4018_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: run `python -m paper_1309_4018_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int32)
+    L.pygbe_create.argtypes = [C.POINTER(pygbe_surface), C.c_int32, C.POINTER(pygbe_charges), dp, dp, C.c_int32,
+                               C.c_int32, C.c_int32, C.c_double, C.POINTER(pygbe_options), C.POINTER(vp)]
+    L.pygbe_destroy.argtypes = [vp]
+    L.pygbe_destroy.restype = None
+    L.pygbe_num_unknowns.argtypes = [vp]
+    L.pygbe_num_unknowns.restype = C.c_int64
+    L.pygbe_matvec.argtypes = [vp, vp, vp]
+    L.pygbe_matvec_host.argtypes = [vp, dp, dp]
+    L.pygbe_rhs.argtypes = [vp, vp]
+    L.pygbe_solve.argtypes = [vp, C.c_double, C.c_int32, C.c_int32, vp, ip, dp]
+    L.pygbe_solve_host.argtypes = [vp, C.c_double, C.c_int32, C.c_int32, dp, ip, dp, dp, dp]
+    L.pygbe_energy.argtypes = [vp, vp, dp, dp]
+    L.pygbe_reaction_potential.argtypes = [vp, vp, vp]
+    L.pygbe_stats.argtypes = [vp, C.POINTER(pygbe_stats_t)]
+    L.pygbe_last_error.restype = C.c_char_p
+    L.pygbe_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc, allow=()):
+    if rc != PYGBE_OK and rc not in allow:
+        raise PygbeError(rc, lib().pygbe_last_error().decode())
+    return rc
+
+
+def _dptr(t):
+    """Device pointer of a contiguous fp64 CUDA torch tensor."""
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError("expected a contiguous float64 CUDA tensor")
+    return C.c_void_p(t.data_ptr())
+
+
+class Handle:
+    """Owner of a pygbe_handle.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, surfaces, charges, eps, kappa, K=4, P=6, theta=0.5, K_fine=0, thres=0.0, N_k=0, ncrit=0,
+                 precision=PRECISION_FP64, device=0, stream=None, check_mesh=False):
+        """surfaces: list of (vertices [nv,3] f64, triangles [nt,3] i32, region_in, region_out);
+        charges: (xyz [nq,3], q [nq], region [nq] or None) or None."""
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("pygbe needs a CUDA device (there is no CPU fallback)")
+        L = lib()
+        self._keep = []
+        arr = (pygbe_surface * len(surfaces))()
+        for i, (v, t, rin, rout) in enumerate(surfaces):
+            v = np.ascontiguousarray(v, dtype=np.float64)
+            t = np.ascontiguousarray(t, dtype=np.int32)
+            self._keep += [v, t]
+            arr[i] = pygbe_surface(v.ctypes.data_as(C.POINTER(C.c_double)), v.shape[0],
+                                   t.ctypes.data_as(C.POINTER(C.c_int32)), t.shape[0], int(rin), int(rout))
+        ch = None
+        if charges is not None and len(charges[1]) > 0:
+            xyz = np.ascontiguousarray(charges[0], dtype=np.float64).reshape(-1, 3)
+            q = np.ascontiguousarray(charges[1], dtype=np.float64).reshape(-1)
+            reg = None
+            if len(charges) > 2 and charges[2] is not None:
+                reg = np.ascontiguousarray(charges[2], dtype=np.int32).reshape(-1)
+            self._keep += [xyz, q, reg]
+            ch = pygbe_charges(xyz.ctypes.data_as(C.POINTER(C.c_double)), q.ctypes.data_as(C.POINTER(C.c_double)),
+                               reg.ctypes.data_as(C.POINTER(C.c_int32)) if reg is not None else None, q.shape[0])
+        eps = np.ascontiguousarray(eps, dtype=np.float64)
+        kappa = np.ascontiguousarray(kappa, dtype=np.float64)
+        if stream is None:
+            stream = torch.cuda.current_stream(device).cuda_stream
+        opt = pygbe_options(K_fine=K_fine, thres=thres, N_k=N_k, ncrit=ncrit, precision=precision, device=device,
+                            stream=C.c_void_p(stream), check_mesh=int(check_mesh))
+        h = C.c_void_p()
+        _check(L.pygbe_create(arr, len(surfaces), C.byref(ch) if ch is not None else None,
+                              eps.ctypes.data_as(C.POINTER(C.c_double)), kappa.ctypes.data_as(C.POINTER(C.c_double)),
+                              len(eps), K, P, float(theta), C.byref(opt), C.byref(h)))
+        self._h = h
+        self.device = torch.device("cuda", device)
+        self.n = int(L.pygbe_num_unknowns(h))
+        self._keep = []
+
+    @classmethod
+    def from_problem(cls, p, **kw):
+        """Build from a workloads.Problem-like object (surfaces, eps, kappa, charge_* attributes)."""
+        surfaces = [(s.vertices, s.triangles, s.region_in, s.region_out) for s in p.surfaces]
+        return cls(surfaces, (p.charge_xyz, p.charge_q, p.charge_region), p.eps, p.kappa, **kw)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().pygbe_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def num_unknowns(self):
+        return self.n
+
+    def matvec(self, x, y=None):
+        import torch
+        if y is None:
+            y = torch.empty(self.n, dtype=torch.float64, device=self.device)
+        _check(lib().pygbe_matvec(self._h, _dptr(x), _dptr(y)))
+        return y
+
+    def matvec_host(self, x, y=None):
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        if y is None:
+            y = np.empty(self.n)
+        dp = C.POINTER(C.c_double)
+        _check(lib().pygbe_matvec_host(self._h, x.ctypes.data_as(dp), y.ctypes.data_as(dp)))
+        return y
+
+    def rhs(self, b=None):
+        import torch
+        if b is None:
+            b = torch.empty(self.n, dtype=torch.float64, device=self.device)
+        _check(lib().pygbe_rhs(self._h, _dptr(b)))
+        return b
+
+    def solve(self, tol=1e-6, restart=100, max_iter=1000, x=None, raise_on_noconv=True):
+        import torch
+        if x is None:
+            x = torch.empty(self.n, dtype=torch.float64, device=self.device)
+        it = C.c_int32(); rel = C.c_double()
+        rc = _check(lib().pygbe_solve(self._h, tol, restart, max_iter, _dptr(x), C.byref(it), C.byref(rel)),
+                    allow=() if raise_on_noconv else (PYGBE_ENOCONV,))
+        return x, it.value, rel.value, rc
+
+    def solve_host(self, tol=1e-6, restart=100, max_iter=1000, want_x=True):
+        x = np.empty(self.n) if want_x else None
+        it = C.c_int32(); rel = C.c_double(); es = C.c_double(); ec = C.c_double()
+        dp = C.POINTER(C.c_double)
+        _check(lib().pygbe_solve_host(self._h, tol, restart, max_iter, x.ctypes.data_as(dp) if want_x else None,
+                                      C.byref(it), C.byref(rel), C.byref(es), C.byref(ec)))
+        return x, it.value, rel.value, es.value, ec.value
+
+    def energy(self, x):
+        es = C.c_double(); ec = C.c_double()
+        _check(lib().pygbe_energy(self._h, _dptr(x), C.byref(es), C.byref(ec)))
+        return es.value, ec.value
+
+    def reaction_potential(self, x, n_charges):
+        import torch
+        phi = torch.empty(n_charges, dtype=torch.float64, device=self.device)
+        _check(lib().pygbe_reaction_potential(self._h, _dptr(x), _dptr(phi)))
+        return phi
+
+    def stats(self):
+        s = pygbe_stats_t()
+        _check(lib().pygbe_stats(self._h, C.byref(s)))
+        return {name: getattr(s, name) for name, _ in pygbe_stats_t._fields_}
+
+
+def pygbe_version():
+    return lib().pygbe_version().decode()

@@ -1,0 +1,71 @@
+"""Build libpygbe.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+
+    python -m paper_1309_4018_b200.build [--force]
+
+One object per translation unit, compiled in parallel: pygbe.cu (ABI + all kernels except M2P) and
+m2p_inst.cu once per expansion order P = 1..12 (the fully unrolled Taylor recurrences).
+"""
+import os
+import subprocess
+import sys
+from concurrent.futures import ThreadPoolExecutor
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
+LIB = os.path.join(HERE, "libpygbe.so")
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+         "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+PMAX = 12
+
+
+def _newest_source():
+    t = 0.0
+    for f in os.listdir(CSRC):
+        t = max(t, os.path.getmtime(os.path.join(CSRC, f)))
+    t = max(t, os.path.getmtime(os.path.join(HERE, "..", "include", "pygbe.h")))
+    return t
+
+
+def _compile(job):
+    src, obj, extra = job
+    if src.endswith("m2p_inst.cu"):
+        deps = [src, os.path.join(CSRC, "m2p.cuh")]
+    else:
+        deps = [src] + [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")]
+        deps.append(os.path.join(HERE, "..", "include", "pygbe.h"))
+    if os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(d) for d in deps):
+        return obj, ""
+    cmd = [NVCC] + FLAGS + extra + ["-c", src, "-o", obj]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed: %s\n%s" % (" ".join(cmd), r.stderr[-4000:]))
+    with open(obj + ".log", "w") as f:
+        f.write(" ".join(cmd) + "\n" + r.stderr)
+    return obj, r.stderr
+
+
+def build(force=False, verbose=False):
+    os.makedirs(OBJ, exist_ok=True)
+    if force:
+        for f in os.listdir(OBJ):
+            os.remove(os.path.join(OBJ, f))
+    jobs = [(os.path.join(CSRC, "pygbe.cu"), os.path.join(OBJ, "pygbe.o"), [])]
+    # the largest orders first: they take longest
+    for p in range(PMAX, 0, -1):
+        jobs.append((os.path.join(CSRC, "m2p_inst.cu"), os.path.join(OBJ, "m2p_%d.o" % p), ["-DM2P_P=%d" % p]))
+    with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
+        objs = [o for o, _ in ex.map(_compile, jobs)]
+    if (not os.path.exists(LIB)) or os.path.getmtime(LIB) < max(os.path.getmtime(o) for o in objs):
+        cmd = [NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("link failed: %s\n%s" % (" ".join(cmd), r.stderr[-4000:]))
+    if verbose:
+        print("built", LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    build(force="--force" in sys.argv, verbose=True)

@@ -1,0 +1,176 @@
+// common.cuh -- shared declarations of libpygbe (CUDA, sm_100a).  See include/pygbe.h for the ABI and
+// DESIGN.md for the data layout.  Paper citations are PAPER.md:<line>.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <cmath>
+#include <vector>
+#include <algorithm>
+#include <chrono>
+#include "../../include/pygbe.h"
+
+#define PYGBE_PMAX 12
+#define PYGBE_NCMAX 455              // (P+1)(P+2)(P+3)/6 at P = 12
+#define PYGBE_TG 128                 // targets per group = threads per CTA of the P2P / M2P kernels
+#define PYGBE_MAXLEVEL 21            // 21 bits per dimension in the 63-bit Morton key
+
+void pygbe_set_error(const char *fmt, ...);
+
+#define CUDA_TRY(expr)                                                                                \
+    do {                                                                                              \
+        cudaError_t e_ = (expr);                                                                      \
+        if (e_ != cudaSuccess) {                                                                      \
+            pygbe_set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #expr, cudaGetErrorString(e_));    \
+            return PYGBE_ECUDA;                                                                       \
+        }                                                                                             \
+    } while (0)
+
+#define TRY(expr)                                                                                     \
+    do {                                                                                              \
+        int rc_ = (expr);                                                                             \
+        if (rc_ != PYGBE_OK) return rc_;                                                              \
+    } while (0)
+
+// Launch bookkeeping: every kernel launch of the library goes through LAUNCH so that
+// pygbe_stats().kernel_launches is a count, not a guess.
+#define LAUNCH(h, kernel, grid, block, smem, ...)                                                     \
+    do {                                                                                              \
+        kernel<<<(grid), (block), (smem), (h)->stream>>>(__VA_ARGS__);                                \
+        (h)->launches++;                                                                              \
+    } while (0)
+
+static inline int nc_of(int P) { return (P + 1) * (P + 2) * (P + 3) / 6; }
+static inline int cdiv(long a, long b) { return (int)((a + b - 1) / b); }
+
+// ---------------------------------------------------------------------------------------------------
+// Device memory owned by a handle: a trivial arena of cudaMalloc'ed blocks, freed together.
+struct DeviceArena {
+    std::vector<void *> blocks;
+    size_t bytes = 0;
+    template <class T> int alloc(T **p, size_t n)
+    {
+        *p = nullptr;
+        if (n == 0) n = 1;
+        void *q = nullptr;
+        cudaError_t e = cudaMalloc(&q, n * sizeof(T));
+        if (e != cudaSuccess) {
+            pygbe_set_error("cudaMalloc of %zu bytes failed: %s", n * sizeof(T), cudaGetErrorString(e));
+            return PYGBE_ENOMEM;
+        }
+        blocks.push_back(q);
+        bytes += n * sizeof(T);
+        *p = (T *)q;
+        return PYGBE_OK;
+    }
+    void release_one(void *q)
+    {
+        for (size_t i = 0; i < blocks.size(); i++)
+            if (blocks[i] == q) { cudaFree(q); blocks.erase(blocks.begin() + i); return; }
+    }
+    void release()
+    {
+        for (void *q : blocks) cudaFree(q);
+        blocks.clear();
+        bytes = 0;
+    }
+};
+
+// ---------------------------------------------------------------------------------------------------
+// One region Omega of the multi-surface problem: its boundary panels are both the
+// sources (K Gauss points each) and the targets (centroids) of one N-body sum with the region's kernel.
+struct Region {
+    int id = 0;
+    double eps = 1, kappa = 0;
+    bool yukawa = false;
+    int np = 0, npts = 0;           // boundary panels, Gauss points (np * K)
+    // per panel, Morton-sorted order -------------------------------------------------------------
+    int *gid = nullptr;             // global panel id
+    int *phi_idx = nullptr, *dphi_idx = nullptr, *row_idx = nullptr;   // positions in x / y
+    double *cV = nullptr, *cK = nullptr;   // sigma_S c_S and sigma_S of the panel's surface
+    double4 *tpos = nullptr;        // collocation point (x,y,z, L = sqrt(2A))
+    double4 *pnrm = nullptr;        // unit normal (x,y,z) and area
+    // per Gauss point (K consecutive per panel) ------------------------------------------------------
+    double4 *spos = nullptr;        // (x, y, z, w_g A_j / 4pi)
+    double4 *schg = nullptr;        // per matvec: (mV, mKx, mKy, mKz)
+    float4 *sposf = nullptr;        // mixed precision: position relative to root centre? (see prep)
+    float4 *schgf = nullptr;
+    double *pphi = nullptr, *pdphi = nullptr;   // per matvec: gathered densities
+    double *out = nullptr;          // per matvec: sum_S sigma_S [c_S V dphi - K phi] at each target
+    // octree ----------------------------------------------------------------------------------------
+    unsigned long long *keys = nullptr;
+    int ncells = 0, nleaves = 0, depth = 0;
+    double4 *cgeo = nullptr;        // cell centre (x,y,z) and edge length r_b
+    int2 *crange = nullptr;         // panel range [lo, hi)
+    int2 *cchild = nullptr;         // (first child, number of children)
+    int *cparent = nullptr;
+    unsigned long long *ckey = nullptr;
+    std::vector<int> level_begin;   // host: cells of level l are [level_begin[l], level_begin[l+1])
+    int *leaf_cell = nullptr;       // leaves in Morton order
+    double Lmax = 0;                // max panel length sqrt(2A) on this region's boundary
+    double root_c[3] = {0, 0, 0}, root_edge = 1;
+    // target groups and interaction lists -----------------------------------------------------------
+    int ng = 0;
+    double4 *ggeo = nullptr;        // group centre and radius
+    int *m2p_off = nullptr, *m2p_cell = nullptr;
+    int *p2p_off = nullptr;
+    int2 *p2p_rng = nullptr;        // source panel ranges
+    int n_p2p_items = 0, n_m2p_items = 0;
+    int4 *p2p_items = nullptr;      // (group, first range, last range+1, unused) over p2p_sub
+    int2 *p2p_sub = nullptr;        // refined (chunked) panel ranges
+    int4 *m2p_items = nullptr;      // (group, first list slot, last slot+1, unused)
+    long p2p_pairs = 0, m2p_evals = 0;
+    // multipoles ------------------------------------------------------------------------------------
+    double *mom = nullptr;          // [ncells][Nc]
+    float *momf = nullptr;
+    // singular / near-singular corrections (CSR over targets) ----------------------------------------
+    int *corr_off = nullptr, *corr_col = nullptr;
+    double2 *corr_val = nullptr;    // (sigma c (fine - coarse)_V, sigma (fine - coarse)_K)
+    long corr_nnz = 0;
+    // charges of this region -------------------------------------------------------------------------
+    int nq = 0;
+    double4 *qpos = nullptr;        // (x, y, z, q)
+    int *qid = nullptr;             // caller's charge index
+};
+
+struct GmresWork {
+    int m = 0;                      // restart length the buffers were sized for
+    long n = 0;
+    double *V = nullptr;            // [(m+1)][n]
+    double *w = nullptr, *b = nullptr;
+    double *H = nullptr;            // [(m+1)][m] column-major by column j: H[j*(m+1) + i]
+    double *h1 = nullptr, *h2 = nullptr, *cs = nullptr, *sn = nullptr, *g = nullptr, *yk = nullptr;
+    double *scal = nullptr;         // [0]=bnorm [1]=beta [2]=rel [3]=nrm2 scratch
+    int *flags = nullptr;           // [0]=done [1]=k at convergence
+};
+
+struct pygbe_handle {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int K = 4, P = 6, Nc = 84, Kfine = 19, Nk = 5, ncrit = 0, precision = 0;
+    double theta = 0.5, thres = 2.0;
+    long npan = 0, nq = 0;
+    int nsurf = 0, nreg = 0;
+    std::vector<long> surf_first, surf_count;
+    std::vector<int> rin, rout;
+    std::vector<double> eps, kappa;
+    DeviceArena mem;
+    // global panel geometry (caller order)
+    double *tri = nullptr;          // [npan][9]
+    double4 *gcen = nullptr;        // centroid, L
+    double4 *gnrm = nullptr;        // normal, area
+    std::vector<Region> regions;
+    GmresWork gm;
+    double *phi_reac = nullptr;     // [nq]
+    double *scratch = nullptr;      // small device scratch (16 doubles)
+    double *xh = nullptr, *yh = nullptr;   // device staging for the *_host entry points
+    int *pinned_flags = nullptr;    // host pinned, 4 ints
+    double *pinned_scal = nullptr;  // host pinned, 8 doubles
+    std::vector<double> qxyz, qq;   // host copies of the charges
+    std::vector<int> qreg;
+    long launches = 0, n_matvec = 0, kernels_per_matvec = 0;
+    double create_ms = 0, last_solve_ms = 0;
+    int last_iters = 0;
+};

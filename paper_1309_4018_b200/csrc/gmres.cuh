@@ -1,0 +1,156 @@
+// gmres.cuh -- device-resident restarted GMRES (a11).  PAPER.md:169 "PyGBe uses a Krylov method ... one
+// evaluation of the treecode per iteration"; tolerances Tables 1, 3 (:197-203, :223-227); reading A16.
+// Arnoldi with classical Gram-Schmidt applied twice (CGS2: two batched dot passes instead of j
+// sequential ones), Givens rotations and the convergence test run in kernels; every kernel returns
+// immediately once flags[0] ("done") is set, so the host can queue iterations ahead and only polls.
+#pragma once
+#include "common.cuh"
+#include <cub/cub.cuh>
+
+#define GM_THREADS 256
+#define GM_ROWS_PER_CTA 2048
+
+// out[i] += V_i . w for i < nvec (out pre-zeroed); V row-major [nvec][n].
+__global__ void __launch_bounds__(GM_THREADS)
+k_gm_dots(const int *__restrict__ flags, const double *__restrict__ V, long n, int nvec,
+          const double *__restrict__ w, double *__restrict__ out)
+{
+    if (flags[0]) return;
+    typedef cub::BlockReduce<double, GM_THREADS> Red;
+    __shared__ typename Red::TempStorage tmp;
+    long lo = (long)blockIdx.x * GM_ROWS_PER_CTA, hi = min(n, lo + GM_ROWS_PER_CTA);
+    double wr[GM_ROWS_PER_CTA / GM_THREADS];
+#pragma unroll
+    for (int k = 0; k < GM_ROWS_PER_CTA / GM_THREADS; k++) {
+        long r = lo + threadIdx.x + (long)k * GM_THREADS;
+        wr[k] = r < hi ? w[r] : 0.0;
+    }
+    for (int i = 0; i < nvec; i++) {
+        const double *v = V + (long)i * n;
+        double acc = 0.0;
+#pragma unroll
+        for (int k = 0; k < GM_ROWS_PER_CTA / GM_THREADS; k++) {
+            long r = lo + threadIdx.x + (long)k * GM_THREADS;
+            if (r < hi) acc += v[r] * wr[k];
+        }
+        double s = Red(tmp).Sum(acc);
+        if (threadIdx.x == 0) atomicAdd(out + i, s);
+        __syncthreads();
+    }
+}
+
+// w -= sum_i h[i] V_i
+__global__ void __launch_bounds__(GM_THREADS)
+k_gm_axpys(const int *__restrict__ flags, const double *__restrict__ V, long n, int nvec,
+           const double *__restrict__ h, double *__restrict__ w)
+{
+    if (flags[0]) return;
+    long r = (long)blockIdx.x * GM_THREADS + threadIdx.x;
+    if (r >= n) return;
+    double acc = w[r];
+    for (int i = 0; i < nvec; i++) acc -= h[i] * V[(long)i * n + r];
+    w[r] = acc;
+}
+
+__global__ void k_gm_zero(const int *__restrict__ flags, double *a, int na, double *b, int nb, double *c, int nc)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < na) a[i] = 0.0;
+    if (i < nb) b[i] = 0.0;
+    if (i < nc) c[i] = 0.0;
+}
+
+// Start of a cycle: r = b - w (w = A x, or 0 on the first cycle); beta^2 accumulated in scal[3].
+__global__ void __launch_bounds__(GM_THREADS)
+k_gm_residual(const int *__restrict__ flags, long n, const double *__restrict__ b, const double *__restrict__ w,
+              int use_w, double *__restrict__ r, double *__restrict__ scal)
+{
+    if (flags[0]) return;
+    typedef cub::BlockReduce<double, GM_THREADS> Red;
+    __shared__ typename Red::TempStorage tmp;
+    long i = (long)blockIdx.x * GM_THREADS + threadIdx.x;
+    double v = 0.0;
+    if (i < n) { v = b[i] - (use_w ? w[i] : 0.0); r[i] = v; }
+    double s = Red(tmp).Sum(v * v);
+    if (threadIdx.x == 0) atomicAdd(scal + 3, s);
+}
+
+// beta = sqrt(scal[3]); first cycle: bnorm = beta.  g = beta e_0; done if beta/bnorm <= tol.
+__global__ void k_gm_begin(int *flags, double *scal, double *g, int m, int first, double tol)
+{
+    if (flags[0]) return;
+    double beta = sqrt(scal[3]);
+    if (first) scal[0] = beta;
+    scal[1] = beta;
+    double bn = scal[0];
+    scal[2] = bn > 0.0 ? beta / bn : 0.0;
+    for (int i = 0; i <= m; i++) g[i] = 0.0;
+    g[0] = beta;
+    if (bn == 0.0 || beta / bn <= tol) { flags[0] = 1; flags[1] = 0; }
+    scal[3] = 0.0;
+}
+
+// dst = src * (1/s) with s = sqrt(*s2) if is_sq else *s2
+__global__ void __launch_bounds__(GM_THREADS)
+k_gm_scale(const int *__restrict__ flags, long n, const double *__restrict__ src, const double *__restrict__ s2,
+           int is_sq, double *__restrict__ dst)
+{
+    if (flags[0]) return;
+    long i = (long)blockIdx.x * GM_THREADS + threadIdx.x;
+    if (i >= n) return;
+    double s = is_sq ? sqrt(*s2) : *s2;
+    dst[i] = s > 0.0 ? src[i] / s : 0.0;
+}
+
+// Column j of the Hessenberg matrix: H[0..j][j] = h1 + h2, H[j+1][j] = sqrt(nrm2); apply the previous
+// rotations, form the new one, update g; rel = |g[j+1]| / bnorm; raise done when rel <= tol.
+__global__ void k_gm_givens(int *flags, int j, int m, const double *__restrict__ h1, const double *__restrict__ h2,
+                            const double *__restrict__ nrm2, double *H, double *cs, double *sn, double *g,
+                            double *scal, double tol)
+{
+    if (flags[0]) return;
+    double *col = H + (long)j * (m + 1);
+    for (int i = 0; i <= j; i++) col[i] = h1[i] + h2[i];
+    col[j + 1] = sqrt(*nrm2);
+    for (int i = 0; i < j; i++) {
+        double t = cs[i] * col[i] + sn[i] * col[i + 1];
+        col[i + 1] = -sn[i] * col[i] + cs[i] * col[i + 1];
+        col[i] = t;
+    }
+    double d = hypot(col[j], col[j + 1]);
+    double c = d > 0.0 ? col[j] / d : 1.0, s = d > 0.0 ? col[j + 1] / d : 0.0;
+    cs[j] = c; sn[j] = s;
+    col[j] = d; col[j + 1] = 0.0;
+    g[j + 1] = -s * g[j];
+    g[j] = c * g[j];
+    double rel = fabs(g[j + 1]) / scal[0];
+    scal[2] = rel;
+    flags[1] = j + 1;
+    flags[2] += 1;                       // total iterations
+    if (rel <= tol) flags[0] = 1;
+}
+
+// Back substitution R y = g for the k = flags[1] columns built in this cycle (single thread, k <= m).
+__global__ void k_gm_solve_small(const int *__restrict__ flags, int m, const double *__restrict__ H,
+                                 const double *__restrict__ g, double *__restrict__ yk)
+{
+    int k = flags[1];
+    for (int i = k - 1; i >= 0; i--) {
+        double s = g[i];
+        for (int c = i + 1; c < k; c++) s -= H[(long)c * (m + 1) + i] * yk[c];
+        yk[i] = s / H[(long)i * (m + 1) + i];
+    }
+}
+
+// x += sum_{i < k} yk[i] V_i
+__global__ void __launch_bounds__(GM_THREADS)
+k_gm_update(const int *__restrict__ flags, long n, const double *__restrict__ V, const double *__restrict__ yk,
+            double *__restrict__ x)
+{
+    long r = (long)blockIdx.x * GM_THREADS + threadIdx.x;
+    if (r >= n) return;
+    int k = flags[1];
+    double acc = x[r];
+    for (int i = 0; i < k; i++) acc += yk[i] * V[(long)i * n + r];
+    x[r] = acc;
+}

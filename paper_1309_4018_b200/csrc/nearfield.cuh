@@ -1,0 +1,343 @@
+// nearfield.cuh -- direct interactions: P2P (a7), singular / near-singular corrections (a8), density
+// weighting and block combination (a9), right-hand side (a10), reaction potential (a12).
+#pragma once
+#include "common.cuh"
+#include "tables.cuh"
+#include <cub/cub.cuh>
+
+// One (target, Gauss point) interaction with the region's kernel, both layers at once (eq. 2 / 9,
+// PAPER.md:55-58, :98):   mV G(r) - mK . grad_y G,   G = exp(-kappa r)/r   (1/(4 pi) is in the weights),
+//   grad_y G = d (1 + kappa r) exp(-kappa r) / r^3,  d = x - y.
+// A pair at zero distance (the K = 4 rule has a node at the collocation point of the self panel,
+// reading A5) contributes nothing here; the self panel is handled by the correction (a8).
+template <bool YUKAWA>
+__device__ __forceinline__ double pair_f64(double dx, double dy, double dz, double mV, double mKx, double mKy,
+                                           double mKz, double kappa)
+{
+    double r2 = dx * dx + dy * dy + dz * dz;
+    double rinv = r2 > 0.0 ? rsqrt(r2) : 0.0;
+    double mKd = mKx * dx + mKy * dy + mKz * dz;
+    double rinv2 = rinv * rinv;
+    if (!YUKAWA) {
+        return (mV - mKd * rinv2) * rinv;
+    } else {
+        double kr = kappa * (r2 * rinv);
+        double e = exp(-kr);
+        return (mV - mKd * (1.0 + kr) * rinv2) * (rinv * e);
+    }
+}
+
+template <bool YUKAWA>
+__device__ __forceinline__ float pair_f32(float dx, float dy, float dz, float mV, float mKx, float mKy,
+                                          float mKz, float kappa_log2e, float kappa)
+{
+    float r2 = dx * dx + dy * dy + dz * dz;
+    float rinv = r2 > 0.0f ? rsqrtf(r2) : 0.0f;
+    float mKd = mKx * dx + mKy * dy + mKz * dz;
+    float rinv2 = rinv * rinv;
+    if (!YUKAWA) {
+        return (mV - mKd * rinv2) * rinv;
+    } else {
+        float r = r2 * rinv;
+        float e = exp2f(-kappa_log2e * r);
+        return (mV - mKd * fmaf(kappa, r, 1.0f) * rinv2) * (rinv * e);
+    }
+}
+
+// ------------------------------------------------------------------------------- per-matvec weighting
+// Gather the densities of the region's panels from x and turn them into point "charges":
+//   mV_g = w_g A_j/(4pi) sigma_S c_S dphi_j,   mK_g = w_g A_j/(4pi) sigma_S phi_j n_j     (reading A4)
+// and clear the accumulator.
+__global__ void k_prep(const int *__restrict__ skip, int np, int K, const double *__restrict__ x, const int *__restrict__ phi_idx,
+                       const int *__restrict__ dphi_idx, const double *__restrict__ cV,
+                       const double *__restrict__ cK, const double4 *__restrict__ pnrm,
+                       const double4 *__restrict__ spos, double4 *__restrict__ schg,
+                       float4 *__restrict__ schgf, double *__restrict__ pphi, double *__restrict__ pdphi,
+                       double *__restrict__ out)
+{
+    if (skip && *skip) return;
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    double phi = x[phi_idx[p]], dphi = x[dphi_idx[p]];
+    pphi[p] = phi; pdphi[p] = dphi;
+    out[p] = 0.0;
+    double qV = cV[p] * dphi, qK = cK[p] * phi;
+    double4 n = pnrm[p];
+    for (int g = 0; g < K; g++) {
+        double w = spos[(long)p * K + g].w;
+        double4 c = make_double4(w * qV, w * qK * n.x, w * qK * n.y, w * qK * n.z);
+        schg[(long)p * K + g] = c;
+        if (schgf) schgf[(long)p * K + g] = make_float4((float)c.x, (float)c.y, (float)c.z, (float)c.w);
+    }
+}
+
+// Row of region Omega collocated on the panel (eq. 10):  y = 1/2 phi - out.
+__global__ void k_combine(const int *__restrict__ skip, int np, const int *__restrict__ row_idx, const double *__restrict__ pphi,
+                          const double *__restrict__ out, double *__restrict__ y)
+{
+    if (skip && *skip) return;
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    y[row_idx[p]] = 0.5 * pphi[p] - out[p];
+}
+
+// ------------------------------------------------------------------------------------------ P2P fp64
+// Work item = (target group, a run of chunked source panel ranges).  One thread per target; source points
+// are staged through shared memory in tiles (both double4 streams: position+weight, charges).
+#define P2P_TILE 256
+template <bool YUKAWA>
+__global__ void __launch_bounds__(PYGBE_TG)
+k_p2p_f64(const int *__restrict__ skip, const int4 *__restrict__ items, const int2 *__restrict__ sub, int K, int np,
+          const double4 *__restrict__ tpos, const double4 *__restrict__ spos,
+          const double4 *__restrict__ schg, double kappa, double *__restrict__ out)
+{
+    __shared__ double4 s_pos[P2P_TILE];
+    __shared__ double4 s_chg[P2P_TILE];
+    if (skip && *skip) return;
+    const int4 it = items[blockIdx.x];
+    const int t = it.x * PYGBE_TG + threadIdx.x;
+    const bool ok = t < np;
+    double4 X = ok ? tpos[t] : make_double4(0, 0, 0, 0);
+    double acc0 = 0.0, acc1 = 0.0;
+    for (int r = it.y; r < it.z; r++) {
+        int2 rg = sub[r];
+        long p0 = (long)rg.x * K, p1 = (long)rg.y * K;
+        for (long base = p0; base < p1; base += P2P_TILE) {
+            int n = (int)min((long)P2P_TILE, p1 - base);
+            __syncthreads();
+            for (int i = threadIdx.x; i < n; i += PYGBE_TG) {
+                s_pos[i] = spos[base + i];
+                s_chg[i] = schg[base + i];
+            }
+            __syncthreads();
+            int i = 0;
+            for (; i + 1 < n; i += 2) {
+                double4 a = s_pos[i], c = s_chg[i];
+                double4 a2 = s_pos[i + 1], c2 = s_chg[i + 1];
+                acc0 += pair_f64<YUKAWA>(X.x - a.x, X.y - a.y, X.z - a.z, c.x, c.y, c.z, c.w, kappa);
+                acc1 += pair_f64<YUKAWA>(X.x - a2.x, X.y - a2.y, X.z - a2.z, c2.x, c2.y, c2.z, c2.w, kappa);
+            }
+            if (i < n) {
+                double4 a = s_pos[i], c = s_chg[i];
+                acc0 += pair_f64<YUKAWA>(X.x - a.x, X.y - a.y, X.z - a.z, c.x, c.y, c.z, c.w, kappa);
+            }
+        }
+    }
+    if (ok) atomicAdd(out + t, acc0 + acc1);
+}
+
+// ------------------------------------------------------------------- singular / near-singular panels
+// Step 1: for each target, find the source panels of its group's P2P ranges that are the target's own
+// panel or lie inside the near-singular region |x_i - c_j|^2 < thres^2 * 2 A_j  (
+// reading A7).  fill == 0 counts, fill == 1 writes column indices (ascending).
+__global__ void __launch_bounds__(PYGBE_TG)
+k_near_find(int np, const double4 *__restrict__ tpos, const double4 *__restrict__ pnrm,
+            const int *__restrict__ p2p_off,
+            const int2 *__restrict__ p2p_rng, double thres2, int fill, int *__restrict__ cnt,
+            const int *__restrict__ off, int *__restrict__ col)
+{
+    int g = blockIdx.x;
+    int t = g * PYGBE_TG + threadIdx.x;
+    if (t >= np) return;
+    double4 X = tpos[t];
+    int n = 0;
+    int base = fill ? off[t] : 0;
+    for (int r = p2p_off[g]; r < p2p_off[g + 1]; r++) {
+        int2 rg = p2p_rng[r];
+        for (int j = rg.x; j < rg.y; j++) {
+            double4 c = tpos[j];
+            double dx = X.x - c.x, dy = X.y - c.y, dz = X.z - c.z;
+            bool near = (j == t) || (thres2 > 0.0 && dx * dx + dy * dy + dz * dz < thres2 * 2.0 * pnrm[j].w);
+            if (near) {
+                if (fill) col[base + n] = j;
+                n++;
+            }
+        }
+    }
+    if (!fill) cnt[t] = n;
+}
+
+// Semi-analytic self integral of the single-layer kernel (PAPER.md:165 [22], :235 "N_k"; reading A6):
+// polar coordinates about the centroid in the panel plane, radial integral analytic
+//   int_0^R exp(-kappa r) dr = R  or  (1 - exp(-kappa R))/kappa,   R(theta) = h / cos(theta),
+// angular integral by N_k-point Gauss-Legendre on each side's angular interval.  Without 1/(4 pi).
+__device__ double self_integral(const double *t, double kappa, const QuadTables &q)
+{
+    double c[3] = {(t[0] + t[3] + t[6]) / 3.0, (t[1] + t[4] + t[7]) / 3.0, (t[2] + t[5] + t[8]) / 3.0};
+    double total = 0.0;
+    for (int s = 0; s < 3; s++) {
+        const double *a = t + 3 * s, *b = t + 3 * ((s + 1) % 3);
+        double e[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]};
+        double len = sqrt(e[0] * e[0] + e[1] * e[1] + e[2] * e[2]);
+        e[0] /= len; e[1] /= len; e[2] /= len;
+        double ac[3] = {a[0] - c[0], a[1] - c[1], a[2] - c[2]};
+        double sa = ac[0] * e[0] + ac[1] * e[1] + ac[2] * e[2];
+        double sb = sa + len;
+        double px = ac[0] - sa * e[0], py = ac[1] - sa * e[1], pz = ac[2] - sa * e[2];
+        double h = sqrt(px * px + py * py + pz * pz);
+        double th1 = atan2(sa, h), th2 = atan2(sb, h);
+        double half = 0.5 * (th2 - th1), mid = 0.5 * (th2 + th1), acc = 0.0;
+        for (int k = 0; k < q.Nk; k++) {
+            double R = h / cos(mid + half * q.glx[k]);
+            acc += q.glw[k] * (kappa == 0.0 ? R : (1.0 - exp(-kappa * R)) / kappa);
+        }
+        total += half * acc;
+    }
+    return total;
+}
+
+// Step 2: value of each correction entry = (fine rule or semi-analytic) - (what P2P adds with the K-point
+// rule), for the single- and the double-layer kernel, with sigma_S c_S / sigma_S of the source panel
+// folded in.  One thread per entry.  Self panel: V = semi-analytic, K = 0 (flat panel).
+__global__ void k_near_values(int np, QuadTables q, bool yukawa, double kappa, const int *__restrict__ off,
+                              const int *__restrict__ col, const int *__restrict__ gid,
+                              const double *__restrict__ tri, const double4 *__restrict__ tpos,
+                              const double4 *__restrict__ pnrm, const double4 *__restrict__ spos,
+                              const double *__restrict__ cV, const double *__restrict__ cK,
+                              double2 *__restrict__ val)
+{
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= np) return;
+    double4 X = tpos[t];
+    const double inv4pi = 0.07957747154594767;
+    for (int e = off[t]; e < off[t + 1]; e++) {
+        int j = col[e];
+        double4 nA = pnrm[j];
+        // coarse part, exactly as k_p2p evaluates it (unit densities)
+        double cv = 0.0, ck = 0.0;
+        for (int g = 0; g < q.K; g++) {
+            double4 a = spos[(long)j * q.K + g];
+            double dx = X.x - a.x, dy = X.y - a.y, dz = X.z - a.z;
+            if (yukawa) {
+                cv += pair_f64<true>(dx, dy, dz, a.w, 0, 0, 0, kappa);
+                ck -= pair_f64<true>(dx, dy, dz, 0, a.w * nA.x, a.w * nA.y, a.w * nA.z, kappa);
+            } else {
+                cv += pair_f64<false>(dx, dy, dz, a.w, 0, 0, 0, kappa);
+                ck -= pair_f64<false>(dx, dy, dz, 0, a.w * nA.x, a.w * nA.y, a.w * nA.z, kappa);
+            }
+        }
+        const double *tj = tri + 9 * (long)gid[j];
+        double fv = 0.0, fk = 0.0;
+        if (j == t) {
+            fv = self_integral(tj, kappa, q) * inv4pi;
+            fk = 0.0;
+        } else {
+            for (int g = 0; g < q.Kfine; g++) {
+                double b0 = q.bF[g][0], b1 = q.bF[g][1], b2 = q.bF[g][2];
+                double yx = b0 * tj[0] + b1 * tj[3] + b2 * tj[6];
+                double yy = b0 * tj[1] + b1 * tj[4] + b2 * tj[7];
+                double yz = b0 * tj[2] + b1 * tj[5] + b2 * tj[8];
+                double w = q.wF[g] * nA.w * inv4pi;
+                double dx = X.x - yx, dy = X.y - yy, dz = X.z - yz;
+                if (yukawa) {
+                    fv += pair_f64<true>(dx, dy, dz, w, 0, 0, 0, kappa);
+                    fk -= pair_f64<true>(dx, dy, dz, 0, w * nA.x, w * nA.y, w * nA.z, kappa);
+                } else {
+                    fv += pair_f64<false>(dx, dy, dz, w, 0, 0, 0, kappa);
+                    fk -= pair_f64<false>(dx, dy, dz, 0, w * nA.x, w * nA.y, w * nA.z, kappa);
+                }
+            }
+        }
+        val[e] = make_double2(cV[j] * (fv - cv), cK[j] * (fk - ck));
+    }
+}
+
+// Per-matvec application: out_i += sum_e [ val.x dphi_j - val.y phi_j ]  (CSR SpMV, fp64 always).
+__global__ void k_near_apply(const int *__restrict__ skip, int np, const int *__restrict__ off, const int *__restrict__ col,
+                             const double2 *__restrict__ val, const double *__restrict__ pphi,
+                             const double *__restrict__ pdphi, double *__restrict__ out)
+{
+    if (skip && *skip) return;
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= np) return;
+    double acc = 0.0;
+    for (int e = off[t]; e < off[t + 1]; e++) {
+        int j = col[e];
+        double2 v = val[e];
+        acc += v.x * pdphi[j] - v.y * pphi[j];
+    }
+    out[t] += acc;
+}
+
+// ------------------------------------------------------------------------------------------------ RHS
+// b[row(Omega,T,i)] = sum_{k in Omega} q_k G_Omega(x_i, r_k) / eps_Omega   (eq. 9 / 11).
+#define RHS_TILE 256
+template <bool YUKAWA>
+__global__ void __launch_bounds__(128)
+k_rhs(int np, const double4 *__restrict__ tpos, const int *__restrict__ row_idx, int nq,
+      const double4 *__restrict__ qpos, double kappa, double inv_eps_4pi, double *__restrict__ b)
+{
+    __shared__ double4 s_q[RHS_TILE];
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    bool ok = t < np;
+    double4 X = ok ? tpos[t] : make_double4(0, 0, 0, 0);
+    double acc = 0.0;
+    for (int base = 0; base < nq; base += RHS_TILE) {
+        int n = min(RHS_TILE, nq - base);
+        __syncthreads();
+        for (int i = threadIdx.x; i < n; i += blockDim.x) s_q[i] = qpos[base + i];
+        __syncthreads();
+        for (int i = 0; i < n; i++) {
+            double4 a = s_q[i];
+            acc += pair_f64<YUKAWA>(X.x - a.x, X.y - a.y, X.z - a.z, a.w, 0, 0, 0, kappa);
+        }
+    }
+    if (ok) b[row_idx[t]] = acc * inv_eps_4pi;
+}
+
+// ------------------------------------------------------------------------------- reaction potential
+// phi_reac(r_k) = sum_{S in dOmega} sigma_S [ c_S V dphi_S - K phi_S ](r_k)  with the plain K-point rule
+// (eq. 4; discretised :119).  The point charges schg come from k_prep with the solution.
+// grid = (source chunks, charges); block reduce, one atomicAdd per CTA.
+#define EN_THREADS 256
+#define EN_CHUNK 4096
+template <bool YUKAWA>
+__global__ void __launch_bounds__(EN_THREADS)
+k_reaction(int npts, const double4 *__restrict__ spos, const double4 *__restrict__ schg, int nq,
+           const double4 *__restrict__ qpos, const int *__restrict__ qid, double kappa,
+           double *__restrict__ phi_reac)
+{
+    typedef cub::BlockReduce<double, EN_THREADS> Red;
+    __shared__ typename Red::TempStorage tmp;
+    int k = blockIdx.y;
+    double4 X = qpos[k];
+    long lo = (long)blockIdx.x * EN_CHUNK, hi = min((long)npts, lo + EN_CHUNK);
+    double acc = 0.0;
+    for (long i = lo + threadIdx.x; i < hi; i += EN_THREADS) {
+        double4 a = spos[i], c = schg[i];
+        acc += pair_f64<YUKAWA>(X.x - a.x, X.y - a.y, X.z - a.z, c.x, c.y, c.z, c.w, kappa);
+    }
+    double s = Red(tmp).Sum(acc);
+    if (threadIdx.x == 0) atomicAdd(phi_reac + qid[k], s);
+}
+
+// sum_k q_k phi_reac[k] (eq. 6) -> out[0]; single CTA.
+__global__ void __launch_bounds__(256) k_dot_q(int nq, const double *__restrict__ q,
+                                               const double *__restrict__ phi, double *__restrict__ out)
+{
+    typedef cub::BlockReduce<double, 256> Red;
+    __shared__ typename Red::TempStorage tmp;
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < nq; i += 256) acc += q[i] * phi[i];
+    double s = Red(tmp).Sum(acc);
+    if (threadIdx.x == 0) out[0] = s;
+}
+
+// Coulomb energy sum over pairs inside one region (eq. 8): sum_{k != l} q_k q_l / r_kl.
+__global__ void __launch_bounds__(128) k_coulomb(int nq, const double4 *__restrict__ qpos, double *__restrict__ out)
+{
+    typedef cub::BlockReduce<double, 128> Red;
+    __shared__ typename Red::TempStorage tmp;
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    double acc = 0.0;
+    if (k < nq) {
+        double4 X = qpos[k];
+        for (int l = 0; l < nq; l++) {
+            double4 a = qpos[l];
+            acc += pair_f64<false>(X.x - a.x, X.y - a.y, X.z - a.z, a.w, 0, 0, 0, 0.0);   // r = 0 -> 0
+        }
+        acc *= X.w;
+    }
+    double s = Red(tmp).Sum(acc);
+    if (threadIdx.x == 0) atomicAdd(out, s);
+}

@@ -1,0 +1,144 @@
+// tables.cuh -- quadrature rules (host side, handed to kernels by value) and the multi-index tables of
+// the Cartesian Taylor expansion (constant memory, valid for every P <= PYGBE_PMAX).
+#pragma once
+#include "common.cuh"
+
+// Gauss rules on the triangle in barycentric coordinates, weights summing to 1 ("Gauss
+// quadrature"; K in Tables 1, 3 :197-225; K_fine = 19 in Tables 4, 6 :237-278).  The paper prints no
+// rule; readings A5 (K = 1, 3, 4, 7) and A7b (19-point degree-9 rule).
+struct QuadTables {
+    int K, Kfine, Nk;
+    double bK[7][3], wK[7];
+    double bF[19][3], wF[19];
+    double glx[64], glw[64];        // Gauss-Legendre on [-1,1] for the semi-analytic self integral
+};
+
+static void orbit3(double (*b)[3], double *w, int &at, double a, double wt)
+{
+    double r = 0.5 * (1.0 - a);
+    for (int k = 0; k < 3; k++) {
+        b[at][0] = b[at][1] = b[at][2] = r;
+        b[at][k] = a;
+        w[at++] = wt;
+    }
+}
+static void orbit6(double (*b)[3], double *w, int &at, double a, double bb, double c, double wt)
+{
+    const double v[3] = {a, bb, c};
+    const int perm[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
+    for (int k = 0; k < 6; k++) {
+        for (int i = 0; i < 3; i++) b[at][i] = v[perm[k][i]];
+        w[at++] = wt;
+    }
+}
+
+static int fill_triangle_rule(int K, double (*b)[3], double *w)
+{
+    int at = 0;
+    const double t = 1.0 / 3.0;
+    if (K == 1) {
+        b[0][0] = b[0][1] = b[0][2] = t; w[0] = 1.0;
+    } else if (K == 3) {
+        orbit3(b, w, at, 2.0 / 3.0, t);
+    } else if (K == 4) {
+        b[0][0] = b[0][1] = b[0][2] = t; w[0] = -27.0 / 48.0; at = 1;
+        orbit3(b, w, at, 0.6, 25.0 / 48.0);
+    } else if (K == 7) {
+        const double s = std::sqrt(15.0);
+        b[0][0] = b[0][1] = b[0][2] = t; w[0] = 9.0 / 40.0; at = 1;
+        orbit3(b, w, at, 1.0 - 2.0 * (6.0 - s) / 21.0, (155.0 - s) / 1200.0);
+        orbit3(b, w, at, 1.0 - 2.0 * (6.0 + s) / 21.0, (155.0 + s) / 1200.0);
+    } else if (K == 19) {
+        b[0][0] = b[0][1] = b[0][2] = t; w[0] = 0.0971357962827988; at = 1;
+        orbit3(b, w, at, 0.9105409732110946, 0.0255776756586980);
+        orbit3(b, w, at, 0.0206349616025247, 0.0313347002271391);
+        orbit3(b, w, at, 0.1258208170141267, 0.0778275410047743);
+        orbit3(b, w, at, 0.6235929287619345, 0.0796477389272102);
+        orbit6(b, w, at, 0.2219629891607657, 0.0368384120547363, 0.7411985987844980, 0.0432835393772894);
+    } else {
+        return PYGBE_EINVAL;
+    }
+    return PYGBE_OK;
+}
+
+static void fill_gauss_legendre(int N, double *x, double *w)
+{
+    // roots of P_N by Newton from the Chebyshev guess; standard three-term recurrence
+    const double pi = 3.14159265358979323846;
+    for (int i = 0; i < N; i++) {
+        double z = std::cos(pi * (i + 0.75) / (N + 0.5)), dp = 1.0;
+        for (int it = 0; it < 100; it++) {
+            double p0 = 1.0, p1 = z;
+            for (int k = 2; k <= N; k++) {
+                double p2 = ((2.0 * k - 1.0) * z * p1 - (k - 1.0) * p0) / k;
+                p0 = p1; p1 = p2;
+            }
+            if (N == 1) { p0 = 1.0; p1 = z; }
+            dp = N * (z * p1 - p0) / (z * z - 1.0);
+            double dz = p1 / dp;
+            z -= dz;
+            if (std::fabs(dz) < 1e-16) break;
+        }
+        x[i] = z;
+        w[i] = 2.0 / ((1.0 - z * z) * dp * dp);
+    }
+}
+
+static int make_quad_tables(int K, int Kfine, int Nk, QuadTables *q)
+{
+    memset(q, 0, sizeof(*q));
+    if (!(K == 1 || K == 3 || K == 4 || K == 7)) {
+        pygbe_set_error("K = %d: supported Gauss rules are 1, 3, 4, 7", K);
+        return PYGBE_EINVAL;
+    }
+    if (!(Kfine == 1 || Kfine == 3 || Kfine == 4 || Kfine == 7 || Kfine == 19)) {
+        pygbe_set_error("K_fine = %d: supported rules are 1, 3, 4, 7, 19", Kfine);
+        return PYGBE_EINVAL;
+    }
+    if (Nk < 1 || Nk > 64) {
+        pygbe_set_error("N_k = %d out of range 1..64", Nk);
+        return PYGBE_EINVAL;
+    }
+    q->K = K; q->Kfine = Kfine; q->Nk = Nk;
+    fill_triangle_rule(K, q->bK, q->wK);
+    fill_triangle_rule(Kfine, q->bF, q->wF);
+    fill_gauss_legendre(Nk, q->glx, q->glw);
+    return PYGBE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Multi-index tables.  Canonical order of the coefficients k = (kx,ky,kz), |k| <= P: by total order n,
+// then kx descending, then ky descending.  The first Nc(P') entries are the set for any P' <= PMAX.
+__constant__ unsigned char c_kxyz[PYGBE_NCMAX][4];                              // kx, ky, kz, n
+__constant__ short c_idx3[PYGBE_PMAX + 1][PYGBE_PMAX + 1][PYGBE_PMAX + 1];       // -> canonical index
+__constant__ double c_binom[PYGBE_PMAX + 1][PYGBE_PMAX + 1];
+
+static int upload_index_tables()
+{
+    static bool done[64] = {false};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev >= 0 && dev < 64 && done[dev]) return PYGBE_OK;
+    static unsigned char kxyz[PYGBE_NCMAX][4];
+    static short idx3[PYGBE_PMAX + 1][PYGBE_PMAX + 1][PYGBE_PMAX + 1];
+    static double binom[PYGBE_PMAX + 1][PYGBE_PMAX + 1];
+    memset(idx3, 0xff, sizeof(idx3));
+    int at = 0;
+    for (int n = 0; n <= PYGBE_PMAX; n++)
+        for (int kx = n; kx >= 0; kx--)
+            for (int ky = n - kx; ky >= 0; ky--) {
+                int kz = n - kx - ky;
+                kxyz[at][0] = kx; kxyz[at][1] = ky; kxyz[at][2] = kz; kxyz[at][3] = n;
+                idx3[kx][ky][kz] = (short)at++;
+            }
+    for (int n = 0; n <= PYGBE_PMAX; n++)
+        for (int m = 0; m <= PYGBE_PMAX; m++) {
+            if (m > n) { binom[n][m] = 0; continue; }
+            binom[n][m] = (m == 0 || m == n) ? 1.0 : binom[n - 1][m - 1] + binom[n - 1][m];
+        }
+    CUDA_TRY(cudaMemcpyToSymbol(c_kxyz, kxyz, sizeof(kxyz)));
+    CUDA_TRY(cudaMemcpyToSymbol(c_idx3, idx3, sizeof(idx3)));
+    CUDA_TRY(cudaMemcpyToSymbol(c_binom, binom, sizeof(binom)));
+    if (dev >= 0 && dev < 64) done[dev] = true;
+    return PYGBE_OK;
+}
