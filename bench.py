@@ -1,0 +1,297 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the treecode BEM matvec (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config kirkwood_l5]
+                    [--precision fp64|mixed]
+
+A step = one matvec y = A x (the hot loop of PAPER.md:169: "one evaluation of the treecode per iteration")
+of the whole coupled system: density weighting, P2M, upward pass, M2P, P2P, near-field corrections and
+block combination for every region.  value = direct-equivalent interactions per second
+(sum_regions N_targets x N_gauss_points per matvec) with x and y resident in HBM; e2e = the
+same through pygbe_matvec_host (pinned host buffers, copies inside the timed region).  The second half of
+the metric, GMRES time-to-solution, is reported under "solve" (create + rhs + GMRES + energy).
+L2 is flushed between timed iterations.  Multi-GPU: independent replicas of the workload, one per rank
+("replicas only"), no data-path collective.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "BEM matvec interactions/s (Laplace+Yukawa), direct-equivalent"
+UNIT = "interactions/s"
+
+
+def make_problem(name):
+    import workloads as W
+    if name == "kirkwood_l5":
+        return W.kirkwood_problem(5), dict(K=4, P=6, theta=0.5), "BASELINE.json configs[1]: Kirkwood sphere R=10 A, icosphere level 5 (20480 panels), K=4, P=6, theta=0.5"
+    if name == "born_l3":
+        return W.born_problem(3), dict(K=4, P=6, theta=0.0), "BASELINE.json configs[0]: Born sphere, 1280 panels, direct"
+    if name == "kirkwood_l6":
+        return W.kirkwood_problem(6), dict(K=4, P=6, theta=0.5), "Kirkwood sphere level 6 (81920 panels), K=4, P=6, theta=0.5"
+    raise SystemExit(f"unknown config {name}")
+
+
+# ------------------------------------------------------------------------------------------ flop model
+def m2p_flops(P, yukawa):
+    """Algorithmic flops of one (target, cell) Taylor evaluation: the recurrence of reading A13 term by
+    term (multiply-add = 2) plus the contraction with the moments.  DESIGN.md 'Flop model'."""
+    f = 3 + 5 + 2 + (3 if yukawa else 0) + 1          # d, R^2, 1/R^2 & 1/R, [exp, kR, *], a0*M0
+    for n in range(1, P + 1):
+        f += 4 if not yukawa else 6                    # c1..c4
+        for kx in range(n, -1, -1):
+            for ky in range(n - kx, -1, -1):
+                kz = n - kx - ky
+                n1 = sum(1 for k in (kx, ky, kz) if k > 0)
+                n2 = sum(1 for k in (kx, ky, kz) if k > 1)
+                s = (2 * n1 - 1) + max(n2 - 1, 0)      # s1 (mul+add chain), s2 (adds)
+                f += s + 3 + 2                         # v = c1 s1 - c2 s2 ; acc += v M
+                if yukawa:
+                    f += s + 2 + 3                     # t1, t2 ; b = c3 (s1 - s2) ; v += c4 (t1 - t2)
+    return f
+
+
+P2P_FLOPS = {False: 19, True: 25}     # per (target, Gauss point) pair, Laplace / Yukawa (rsqrt, exp = 1)
+
+
+def clocks_sampler(stop, out):
+    q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+    while not stop.is_set():
+        try:
+            r = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i",
+                                os.environ.get("LOCAL_RANK", "0")], capture_output=True, text=True, timeout=5)
+            out.append([c.strip() for c in r.stdout.strip().split(",")])
+        except Exception:
+            pass
+        stop.wait(0.2)
+
+
+def summarize_clocks(samples):
+    sm = [float(s[0]) for s in samples if len(s) >= 7 and s[0].replace(".", "").isdigit()]
+    mx = [float(s[1]) for s in samples if len(s) >= 7 and s[1].replace(".", "").isdigit()]
+    reasons = []
+    for i, name in enumerate(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")):
+        if any(len(s) >= 7 and s[3 + i].lower().startswith("active") for s in samples):
+            reasons.append(name)
+    return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+            "reasons": reasons, "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------- reference arm
+def oracle_sample(prob, kw, seconds_target=15.0):
+    """Time the oracle (as it stands, all host cores through its own OpenMP loop) on a bounded sample of
+    rows of the same matvec; returns (interactions/s, cores, description, seconds)."""
+    import oracle
+    o = oracle.Oracle(prob, K=kw["K"])
+    rng = np.random.default_rng(42)
+    x = rng.normal(size=o.n)
+    per_row = o.npan * kw["K"]                      # single-surface configs: every row sees all points
+    probe = np.sort(rng.choice(o.n, 64, replace=False))
+    t = time.perf_counter(); o.matvec(x, probe); dt = time.perf_counter() - t
+    nrows = int(min(o.n, max(64, 64 * seconds_target / max(dt, 1e-3))))
+    rows = np.sort(rng.choice(o.n, nrows, replace=False))
+    t = time.perf_counter(); o.matvec(x, rows); dt = time.perf_counter() - t
+    return nrows * per_row / dt, oracle.num_threads(), f"{nrows} of {o.n} seeded rows of one matvec ({nrows * per_row:.3g} interactions, {dt:.1f} s)", dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    prob, kw, desc = make_problem(args.config)
+    vals, secs = [], []
+    for _ in range(args.warmup):
+        oracle_sample(prob, kw, seconds_target=1.0)
+    sample = ""
+    for _ in range(args.steps):
+        v, cores, sample, dt = oracle_sample(prob, kw, seconds_target=max(2.0, 60.0 / max(args.steps, 1)))
+        vals.append(v); secs.append(dt)
+    v = float(np.mean(vals))
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "l2": "n/a (CPU)"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import paper_1309_4018_b200 as pg
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    pg.lib()
+    prob, kw, desc = make_problem(args.config)
+    precision = pg.PRECISION_MIXED if args.precision == "mixed" else pg.PRECISION_FP64
+    t0 = time.perf_counter()
+    h = pg.Handle.from_problem(prob, precision=precision, device=local, **kw)
+    torch.cuda.synchronize()
+    create_ms = 1e3 * (time.perf_counter() - t0)
+    st = h.stats()
+    n = h.n
+    rng = np.random.default_rng(7)
+    x = torch.tensor(rng.normal(size=n), device="cuda")
+    y = torch.empty_like(x)
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")   # 256 MB > 126 MB L2
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        h.matvec(x, y)
+    # ---- timed region: K matvecs, each bracketed by its own events, L2 flushed in between
+    stop, samples = threading.Event(), []
+    th = threading.Thread(target=clocks_sampler, args=(stop, samples), daemon=True)
+    th.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches0 = h.stats()["kernel_launches"]
+    barrier()
+    for a, b in ev:
+        flush.zero_()
+        a.record()
+        h.matvec(x, y)
+        b.record()
+    barrier()
+    launches = h.stats()["kernel_launches"] - launches0
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    # keep the sampler alive over a short sustained burst so that clocks under load are seen
+    tend = time.perf_counter() + 1.0
+    while time.perf_counter() < tend:
+        h.matvec(x, y)
+    torch.cuda.synchronize()
+    stop.set(); th.join()
+    tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms = float(tmax.item())
+    ms_per_step = ms / args.steps
+    value = world * st["direct_equiv"] * args.steps / (ms * 1e-3)
+
+    # ---- e2e: host buffers through pygbe_matvec_host (pinned), copies inside the timed region
+    xh = torch.empty(n, dtype=torch.float64).pin_memory(); xh.copy_(x.cpu())
+    yh = torch.empty(n, dtype=torch.float64).pin_memory()
+    xn, yn = xh.numpy(), yh.numpy()
+    for _ in range(3):
+        h.matvec_host(xn, yn)
+    barrier()
+    t = time.perf_counter()
+    for _ in range(args.steps):
+        flush.zero_()
+        torch.cuda.synchronize()
+        h.matvec_host(xn, yn)
+    e2e_s = time.perf_counter() - t
+    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e = world * st["direct_equiv"] * args.steps / float(te.item())
+
+    line = None
+    if rank == 0:
+        # ---- per-stage timers (profiled matvecs are not the ones timed above)
+        h.profile(True)
+        for _ in range(args.steps):
+            flush.zero_()
+            h.matvec(x, y)
+        stages = h.stage_times()
+        h.profile(False)
+        nreg_launch = {k: v[1] / args.steps for k, v in stages.items()}
+        stage_ms = {k: v[0] / args.steps for k, v in stages.items()}
+        dom = max(("p2p", "m2p"), key=lambda k: stage_ms[k])
+        yuk = [float(k) > 0 for k in prob.kappa]
+        # algorithmic flops of the dominant stage per matvec (all regions), DESIGN.md "Flop model"
+        # single-surface configs: one Laplace and one Yukawa region with identical lists
+        nreg = len(yuk)
+        if dom == "p2p":
+            flops = st["p2p_pairs"] / nreg * sum(P2P_FLOPS[yk] for yk in yuk)
+        else:
+            flops = st["m2p_evals"] / nreg * sum(m2p_flops(kw["P"], yk) for yk in yuk)
+        peaks = pg.alu_peaks(local)
+        mp = {}
+        try:
+            mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        sm_max = float(mp.get("sm_max_mhz", 1965.0))
+        nominal = {"f64": 148 * 64 * 2 * sm_max * 1e6 / 1e12, "f32": 148 * 128 * 2 * sm_max * 1e6 / 1e12}
+        dt = "f32" if precision == pg.PRECISION_MIXED else "f64"
+        achieved = flops / (stage_ms[dom] * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "k_%s_%s (both regions, %d launches/matvec)" % (dom, dt, round(nreg_launch[dom])),
+                    "achieved": achieved, "peak": nominal[dt], "unit": "TFLOP/s", "frac": achieved / nominal[dt],
+                    "peak_kind": "derived: 148 SM x %d lanes x 2 x %.0f MHz (DESIGN.md); FMA micro-benchmark in this run: %.1f TFLOP/s"
+                                 % (64 if dt == "f64" else 128, sm_max, peaks["fp64_tflops" if dt == "f64" else "fp32_tflops"]),
+                    "traffic": None, "stage_ms": stage_ms, "alu_peaks_measured": peaks,
+                    "flops_per_launchset": flops,
+                    "hbm_peak_gbs": mp.get("hbm_gbs")}
+        # ---- time-to-solution (second half of the metric): create + rhs + GMRES + energy, host buffers
+        t = time.perf_counter()
+        xs, iters, rr, es, ec = h.solve_host(tol=1e-6)
+        solve_ms = 1e3 * (time.perf_counter() - t)
+        solve = {"create_ms": create_ms, "solve_ms": solve_ms, "time_to_solution_ms": create_ms + solve_ms,
+                 "gmres_iters": iters, "rel_resid": rr, "tol": 1e-6, "E_solv_kJ_mol": es, "E_coul_kJ_mol": ec}
+        # ---- oracle on the host cores, bounded sample
+        cv, cores, sample, _ = oracle_sample(prob, kw, seconds_target=15.0)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": dt, "data": "synthetic",
+                "config": {"workload": desc, "n_panels": st["n_panels"], "n_unknowns": st["n_unknowns"],
+                           "direct_equiv_interactions": st["direct_equiv"], "p2p_pairs": st["p2p_pairs"],
+                           "m2p_evals": st["m2p_evals"], "precision": args.precision,
+                           "l2": "flushed between timed iterations (256 MB write)",
+                           "parallelism": "replicas only" if world > 1 else "single GPU"},
+                "clocks": summarize_clocks(samples),
+                "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n},
+                "gpu_launches": int(launches),
+                "roofline": roofline,
+                "cpu_baseline": {"value": cv, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+                "solve": solve,
+                "actual": {"p2p_pairs_per_s": st["p2p_pairs"] / (stage_ms["p2p"] * 1e-3) if stage_ms["p2p"] > 0 else None,
+                           "m2p_evals_per_s": st["m2p_evals"] / (stage_ms["m2p"] * 1e-3) if stage_ms["m2p"] > 0 else None}}
+    h.close()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="kirkwood_l5")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -163,8 +163,28 @@ int pygbe_reaction_potential(pygbe_handle *h, const double *x_dev, double *phi_d
 
 int pygbe_stats(const pygbe_handle *h, pygbe_stats_t *out);
 
+/* Per-stage CUDA-event timers of the matvec (SURVEY 5 "tracing / profiling").  pygbe_profile(h, 1) resets
+ * and enables them, pygbe_profile(h, 0) disables; while enabled every matvec records one event per stage
+ * start on the handle's stream (so a profiled matvec is a little slower: never quote its total time).
+ * pygbe_stage_times synchronises and returns the accumulated milliseconds and kernel-launch counts per
+ * stage since enabling: ms and launches are HOST arrays of PYGBE_N_STAGES entries (launches may be NULL). */
+#define PYGBE_STAGE_PREP    0  /* density weighting (a9 input side)             */
+#define PYGBE_STAGE_P2M     1  /* a3                                            */
+#define PYGBE_STAGE_M2M     2  /* a4                                            */
+#define PYGBE_STAGE_M2P     3  /* a6                                            */
+#define PYGBE_STAGE_P2P     4  /* a7                                            */
+#define PYGBE_STAGE_NEAR    5  /* a8 correction SpMV                            */
+#define PYGBE_STAGE_COMBINE 6  /* a9 block combination                          */
+#define PYGBE_N_STAGES      8
+int pygbe_profile(pygbe_handle *h, int enable);
+int pygbe_stage_times(pygbe_handle *h, double *ms, int64_t *launches);
+
 /* Thread-local message of the last failing call ("" if none). */
 const char *pygbe_last_error(void);
+
+/* ALU roofline denominators measured on `device` with dependent-FMA / MUFU micro-kernels (synchronous,
+ * ~50 ms): out3[0] = fp32 FMA TFLOP/s, out3[1] = fp64 FMA TFLOP/s, out3[2] = MUFU.RSQ Gop/s.  HOST. */
+int pygbe_alu_peaks(int32_t device, double *out3);
 
 /* Library / build identification, e.g. "pygbe-b200 0.1 sm_100a". */
 const char *pygbe_version(void);

@@ -77,6 +77,8 @@ def lib():
     L.pygbe_energy.argtypes = [vp, vp, dp, dp]
     L.pygbe_reaction_potential.argtypes = [vp, vp, vp]
     L.pygbe_stats.argtypes = [vp, C.POINTER(pygbe_stats_t)]
+    L.pygbe_profile.argtypes = [vp, C.c_int]
+    L.pygbe_stage_times.argtypes = [vp, dp, C.POINTER(C.c_int64)]
     L.pygbe_last_error.restype = C.c_char_p
     L.pygbe_version.restype = C.c_char_p
     _lib = L
@@ -211,10 +213,31 @@ class Handle:
         _check(lib().pygbe_reaction_potential(self._h, _dptr(x), _dptr(phi)))
         return phi
 
+    STAGES = ("prep", "p2m", "m2m", "m2p", "p2p", "near", "combine", "reserved")
+
+    def profile(self, enable=True):
+        _check(lib().pygbe_profile(self._h, int(bool(enable))))
+
+    def stage_times(self):
+        """{stage: (accumulated ms, kernel launches)} since profile(True)."""
+        ms = (C.c_double * 8)()
+        ln = (C.c_int64 * 8)()
+        _check(lib().pygbe_stage_times(self._h, ms, ln))
+        return {name: (ms[i], ln[i]) for i, name in enumerate(self.STAGES) if name != "reserved"}
+
     def stats(self):
         s = pygbe_stats_t()
         _check(lib().pygbe_stats(self._h, C.byref(s)))
         return {name: getattr(s, name) for name, _ in pygbe_stats_t._fields_}
+
+
+def alu_peaks(device=0):
+    """Measured ALU peaks of the device: dict(fp32_tflops, fp64_tflops, mufu_gops)."""
+    L = lib()
+    L.pygbe_alu_peaks.argtypes = [C.c_int32, C.POINTER(C.c_double)]
+    out = (C.c_double * 3)()
+    _check(L.pygbe_alu_peaks(device, out))
+    return dict(fp32_tflops=out[0], fp64_tflops=out[1], mufu_gops=out[2])
 
 
 def pygbe_version():

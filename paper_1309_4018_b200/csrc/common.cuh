@@ -171,6 +171,13 @@ struct pygbe_handle {
     std::vector<double> qxyz, qq;   // host copies of the charges
     std::vector<int> qreg;
     long launches = 0, n_matvec = 0, kernels_per_matvec = 0;
+    // optional per-stage CUDA-event timers (pygbe_profile / pygbe_stage_times)
+    bool profile = false;
+    std::vector<cudaEvent_t> ev_pool;
+    std::vector<int> ev_stage;          // stage started at event i (-1 = end marker)
+    size_t ev_used = 0;
+    double stage_ms[PYGBE_N_STAGES] = {0};
+    long stage_launches[PYGBE_N_STAGES] = {0};
     double create_ms = 0, last_solve_ms = 0;
     int last_iters = 0;
 };

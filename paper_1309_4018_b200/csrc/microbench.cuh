@@ -1,0 +1,67 @@
+// microbench.cuh -- ALU peak probes used as roofline denominators for the P2P / M2P stages, whose bound
+// is the CUDA-core pipes and not HBM or the tensor cores (MEASURED_PEAKS.json holds only the latter two).
+// Dependent FMA chains, 8 per thread, enough warps to fill every SM; one MUFU.RSQ chain set for the SFU.
+#pragma once
+#include "common.cuh"
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_fma_peak(int iters, T a, T b, T *out)
+{
+    T x0 = T(threadIdx.x), x1 = x0 + T(1), x2 = x0 + T(2), x3 = x0 + T(3);
+    T x4 = x0 + T(4), x5 = x0 + T(5), x6 = x0 + T(6), x7 = x0 + T(7);
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            x0 = x0 * a + b; x1 = x1 * a + b; x2 = x2 * a + b; x3 = x3 * a + b;
+            x4 = x4 * a + b; x5 = x5 * a + b; x6 = x6 * a + b; x7 = x7 * a + b;
+        }
+    }
+    T s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+    if (s == T(-12345)) out[0] = s;          // never true; keeps the chains alive
+}
+
+__global__ void __launch_bounds__(256) k_mufu_peak(int iters, float *out)
+{
+    float x0 = 1.0f + threadIdx.x, x1 = x0 + 1.f, x2 = x0 + 2.f, x3 = x0 + 3.f;
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            x0 = rsqrtf(x0); x1 = rsqrtf(x1); x2 = rsqrtf(x2); x3 = rsqrtf(x3);
+        }
+    }
+    float s = x0 + x1 + x2 + x3;
+    if (s == -12345.f) out[0] = s;
+}
+
+// out[0] = fp32 FMA TFLOP/s, out[1] = fp64 FMA TFLOP/s, out[2] = MUFU.RSQ Gop/s (best of 5 launches each)
+static int run_alu_peaks(int device, double *out)
+{
+    CUDA_TRY(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, device));
+    const int grid = prop.multiProcessorCount * 8, block = 256;
+    void *buf;
+    CUDA_TRY(cudaMalloc(&buf, 64));
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0)); CUDA_TRY(cudaEventCreate(&e1));
+    for (int which = 0; which < 3; which++) {
+        const int iters = which == 1 ? 2048 : 4096;
+        double best = 0.0;
+        for (int rep = 0; rep < 6; rep++) {
+            CUDA_TRY(cudaEventRecord(e0));
+            if (which == 0) k_fma_peak<float><<<grid, block>>>(iters, 1.0000001f, 1e-7f, (float *)buf);
+            else if (which == 1) k_fma_peak<double><<<grid, block>>>(iters, 1.0000001, 1e-7, (double *)buf);
+            else k_mufu_peak<<<grid, block>>>(iters, (float *)buf);
+            CUDA_TRY(cudaEventRecord(e1));
+            CUDA_TRY(cudaEventSynchronize(e1));
+            float ms = 0;
+            CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+            double ops = (double)grid * block * iters * 8.0 * (which == 2 ? 4.0 : 8.0 * 2.0);
+            if (rep > 0) best = std::max(best, ops / (ms * 1e-3));
+        }
+        out[which] = which == 2 ? best * 1e-9 : best * 1e-12;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(buf);
+    return PYGBE_OK;
+}

@@ -432,6 +432,7 @@ extern "C" void pygbe_destroy(pygbe_handle *h)
     h->mem.release();
     if (h->pinned_flags) cudaFreeHost(h->pinned_flags);
     if (h->pinned_scal) cudaFreeHost(h->pinned_scal);
+    for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     delete h;
 }
 
@@ -461,35 +462,89 @@ static int launch_m2p(pygbe_handle *h, Region &R, const int *skip)
     return PYGBE_OK;
 }
 
+// Stage timers: an event is recorded where a stage starts; the time to the next event belongs to it.
+static void stage_mark(pygbe_handle *h, int stage)
+{
+    if (!h->profile) return;
+    if (h->ev_used == h->ev_pool.size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return;
+        h->ev_pool.push_back(e);
+        h->ev_stage.push_back(-1);
+    }
+    h->ev_stage[h->ev_used] = stage;
+    cudaEventRecord(h->ev_pool[h->ev_used], h->stream);
+    h->ev_used++;
+}
+
+extern "C" int pygbe_profile(pygbe_handle *h, int enable)
+{
+    if (!h) { pygbe_set_error("profile: null handle"); return PYGBE_EINVAL; }
+    h->profile = enable != 0;
+    h->ev_used = 0;
+    for (int i = 0; i < PYGBE_N_STAGES; i++) { h->stage_ms[i] = 0; h->stage_launches[i] = 0; }
+    return PYGBE_OK;
+}
+
+extern "C" int pygbe_stage_times(pygbe_handle *h, double *ms, int64_t *launches)
+{
+    if (!h || !ms) { pygbe_set_error("stage_times: null pointer"); return PYGBE_EINVAL; }
+    CUDA_TRY(cudaSetDevice(h->device));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    for (size_t i = 0; i + 1 < h->ev_used; i++) {
+        int st = h->ev_stage[i];
+        if (st < 0 || st >= PYGBE_N_STAGES) continue;
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, h->ev_pool[i], h->ev_pool[i + 1]) == cudaSuccess) h->stage_ms[st] += t;
+    }
+    h->ev_used = 0;
+    for (int i = 0; i < PYGBE_N_STAGES; i++) { ms[i] = h->stage_ms[i]; if (launches) launches[i] = h->stage_launches[i]; }
+    return PYGBE_OK;
+}
+#define STAGE(h, st) do { stage_mark(h, st); if ((h)->profile) (h)->stage_launches[st] -= (h)->launches; } while (0)
+#define STAGE_END(h, st) do { if ((h)->profile) (h)->stage_launches[st] += (h)->launches; } while (0)
+
 // weights -> (P2M -> M2M -> M2P) + P2P -> corrections; leaves sum_S sigma[c V dphi - K phi] in R.out
 static int region_sum(pygbe_handle *h, Region &R, const double *x, const int *skip)
 {
     if (R.np == 0) return PYGBE_OK;
     const bool mixed = h->precision == PYGBE_PRECISION_MIXED;
+    STAGE(h, PYGBE_STAGE_PREP);
     LAUNCH(h, k_prep, cdiv(R.np, 128), 128, 0, skip, R.np, h->K, x, R.phi_idx, R.dphi_idx, R.cV, R.cK, R.pnrm, R.spos,
            R.schg, R.schgf, R.pphi, R.pdphi, R.out);
+    STAGE_END(h, PYGBE_STAGE_PREP);
     if (mixed) {
         TRY(mixed_region_sum(h, R, skip));
     } else {
         if (R.n_m2p_items > 0) {
+            STAGE(h, PYGBE_STAGE_P2M);
             LAUNCH(h, k_p2m, R.nleaves, P2M_THREADS, 0, skip, h->P, h->Nc, h->K, R.leaf_cell, R.cgeo, R.crange, R.spos,
                    R.schg, R.mom);
+            STAGE_END(h, PYGBE_STAGE_P2M);
+            STAGE(h, PYGBE_STAGE_M2M);
             for (int l = R.depth - 2; l >= 0; l--) {
                 int b = R.level_begin[l], e = R.level_begin[l + 1];
                 LAUNCH(h, k_m2m, e - b, M2M_THREADS, 0, skip, h->P, h->Nc, b, e, R.cgeo, R.cchild, R.mom);
             }
+            STAGE_END(h, PYGBE_STAGE_M2M);
+            STAGE(h, PYGBE_STAGE_M2P);
             TRY(launch_m2p(h, R, skip));
+            STAGE_END(h, PYGBE_STAGE_M2P);
         }
         if (R.n_p2p_items > 0) {
+            STAGE(h, PYGBE_STAGE_P2P);
             if (R.yukawa)
                 LAUNCH(h, k_p2p_f64<true>, R.n_p2p_items, PYGBE_TG, 0, skip, R.p2p_items, R.p2p_sub, h->K, R.np, R.tpos,
                        R.spos, R.schg, R.kappa, R.out);
             else
                 LAUNCH(h, k_p2p_f64<false>, R.n_p2p_items, PYGBE_TG, 0, skip, R.p2p_items, R.p2p_sub, h->K, R.np, R.tpos,
                        R.spos, R.schg, R.kappa, R.out);
+            STAGE_END(h, PYGBE_STAGE_P2P);
         }
     }
+    STAGE(h, PYGBE_STAGE_NEAR);
     LAUNCH(h, k_near_apply, cdiv(R.np, 128), 128, 0, skip, R.np, R.corr_off, R.corr_col, R.corr_val, R.pphi, R.pdphi, R.out);
+    STAGE_END(h, PYGBE_STAGE_NEAR);
     return PYGBE_OK;
 }
 
@@ -499,8 +554,11 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
     for (Region &R : h->regions) {
         if (R.np == 0) continue;
         TRY(region_sum(h, R, x, skip));
+        STAGE(h, PYGBE_STAGE_COMBINE);
         LAUNCH(h, k_combine, cdiv(R.np, 256), 256, 0, skip, R.np, R.row_idx, R.pphi, R.out, y);
+        STAGE_END(h, PYGBE_STAGE_COMBINE);
     }
+    stage_mark(h, -1);
     h->kernels_per_matvec = h->launches - before;
     h->n_matvec++;
     return PYGBE_OK;
@@ -735,4 +793,12 @@ extern "C" int pygbe_stats(const pygbe_handle *h, pygbe_stats_t *s)
     s->create_ms = h->create_ms; s->last_solve_ms = h->last_solve_ms; s->last_iters = h->last_iters;
     s->P = h->P; s->K = h->K; s->precision = h->precision; s->theta = h->theta;
     return PYGBE_OK;
+}
+
+// ------------------------------------------------------------------------------------ ALU peak probes
+#include "microbench.cuh"
+extern "C" int pygbe_alu_peaks(int32_t device, double *out3)
+{
+    if (!out3) { pygbe_set_error("alu_peaks: null pointer"); return PYGBE_EINVAL; }
+    return run_alu_peaks(device, out3);
 }
