@@ -1,0 +1,34 @@
+// mathx.cuh -- precision traits of the P2P / M2P arithmetic.
+//   double: plain fp64 (rsqrt, exp from libdevice).
+//   float : fp32 with the special-function unit: MUFU.RSQ (rsqrt.approx) and MUFU.EX2 (ex2.approx) --
+//           "rsqrt/exp on the SFU" of the north star; ~2 ulp each, far below the 1e-4 parity bar.
+#pragma once
+#include <cuda_runtime.h>
+
+template <typename T> struct Real;
+
+template <> struct Real<double> {
+    typedef double4 vec4;
+    static __device__ __forceinline__ double rsqrt_(double x) { return rsqrt(x); }
+    // exp(-kappa r); ks = kappa
+    static __device__ __forceinline__ double exp_neg(double ks, double r) { return exp(-ks * r); }
+    static __host__ double kscale(double kappa) { return kappa; }
+};
+
+template <> struct Real<float> {
+    typedef float4 vec4;
+    static __device__ __forceinline__ float rsqrt_(float x)
+    {
+        float y;
+        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+        return y;
+    }
+    // exp(-kappa r) = 2^(-kappa log2(e) r); ks = kappa * log2(e)
+    static __device__ __forceinline__ float exp_neg(float ks, float r)
+    {
+        float y;
+        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(-ks * r));
+        return y;
+    }
+    static __host__ double kscale(double kappa) { return kappa * 1.4426950408889634; }
+};
