@@ -1,0 +1,172 @@
+// build_lists.cuh -- octree (a2), target groups, MAC traversal (a5) and work items of one region.
+#pragma once
+#include "common.cuh"
+#include "host_util.cuh"
+#include "tree.cuh"
+#include "p2p.cuh"
+
+// Per-panel constants of a twin region, gathered into the primary region's Morton order.
+__global__ void k_gather_twin(int np, const int *__restrict__ perm, const int *__restrict__ row_u,
+                              const double *__restrict__ cV_u, const double *__restrict__ cK_u,
+                              int *__restrict__ row_idx, double *__restrict__ cV, double *__restrict__ cK)
+{
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    int u = perm[p];
+    row_idx[p] = row_u[u]; cV[p] = cV_u[u]; cK[p] = cK_u[u];
+}
+
+static int build_tree_and_lists(pygbe_handle *h, Region &R)
+{
+    const int K = h->K;
+    const double edge = R.root_edge;
+    // ---- octree: split level by level until no cell holds more than ncrit panels
+    const int ncrit = h->ncrit;
+    long maxcells = 64 + 8L * (R.np / std::max(1, ncrit) + 1) * 12;
+    int *d_ncells;
+    TRY(h->mem.alloc(&R.cgeo, maxcells)); TRY(h->mem.alloc(&R.crange, maxcells)); TRY(h->mem.alloc(&R.cchild, maxcells));
+    TRY(h->mem.alloc(&R.cparent, maxcells)); TRY(h->mem.alloc(&R.ckey, maxcells)); TRY(h->mem.alloc(&d_ncells, 1));
+    {
+        double4 g0 = make_double4(R.root_c[0], R.root_c[1], R.root_c[2], edge);
+        int2 r0 = make_int2(0, R.np), c0 = make_int2(-1, 0);
+        int par = -1, one = 1;
+        unsigned long long k0 = 0;
+        CUDA_TRY(cudaMemcpyAsync(R.cgeo, &g0, sizeof(g0), cudaMemcpyHostToDevice, h->stream));
+        CUDA_TRY(cudaMemcpyAsync(R.crange, &r0, sizeof(r0), cudaMemcpyHostToDevice, h->stream));
+        CUDA_TRY(cudaMemcpyAsync(R.cchild, &c0, sizeof(c0), cudaMemcpyHostToDevice, h->stream));
+        CUDA_TRY(cudaMemcpyAsync(R.cparent, &par, sizeof(par), cudaMemcpyHostToDevice, h->stream));
+        CUDA_TRY(cudaMemcpyAsync(R.ckey, &k0, sizeof(k0), cudaMemcpyHostToDevice, h->stream));
+        CUDA_TRY(cudaMemcpyAsync(d_ncells, &one, sizeof(one), cudaMemcpyHostToDevice, h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+    }
+    R.level_begin.clear();
+    R.level_begin.push_back(0);
+    int ncells = 1;
+    for (int level = 0; level <= PYGBE_MAXLEVEL; level++) {
+        int b = R.level_begin[level], e = ncells;
+        R.level_begin.push_back(e);
+        if (b == e) { R.level_begin.pop_back(); break; }
+        LAUNCH(h, k_split_level, 1, SPLIT_THREADS, 0, R.keys, level, b, e, ncrit, (int)maxcells, R.cgeo, R.crange,
+               R.cchild, R.cparent, R.ckey, d_ncells);
+        CUDA_TRY(cudaMemcpyAsync(&ncells, d_ncells, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+        if (ncells > maxcells) { pygbe_set_error("octree needs %d cells, capacity %ld", ncells, maxcells); return PYGBE_ENOMEM; }
+    }
+    R.ncells = ncells;
+    R.depth = (int)R.level_begin.size() - 1;      // number of levels
+    h->mem.release_one(d_ncells);
+    std::vector<int2> crange_h, cchild_h;
+    std::vector<int> cparent_h;
+    TRY(download(h, crange_h, R.crange, (size_t)ncells));
+    TRY(download(h, cchild_h, R.cchild, (size_t)ncells));
+    TRY(download(h, cparent_h, R.cparent, (size_t)ncells));
+    std::vector<int> clevel(ncells, 0);
+    for (int l = 0; l < R.depth; l++)
+        for (int c = R.level_begin[l]; c < R.level_begin[l + 1]; c++) clevel[c] = l;
+    std::vector<int> leaves;
+    for (int c = 0; c < ncells; c++)
+        if (cchild_h[c].y == 0) leaves.push_back(c);
+    std::sort(leaves.begin(), leaves.end(), [&](int a, int b) { return crange_h[a].x < crange_h[b].x; });
+    R.nleaves = (int)leaves.size();
+    TRY(upload(h, &R.leaf_cell, leaves));
+
+    // ---- anchors (mixed precision): the ancestor of each leaf at the level where cells are <= 16 A wide
+    const bool mixed = h->precision == PYGBE_PRECISION_MIXED;
+    std::vector<int> anchor_of(ncells, 0);
+    if (mixed) {
+        int alevel = 0;
+        while (edge / (double)(1 << alevel) > 16.0 && alevel < PYGBE_MAXLEVEL) alevel++;
+        std::vector<int> panel_anchor(R.np, 0);
+        for (int c : leaves) {
+            int a = c;
+            while (clevel[a] > alevel) a = cparent_h[a];
+            anchor_of[c] = a;
+            for (int p = crange_h[c].x; p < crange_h[c].y; p++) panel_anchor[p] = a;
+        }
+        TRY(upload(h, &R.panel_anchor, panel_anchor));
+        TRY(h->mem.alloc(&R.sposf, R.npts)); TRY(h->mem.alloc(&R.schgf, R.npts));
+        LAUNCH(h, k_make_sposf, cdiv(R.np, 128), 128, 0, R.np, K, R.panel_anchor, R.cgeo, R.spos, R.sposf);
+    }
+
+    // ---- target groups + traversal (count, offsets, fill)
+    R.ng = cdiv(R.np, PYGBE_TG);
+    TRY(h->mem.alloc(&R.ggeo, R.ng));
+    LAUNCH(h, k_group_geometry, R.ng, PYGBE_TG, 0, R.tpos, R.np, R.ggeo);
+    int *d_mcnt, *d_pcnt, *d_over;
+    TRY(h->mem.alloc(&d_mcnt, R.ng)); TRY(h->mem.alloc(&d_pcnt, R.ng)); TRY(h->mem.alloc(&d_over, 1));
+    CUDA_TRY(cudaMemsetAsync(d_over, 0, sizeof(int), h->stream));
+    const double near_dist = h->thres > 0 ? h->thres * R.Lmax : 0.0;
+    LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.ggeo, R.cgeo, R.crange, R.cchild,
+           h->theta, near_dist, 0, d_mcnt, d_pcnt, nullptr, nullptr, nullptr, nullptr, d_over);
+    std::vector<int> mcnt, pcnt;
+    TRY(download(h, mcnt, d_mcnt, (size_t)R.ng));
+    TRY(download(h, pcnt, d_pcnt, (size_t)R.ng));
+    std::vector<int> moff(R.ng + 1, 0), poff(R.ng + 1, 0);
+    for (int g = 0; g < R.ng; g++) { moff[g + 1] = moff[g] + mcnt[g]; poff[g + 1] = poff[g] + pcnt[g]; }
+    int *d_poff_raw, *d_pleaf_raw;
+    TRY(upload(h, &R.m2p_off, moff)); TRY(upload(h, &d_poff_raw, poff));
+    TRY(h->mem.alloc(&R.m2p_cell, moff[R.ng])); TRY(h->mem.alloc(&d_pleaf_raw, poff[R.ng]));
+    LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.ggeo, R.cgeo, R.crange, R.cchild,
+           h->theta, near_dist, 1, d_mcnt, d_pcnt, R.m2p_off, d_poff_raw, R.m2p_cell, d_pleaf_raw, d_over);
+    std::vector<int> pleaf;
+    TRY(download(h, pleaf, d_pleaf_raw, (size_t)poff[R.ng]));
+    int over = 0;
+    CUDA_TRY(cudaMemcpy(&over, d_over, sizeof(int), cudaMemcpyDeviceToHost));
+    if (over) { pygbe_set_error("traversal stack overflow"); return PYGBE_ECUDA; }
+    for (void *q : {(void *)d_mcnt, (void *)d_pcnt, (void *)d_over, (void *)d_poff_raw, (void *)d_pleaf_raw})
+        h->mem.release_one(q);
+
+    // ---- P2P lists: leaves -> panel ranges sorted by position; adjacent ranges with the same anchor merge
+    std::vector<int4> prng;               // merged ranges, CSR by group
+    std::vector<int> poff2(R.ng + 1, 0);
+    long total_src_panels = 0;
+    R.p2p_pairs = 0;
+    std::vector<int4> tmp;
+    for (int g = 0; g < R.ng; g++) {
+        tmp.clear();
+        for (int r = poff[g]; r < poff[g + 1]; r++) {
+            int c = pleaf[r];
+            tmp.push_back(make_int4(crange_h[c].x, crange_h[c].y, anchor_of[c], 0));
+        }
+        std::sort(tmp.begin(), tmp.end(), [](const int4 &a, const int4 &b) { return a.x < b.x; });
+        size_t start = prng.size();
+        for (const int4 &e : tmp) {
+            if (prng.size() > start && prng.back().y == e.x && prng.back().z == e.z) prng.back().y = e.y;
+            else prng.push_back(e);
+        }
+        poff2[g + 1] = (int)prng.size();
+        long ntg = std::min(PYGBE_TG, R.np - g * PYGBE_TG), src = 0;
+        for (size_t r = start; r < prng.size(); r++) src += prng[r].y - prng[r].x;
+        total_src_panels += src;
+        R.p2p_pairs += ntg * src * K;
+    }
+    R.m2p_evals = 0;
+    for (int g = 0; g < R.ng; g++) R.m2p_evals += (long)std::min(PYGBE_TG, R.np - g * PYGBE_TG) * mcnt[g];
+    TRY(upload(h, &R.p2p_off, poff2)); TRY(upload(h, &R.p2p_rng, prng));
+
+    // ---- work items of bounded size, enough of them to fill 148 SMs several times over
+    const long want_items = 148L * 16;
+    int p2p_item = (int)std::min(512L, std::max(32L, total_src_panels / want_items));
+    int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[R.ng] / want_items));
+    m2p_item = (m2p_item + 3) / 4 * 4;
+    std::vector<int4> sub, pitems, mitems;
+    for (int g = 0; g < R.ng; g++) {
+        int first = (int)sub.size(), acc = 0;
+        for (int r = poff2[g]; r < poff2[g + 1]; r++) {
+            int a = prng[r].x;
+            while (a < prng[r].y) {
+                int take = std::min(prng[r].y - a, p2p_item - acc);
+                sub.push_back(make_int4(a, a + take, prng[r].z, 0));
+                a += take; acc += take;
+                if (acc == p2p_item) { pitems.push_back(make_int4(g, first, (int)sub.size(), 0)); first = (int)sub.size(); acc = 0; }
+            }
+        }
+        if (acc > 0) pitems.push_back(make_int4(g, first, (int)sub.size(), 0));
+        for (int s = moff[g]; s < moff[g + 1]; s += m2p_item)
+            mitems.push_back(make_int4(g, s, std::min(s + m2p_item, moff[g + 1]), 0));
+    }
+    R.n_p2p_items = (int)pitems.size(); R.n_m2p_items = (int)mitems.size();
+    TRY(upload(h, &R.p2p_sub, sub)); TRY(upload(h, &R.p2p_items, pitems)); TRY(upload(h, &R.m2p_items, mitems));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return PYGBE_OK;
+}

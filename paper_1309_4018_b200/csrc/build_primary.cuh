@@ -1,0 +1,69 @@
+// build_primary.cuh -- build of a region that owns its tree (see build_region.cuh for the twin case).
+#pragma once
+#include "build_region.cuh"
+
+static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<double> &tri_host, const QuadTables &qt)
+{
+    const int K = h->K;
+    Boundary b;
+    collect_boundary(h, R.id, b);
+    R.np = (int)b.gid.size();
+    R.npts = R.np * K;
+    if (R.np == 0) return PYGBE_OK;
+    // root cube around the centroids; longest panel (for the near-field guard of the traversal)
+    double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+    double Lmax = 0.0;
+    for (int p = 0; p < R.np; p++) {
+        const double *t = tri_host.data() + 9 * (size_t)b.gid[p];
+        double ux = t[3] - t[0], uy = t[4] - t[1], uz = t[5] - t[2];
+        double vx = t[6] - t[0], vy = t[7] - t[1], vz = t[8] - t[2];
+        double cx = uy * vz - uz * vy, cy = uz * vx - ux * vz, cz = ux * vy - uy * vx;
+        Lmax = std::max(Lmax, std::sqrt(std::sqrt(cx * cx + cy * cy + cz * cz)));   // sqrt(2A), 2A = |cross|
+        for (int a = 0; a < 3; a++) {
+            double c = (t[a] + t[3 + a] + t[6 + a]) / 3.0;
+            lo[a] = std::min(lo[a], c); hi[a] = std::max(hi[a], c);
+        }
+    }
+    R.Lmax = Lmax;
+    const double edge = std::max({hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2]}) * (1.0 + 1e-6) + 1e-9;
+    for (int a = 0; a < 3; a++) R.root_c[a] = 0.5 * (lo[a] + hi[a]);
+    R.root_edge = edge;
+
+    // ---- Morton keys, sort, gather into sorted order, Gauss points
+    int *d_gid_u, *d_phi_u, *d_dphi_u, *d_row_u, *d_iota;
+    double *d_cV_u, *d_cK_u;
+    unsigned long long *d_keys_u;
+    TRY(upload(h, &d_gid_u, b.gid)); TRY(upload(h, &d_phi_u, b.phi)); TRY(upload(h, &d_dphi_u, b.dphi));
+    TRY(upload(h, &d_row_u, b.row)); TRY(upload(h, &d_cV_u, b.cV)); TRY(upload(h, &d_cK_u, b.cK));
+    TRY(h->mem.alloc(&d_iota, R.np)); TRY(h->mem.alloc(&R.perm, R.np));
+    TRY(h->mem.alloc(&d_keys_u, R.np)); TRY(h->mem.alloc(&R.keys, R.np));
+    LAUNCH(h, k_region_keys, cdiv(R.np, 256), 256, 0, h->gcen, d_gid_u, R.np, R.root_c[0] - 0.5 * edge,
+           R.root_c[1] - 0.5 * edge, R.root_c[2] - 0.5 * edge, 2097152.0 / edge, d_keys_u, d_iota);
+    {
+        size_t tmp_bytes = 0;
+        cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, d_keys_u, R.keys, d_iota, R.perm, R.np, 0, 63, h->stream);
+        char *tmp;
+        TRY(h->mem.alloc(&tmp, tmp_bytes));
+        CUDA_TRY(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, d_keys_u, R.keys, d_iota, R.perm, R.np, 0, 63, h->stream));
+        h->launches += 4;
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+        h->mem.release_one(tmp);
+    }
+    TRY(h->mem.alloc(&R.gid, R.np)); TRY(h->mem.alloc(&R.phi_idx, R.np)); TRY(h->mem.alloc(&R.dphi_idx, R.np));
+    TRY(h->mem.alloc(&R.row_idx, R.np)); TRY(h->mem.alloc(&R.cV, R.np)); TRY(h->mem.alloc(&R.cK, R.np));
+    TRY(h->mem.alloc(&R.tpos, R.np)); TRY(h->mem.alloc(&R.pnrm, R.np));
+    TRY(h->mem.alloc(&R.spos, R.npts)); TRY(h->mem.alloc(&R.schg, R.npts));
+    TRY(h->mem.alloc(&R.pphi, R.np)); TRY(h->mem.alloc(&R.pdphi, R.np)); TRY(h->mem.alloc(&R.out, R.np));
+    LAUNCH(h, k_region_gather, cdiv(R.np, 128), 128, 0, R.np, K, qt, R.perm, d_gid_u, d_phi_u, d_dphi_u, d_row_u,
+           d_cV_u, d_cK_u, h->tri, h->gcen, h->gnrm, R.gid, R.phi_idx, R.dphi_idx, R.row_idx, R.cV, R.cK, R.tpos,
+           R.pnrm, R.spos);
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    for (void *q : {(void *)d_gid_u, (void *)d_phi_u, (void *)d_dphi_u, (void *)d_row_u, (void *)d_iota,
+                    (void *)d_cV_u, (void *)d_cK_u, (void *)d_keys_u})
+        h->mem.release_one(q);
+    TRY(build_tree_and_lists(h, R));
+    TRY(build_corrections(h, R, qt, nullptr));
+    if (R.n_m2p_items > 0) TRY(h->mem.alloc(&R.mom, (size_t)R.ncells * 2 * h->Nc));
+    CUDA_TRY(cudaGetLastError());
+    return PYGBE_OK;
+}

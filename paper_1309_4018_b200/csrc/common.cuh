@@ -83,6 +83,11 @@ struct DeviceArena {
 // sources (K Gauss points each) and the targets (centroids) of one N-body sum with the region's kernel.
 struct Region {
     int id = 0;
+    int twin_of = -1;               // >= 0: shares tree, order, lists and moments with that region
+    int twin = -1;                  // >= 0: the region that shares this one's structures
+    double twin_rV = 0;             // twin charges: mV_B = twin_rV * mV_A, mK_B = -mK_A
+    int *perm = nullptr;            // sorted position -> position in the unsorted boundary list
+    int *panel_anchor = nullptr;    // anchor cell of each panel (mixed precision)
     double eps = 1, kappa = 0;
     bool yukawa = false;
     int np = 0, npts = 0;           // boundary panels, Gauss points (np * K)
@@ -95,7 +100,7 @@ struct Region {
     // per Gauss point (K consecutive per panel) ------------------------------------------------------
     double4 *spos = nullptr;        // (x, y, z, w_g A_j / 4pi)
     double4 *schg = nullptr;        // per matvec: (mV, mKx, mKy, mKz)
-    float4 *sposf = nullptr;        // mixed precision: position relative to root centre? (see prep)
+    float4 *sposf = nullptr;        // mixed precision: position relative to the anchor cell centre, weight
     float4 *schgf = nullptr;
     double *pphi = nullptr, *pdphi = nullptr;   // per matvec: gathered densities
     double *out = nullptr;          // per matvec: sum_S sigma_S [c_S V dphi - K phi] at each target
@@ -116,15 +121,14 @@ struct Region {
     double4 *ggeo = nullptr;        // group centre and radius
     int *m2p_off = nullptr, *m2p_cell = nullptr;
     int *p2p_off = nullptr;
-    int2 *p2p_rng = nullptr;        // source panel ranges
+    int4 *p2p_rng = nullptr;        // merged source panel ranges (lo, hi, anchor cell, -)
     int n_p2p_items = 0, n_m2p_items = 0;
     int4 *p2p_items = nullptr;      // (group, first range, last range+1, unused) over p2p_sub
-    int2 *p2p_sub = nullptr;        // refined (chunked) panel ranges
+    int4 *p2p_sub = nullptr;        // chunked panel ranges (lo, hi, anchor cell, -)
     int4 *m2p_items = nullptr;      // (group, first list slot, last slot+1, unused)
     long p2p_pairs = 0, m2p_evals = 0;
     // multipoles ------------------------------------------------------------------------------------
-    double *mom = nullptr;          // [ncells][Nc]
-    float *momf = nullptr;
+    double *mom = nullptr;          // [ncells][2][Nc]: MV, MK (farfield.cuh)
     // singular / near-singular corrections (CSR over targets) ----------------------------------------
     int *corr_off = nullptr, *corr_col = nullptr;
     double2 *corr_val = nullptr;    // (sigma c (fine - coarse)_V, sigma (fine - coarse)_K)
@@ -164,6 +168,10 @@ struct pygbe_handle {
     std::vector<Region> regions;
     GmresWork gm;
     double *phi_reac = nullptr;     // [nq]
+    struct IndexTables *itab = nullptr;   // device copy of the multi-index tables
+    cudaStream_t side = nullptr;    // far-field chain (P2M, M2M, M2P) runs here, concurrently with P2P
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    bool overlap = true;
     double *scratch = nullptr;      // small device scratch (16 doubles)
     double *xh = nullptr, *yh = nullptr;   // device staging for the *_host entry points
     int *pinned_flags = nullptr;    // host pinned, 4 ints

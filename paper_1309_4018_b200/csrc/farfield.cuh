@@ -1,22 +1,28 @@
-// farfield.cuh -- P2M (a3), upward pass M2M (a4) and M2P (a6) of the Cartesian Taylor treecode,
-// eq. (13)-(14).
+// farfield.cuh -- P2M (a3) and the upward pass M2M (a4) of the Cartesian Taylor treecode, eq. (13)-(14),
+// PAPER.md:144-153, :161.  (M2P lives in m2p.cuh, compiled once per order.)
 //
-// One combined multipole per cell serves both layers (reading A12): with point charges mV_g (single
-// layer) and vectors mK_g (double layer, normal folded in)
-//     M^k = sum_g [ mV_g d^k - sum_i mK_g,i k_i d^(k - e_i) ],   d = y_g - y_c,
-// so that  sum_g [ mV_g G - mK_g . grad_y G ](x)  ~  sum_|k|<=P a^k(x, y_c) M^k  with the Taylor
-// coefficients a^k = (1/k!) D_y^k G(x, y_c)  (eq. 14).
+// Two multipole sets per cell (reading A12), from the point charges mV_g (single layer) and the vectors
+// mK_g (double layer, normal folded in), d = y_g - y_c:
+//     MV^k = sum_g mV_g d^k                       ("m_c^k" of eq. 14)
+//     MK^k = sum_g sum_i mK_g,i k_i d^(k - e_i)   (n . grad_y applied to the monomial)
+// so that  sum_g [ mV_g G - mK_g . grad_y G ](x) ~ sum_|k|<=P a^k(x, y_c) (MV^k - MK^k).  Keeping the two
+// sets apart lets the two regions on either side of the same surfaces ("twin" regions, e.g. eq. 10's
+// Laplace and Yukawa rows) share one P2M and one upward pass: their moments are c_a MV + c_b MK with
+// different constants.  Layout: mom[cell][set][Nc], fp64.
 #pragma once
 #include "common.cuh"
 #include "tables.cuh"
 
 // ------------------------------------------------------------------------------------------------ P2M
+// One CTA per leaf; thread k owns coefficient k of both sets; the leaf's points go through shared memory
+// as tables of powers d^0..d^P per axis (HBM traffic: each point read once, 64 B).
 #define P2M_THREADS 128
 #define P2M_TILE 64
+#define P2M_SLOTS ((PYGBE_NCMAX + P2M_THREADS - 1) / P2M_THREADS)
 __global__ void __launch_bounds__(P2M_THREADS)
-k_p2m(const int *__restrict__ skip, int P, int Nc, int K, const int *__restrict__ leaf_cell, const double4 *__restrict__ cgeo,
-      const int2 *__restrict__ crange, const double4 *__restrict__ spos, const double4 *__restrict__ schg,
-      double *__restrict__ mom)
+k_p2m(const int *__restrict__ skip, int P, int Nc, int K, const IndexTables *__restrict__ tab,
+      const int *__restrict__ leaf_cell, const double4 *__restrict__ cgeo, const int2 *__restrict__ crange,
+      const double4 *__restrict__ spos, const double4 *__restrict__ schg, double *__restrict__ mom)
 {
     __shared__ double s_pw[P2M_TILE][3][PYGBE_PMAX + 1];
     __shared__ double4 s_chg[P2M_TILE];
@@ -25,9 +31,15 @@ k_p2m(const int *__restrict__ skip, int P, int Nc, int K, const int *__restrict_
     const double4 cg = cgeo[cell];
     const int2 rg = crange[cell];
     const long p0 = (long)rg.x * K, p1 = (long)rg.y * K;
-    double acc[(PYGBE_NCMAX + P2M_THREADS - 1) / P2M_THREADS];
+    double accV[P2M_SLOTS], accK[P2M_SLOTS];
+    int kk[P2M_SLOTS][3];
 #pragma unroll
-    for (int i = 0; i < (PYGBE_NCMAX + P2M_THREADS - 1) / P2M_THREADS; i++) acc[i] = 0.0;
+    for (int s = 0; s < P2M_SLOTS; s++) {
+        accV[s] = accK[s] = 0.0;
+        int k = threadIdx.x + s * P2M_THREADS;
+        if (k < Nc) { kk[s][0] = tab->kxyz[k][0]; kk[s][1] = tab->kxyz[k][1]; kk[s][2] = tab->kxyz[k][2]; }
+        else { kk[s][0] = kk[s][1] = kk[s][2] = 0; }
+    }
     for (long base = p0; base < p1; base += P2M_TILE) {
         int n = (int)min((long)P2M_TILE, p1 - base);
         __syncthreads();
@@ -41,81 +53,112 @@ k_p2m(const int *__restrict__ skip, int P, int Nc, int K, const int *__restrict_
         for (int i = threadIdx.x; i < n; i += P2M_THREADS) s_chg[i] = schg[base + i];
         __syncthreads();
 #pragma unroll
-        for (int s = 0; s < (PYGBE_NCMAX + P2M_THREADS - 1) / P2M_THREADS; s++) {
+        for (int s = 0; s < P2M_SLOTS; s++) {
             int k = threadIdx.x + s * P2M_THREADS;
             if (k >= Nc) break;
-            int kx = c_kxyz[k][0], ky = c_kxyz[k][1], kz = c_kxyz[k][2];
-            double a = 0.0;
+            const int kx = kk[s][0], ky = kk[s][1], kz = kk[s][2];
+            double aV = 0.0, aK = 0.0;
             for (int pt = 0; pt < n; pt++) {
                 double X = s_pw[pt][0][kx], Y = s_pw[pt][1][ky], Z = s_pw[pt][2][kz];
                 double4 c = s_chg[pt];
-                double t = c.x * X * Y * Z;
-                if (kx) t -= c.y * kx * s_pw[pt][0][kx - 1] * Y * Z;
-                if (ky) t -= c.z * ky * X * s_pw[pt][1][ky - 1] * Z;
-                if (kz) t -= c.w * kz * X * Y * s_pw[pt][2][kz - 1];
-                a += t;
+                aV += c.x * X * Y * Z;
+                double t = 0.0;
+                if (kx) t += c.y * kx * s_pw[pt][0][kx - 1] * Y * Z;
+                if (ky) t += c.z * ky * X * s_pw[pt][1][ky - 1] * Z;
+                if (kz) t += c.w * kz * X * Y * s_pw[pt][2][kz - 1];
+                aK += t;
             }
-            acc[s] += a;
+            accV[s] += aV; accK[s] += aK;
         }
     }
 #pragma unroll
-    for (int s = 0; s < (PYGBE_NCMAX + P2M_THREADS - 1) / P2M_THREADS; s++) {
+    for (int s = 0; s < P2M_SLOTS; s++) {
         int k = threadIdx.x + s * P2M_THREADS;
-        if (k < Nc) mom[(long)cell * Nc + k] = acc[s];
+        if (k < Nc) { mom[((long)cell * 2) * Nc + k] = accV[s]; mom[((long)cell * 2 + 1) * Nc + k] = accK[s]; }
     }
 }
 
 // ------------------------------------------------------------------------------------------------ M2M
-// Parent moments from the children's ("shifted and added"):
+// Parent moments from the children's ("shifted and added"), for both sets:
 //   M_p^k = sum_children sum_{l <= k} C(k,l) s^(k-l) M_c^l,   s = y_child - y_parent.
-// One CTA per non-leaf cell of the level; launched level by level from the deepest upward.
-#define M2M_THREADS 128
+// The shift factorises over the axes, so it is applied as three one-dimensional shifts (x, then y, then z)
+// through two shared-memory buffers: O(Nc P) work per child instead of O(Nc P^3).  The index tables are
+// staged in shared memory (the first version read them from constant memory with divergent indices and
+// was latency-bound: 62 us per launch, profiles/r1a_first_path.md).  One CTA per non-leaf cell of the
+// level; launched level by level from the deepest upward.
+#define M2M_THREADS 256
+#define M2M_SLOTS ((2 * PYGBE_NCMAX + M2M_THREADS - 1) / M2M_THREADS)
 __global__ void __launch_bounds__(M2M_THREADS)
-k_m2m(const int *__restrict__ skip, int P, int Nc, int cell_begin, int cell_end, const double4 *__restrict__ cgeo,
-      const int2 *__restrict__ cchild, double *__restrict__ mom)
+k_m2m(const int *__restrict__ skip, int P, int Nc, int cell_begin, int cell_end,
+      const IndexTables *__restrict__ tab, const double4 *__restrict__ cgeo, const int2 *__restrict__ cchild,
+      double *__restrict__ mom)
 {
-    __shared__ double s_M[PYGBE_NCMAX];
+    __shared__ double s_a[2 * PYGBE_NCMAX], s_b[2 * PYGBE_NCMAX];
     __shared__ double s_pw[3][PYGBE_PMAX + 1];
+    __shared__ double s_binom[PYGBE_PMAX + 1][PYGBE_PMAX + 1];
+    __shared__ short s_idx3[PYGBE_PMAX + 1][PYGBE_PMAX + 1][PYGBE_PMAX + 1];
     if (skip && *skip) return;
     const int cell = cell_begin + blockIdx.x;
     if (cell >= cell_end) return;
     const int2 ch = cchild[cell];
     if (ch.y == 0) return;                       // leaf: filled by P2M
+    for (int i = threadIdx.x; i < (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1); i += M2M_THREADS)
+        (&s_binom[0][0])[i] = (&tab->binom[0][0])[i];
+    for (int i = threadIdx.x; i < (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1); i += M2M_THREADS)
+        (&s_idx3[0][0][0])[i] = (&tab->idx3[0][0][0])[i];
     const double4 pg = cgeo[cell];
-    double acc[(PYGBE_NCMAX + M2M_THREADS - 1) / M2M_THREADS];
+    const int n2 = 2 * Nc;
+    double acc[M2M_SLOTS];
+    int kx[M2M_SLOTS], ky[M2M_SLOTS], kz[M2M_SLOTS], so[M2M_SLOTS];
 #pragma unroll
-    for (int i = 0; i < (PYGBE_NCMAX + M2M_THREADS - 1) / M2M_THREADS; i++) acc[i] = 0.0;
+    for (int s = 0; s < M2M_SLOTS; s++) {
+        acc[s] = 0.0;
+        int e = threadIdx.x + s * M2M_THREADS;
+        int k = e < Nc ? e : e - Nc;
+        so[s] = e < Nc ? 0 : Nc;
+        if (e < n2) { kx[s] = tab->kxyz[k][0]; ky[s] = tab->kxyz[k][1]; kz[s] = tab->kxyz[k][2]; }
+        else { kx[s] = ky[s] = kz[s] = 0; }
+    }
     for (int c = ch.x; c < ch.x + ch.y; c++) {
         __syncthreads();
-        for (int i = threadIdx.x; i < Nc; i += M2M_THREADS) s_M[i] = mom[(long)c * Nc + i];
+        for (int i = threadIdx.x; i < n2; i += M2M_THREADS) s_a[i] = mom[(long)c * n2 + i];
         if (threadIdx.x < 3) {
             double4 g = cgeo[c];
-            double s = threadIdx.x == 0 ? g.x - pg.x : (threadIdx.x == 1 ? g.y - pg.y : g.z - pg.z);
+            double sft = threadIdx.x == 0 ? g.x - pg.x : (threadIdx.x == 1 ? g.y - pg.y : g.z - pg.z);
             double pw = 1.0;
-            for (int e = 0; e <= P; e++) { s_pw[threadIdx.x][e] = pw; pw *= s; }
+            for (int e = 0; e <= P; e++) { s_pw[threadIdx.x][e] = pw; pw *= sft; }
         }
         __syncthreads();
 #pragma unroll
-        for (int s = 0; s < (PYGBE_NCMAX + M2M_THREADS - 1) / M2M_THREADS; s++) {
-            int k = threadIdx.x + s * M2M_THREADS;
-            if (k >= Nc) break;
-            int kx = c_kxyz[k][0], ky = c_kxyz[k][1], kz = c_kxyz[k][2];
+        for (int s = 0; s < M2M_SLOTS; s++) {            // shift along x: s_a -> s_b
+            int e = threadIdx.x + s * M2M_THREADS;
+            if (e >= n2) break;
             double a = 0.0;
-            for (int lx = 0; lx <= kx; lx++) {
-                double fx = c_binom[kx][lx] * s_pw[0][kx - lx];
-                for (int ly = 0; ly <= ky; ly++) {
-                    double fy = fx * c_binom[ky][ly] * s_pw[1][ky - ly];
-                    for (int lz = 0; lz <= kz; lz++)
-                        a += fy * c_binom[kz][lz] * s_pw[2][kz - lz] * s_M[c_idx3[lx][ly][lz]];
-                }
-            }
+            for (int l = 0; l <= kx[s]; l++) a += s_binom[kx[s]][l] * s_pw[0][kx[s] - l] * s_a[so[s] + s_idx3[l][ky[s]][kz[s]]];
+            s_b[e] = a;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int s = 0; s < M2M_SLOTS; s++) {            // shift along y: s_b -> s_a
+            int e = threadIdx.x + s * M2M_THREADS;
+            if (e >= n2) break;
+            double a = 0.0;
+            for (int l = 0; l <= ky[s]; l++) a += s_binom[ky[s]][l] * s_pw[1][ky[s] - l] * s_b[so[s] + s_idx3[kx[s]][l][kz[s]]];
+            s_a[e] = a;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int s = 0; s < M2M_SLOTS; s++) {            // shift along z: s_a -> accumulator
+            int e = threadIdx.x + s * M2M_THREADS;
+            if (e >= n2) break;
+            double a = 0.0;
+            for (int l = 0; l <= kz[s]; l++) a += s_binom[kz[s]][l] * s_pw[2][kz[s] - l] * s_a[so[s] + s_idx3[kx[s]][ky[s]][l]];
             acc[s] += a;
         }
     }
 #pragma unroll
-    for (int s = 0; s < (PYGBE_NCMAX + M2M_THREADS - 1) / M2M_THREADS; s++) {
-        int k = threadIdx.x + s * M2M_THREADS;
-        if (k < Nc) mom[(long)cell * Nc + k] = acc[s];
+    for (int s = 0; s < M2M_SLOTS; s++) {
+        int e = threadIdx.x + s * M2M_THREADS;
+        if (e < n2) mom[(long)cell * n2 + e] = acc[s];
     }
 }
-

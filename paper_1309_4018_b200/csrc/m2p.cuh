@@ -2,17 +2,17 @@
 // Compiled once per expansion order P (m2p_inst.cu with -DM2P_P=<P>) so that the orders build in parallel.
 #pragma once
 #include <cuda_runtime.h>
+#include "mathx.cuh"
 #define PYGBE_TG_M2P 128
 
 struct M2PArgs {
     const int *skip; const int4 *items; const int *m2p_cell; int n_items; int np;
-    const double4 *tpos; const double4 *cgeo; const double *mom; double kappa; double *out;
-    int yukawa; cudaStream_t stream;
-    // mixed precision
-    const float4 *tposf; const float4 *cgeof; const float *momf;
+    const double4 *tpos; const double4 *cgeo; const double *mom;   // mom[cell][2][Nc]: MV, MK (farfield.cuh)
+    double ca, cb;             // the region's multipole is ca * MV + cb * MK
+    double kappa; double *out;
+    int yukawa; int fp32; cudaStream_t stream;
 };
 
-// ------------------------------------------------------------------------------------------------ M2P
 // Taylor coefficients by recurrence ("recursive relations for the Green's function of
 // the Poisson equation [20] and linearized Poisson-Boltzmann equation [21]"; reading A13), d = x - y_c,
 // R^2 = |d|^2, n = |k|, terms with a negative index dropped:
@@ -23,16 +23,18 @@ struct M2PArgs {
 //                         + kappa [ sum_i d_i b^(k-e_i) - sum_i b^(k-2e_i) ]
 // The loops are fully unrolled for the compile-time order P: the coefficient arrays live in registers
 // and only two order-shells are alive at a time.  Returns sum_k a^k M^k (M in shared memory).
+// T = double: fp64 throughout.  T = float: fp32 recurrence with MUFU rsqrt / ex2 (mathx.cuh); SURVEY A8b:
+// fp32 coefficient error 1.4e-7 (order 0) .. 1.8e-6 (order 8), far below the truncation error.
 template <int P, bool YUKAWA, typename T>
-__device__ __forceinline__ T m2p_eval(T dx, T dy, T dz, T kappa, const T *__restrict__ M)
+__device__ __forceinline__ T m2p_eval(T dx, T dy, T dz, T kappa, T kscaled, const T *__restrict__ M)
 {
     T a[P + 1][P + 1][P + 1];
     T b[YUKAWA ? P + 1 : 1][YUKAWA ? P + 1 : 1][YUKAWA ? P + 1 : 1];
     const T R2 = dx * dx + dy * dy + dz * dz;
-    const T invR2 = T(1) / R2;
-    const T invR = sqrt(invR2);
+    const T invR = Real<T>::rsqrt_(R2);
+    const T invR2 = invR * invR;
     if constexpr (YUKAWA) {
-        b[0][0][0] = exp(-kappa * R2 * invR);
+        b[0][0][0] = Real<T>::exp_neg(kscaled, R2 * invR);
         a[0][0][0] = b[0][0][0] * invR;
     } else {
         a[0][0][0] = invR;
@@ -77,16 +79,18 @@ __device__ __forceinline__ T m2p_eval(T dx, T dy, T dz, T kappa, const T *__rest
 }
 
 // Work item = (target group, a run of its M2P list).  One thread per target; the moments of M2P_CB cells
-// at a time are staged in shared memory and read by all threads as broadcasts.
+// at a time are staged in shared memory (combined ca MV + cb MK, converted to T) and read by all threads
+// as broadcasts.  The target offset d = x - y_c is always formed in fp64 and then rounded to T, so the
+// fp32 path never subtracts large absolute coordinates; accumulation over cells is fp64.
 #define M2P_CB 4
-template <int P, bool YUKAWA>
+template <int P, bool YUKAWA, typename T>
 __global__ void __launch_bounds__(PYGBE_TG_M2P)
-k_m2p_f64(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
-          const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo,
-          const double *__restrict__ mom, double kappa, double *__restrict__ out)
+k_m2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
+      const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const double *__restrict__ mom,
+      double ca, double cb, double kappa, double kscaled, double *__restrict__ out)
 {
     constexpr int Nc = (P + 1) * (P + 2) * (P + 3) / 6;
-    __shared__ double s_M[M2P_CB][Nc];
+    __shared__ T s_M[M2P_CB][Nc];
     __shared__ double4 s_c[M2P_CB];
     if (skip && *skip) return;
     const int4 it = items[blockIdx.x];
@@ -98,14 +102,16 @@ k_m2p_f64(const int *__restrict__ skip, const int4 *__restrict__ items, const in
         int nb = min(M2P_CB, it.z - s0);
         __syncthreads();
         for (int i = threadIdx.x; i < nb * Nc; i += PYGBE_TG_M2P) {
-            int cb = i / Nc, k = i - cb * Nc;
-            s_M[cb][k] = mom[(long)m2p_cell[s0 + cb] * Nc + k];
+            int cb_ = i / Nc, k = i - cb_ * Nc;
+            const double *m = mom + (long)m2p_cell[s0 + cb_] * 2 * Nc;
+            s_M[cb_][k] = (T)(ca * m[k] + cb * m[Nc + k]);
         }
         if (threadIdx.x < nb) s_c[threadIdx.x] = cgeo[m2p_cell[s0 + threadIdx.x]];
         __syncthreads();
-        for (int cb = 0; cb < nb; cb++) {
-            double4 c = s_c[cb];
-            acc += m2p_eval<P, YUKAWA, double>(X.x - c.x, X.y - c.y, X.z - c.z, kappa, s_M[cb]);
+        for (int c_ = 0; c_ < nb; c_++) {
+            double4 c = s_c[c_];
+            acc += (double)m2p_eval<P, YUKAWA, T>((T)(X.x - c.x), (T)(X.y - c.y), (T)(X.z - c.z), (T)kappa,
+                                                  (T)kscaled, s_M[c_]);
         }
     }
     if (ok) atomicAdd(out + t, acc);

@@ -6,13 +6,15 @@
 #define CAT_(a, b) a##b
 #define CAT(a, b) CAT_(a, b)
 
-int CAT(pygbe_m2p_f64_launch_, M2P_P)(const M2PArgs &a)
+template <bool Y, typename T> static void launch(const M2PArgs &a)
 {
-    if (a.yukawa)
-        k_m2p_f64<M2P_P, true><<<a.n_items, PYGBE_TG_M2P, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo,
-                                                                        a.mom, a.kappa, a.out);
-    else
-        k_m2p_f64<M2P_P, false><<<a.n_items, PYGBE_TG_M2P, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo,
-                                                                         a.mom, a.kappa, a.out);
+    k_m2p<M2P_P, Y, T><<<a.n_items, PYGBE_TG_M2P, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo, a.mom,
+                                                                 a.ca, a.cb, a.kappa, Real<T>::kscale(a.kappa), a.out);
+}
+
+int CAT(pygbe_m2p_launch_, M2P_P)(const M2PArgs &a)
+{
+    if (a.fp32) { if (a.yukawa) launch<true, float>(a); else launch<false, float>(a); }
+    else { if (a.yukawa) launch<true, double>(a); else launch<false, double>(a); }
     return 0;
 }

@@ -12,7 +12,7 @@ template <> struct Real<double> {
     static __device__ __forceinline__ double rsqrt_(double x) { return rsqrt(x); }
     // exp(-kappa r); ks = kappa
     static __device__ __forceinline__ double exp_neg(double ks, double r) { return exp(-ks * r); }
-    static __host__ double kscale(double kappa) { return kappa; }
+    static __host__ __device__ double kscale(double kappa) { return kappa; }
 };
 
 template <> struct Real<float> {
@@ -30,5 +30,5 @@ template <> struct Real<float> {
         asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(-ks * r));
         return y;
     }
-    static __host__ double kscale(double kappa) { return kappa * 1.4426950408889634; }
+    static __host__ __device__ double kscale(double kappa) { return kappa * 1.4426950408889634; }
 };

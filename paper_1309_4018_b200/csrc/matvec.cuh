@@ -1,0 +1,133 @@
+// matvec.cuh -- one evaluation of the treecode, y = A x: kernel launches only.
+//   main stream : prep -> P2P (twin regions fused) ----------------------> near-field corrections -> combine
+//   side stream :      -> P2M -> M2M (per level) -> M2P (per region) ---^   (joined by an event)
+// The far-field chain is latency-bound at small sizes (one launch per tree level); running it beside the
+// compute-bound P2P hides it.  With the stage timers on, everything is issued on the main stream instead.
+#pragma once
+#include "common.cuh"
+#include "nearfield.cuh"
+#include "farfield.cuh"
+#include "p2p.cuh"
+#include "m2p.cuh"
+
+// Stage timers: an event is recorded where a stage starts; the time to the next event belongs to it.
+static void stage_mark(pygbe_handle *h, int stage)
+{
+    if (!h->profile) return;
+    if (h->ev_used == h->ev_pool.size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return;
+        h->ev_pool.push_back(e);
+        h->ev_stage.push_back(-1);
+    }
+    h->ev_stage[h->ev_used] = stage;
+    cudaEventRecord(h->ev_pool[h->ev_used], h->stream);
+    h->ev_used++;
+}
+#define STAGE(h, st) do { stage_mark(h, st); if ((h)->profile) (h)->stage_launches[st] -= (h)->launches; } while (0)
+#define STAGE_END(h, st) do { if ((h)->profile) (h)->stage_launches[st] += (h)->launches; } while (0)
+
+#define M2P_DECL(PP) int pygbe_m2p_launch_##PP(const M2PArgs &);
+M2P_DECL(1) M2P_DECL(2) M2P_DECL(3) M2P_DECL(4) M2P_DECL(5) M2P_DECL(6)
+M2P_DECL(7) M2P_DECL(8) M2P_DECL(9) M2P_DECL(10) M2P_DECL(11) M2P_DECL(12)
+#undef M2P_DECL
+
+// M2P of region R with the multipoles ca MV + cb MK of the tree owner T, on stream st.
+static int launch_m2p(pygbe_handle *h, Region &T, Region &R, double ca, double cb, const int *skip, cudaStream_t st)
+{
+    M2PArgs a;
+    memset(&a, 0, sizeof(a));
+    a.skip = skip; a.items = T.m2p_items; a.m2p_cell = T.m2p_cell; a.n_items = T.n_m2p_items; a.np = T.np;
+    a.tpos = T.tpos; a.cgeo = T.cgeo; a.mom = T.mom; a.ca = ca; a.cb = cb; a.kappa = R.kappa; a.out = R.out;
+    a.yukawa = R.yukawa; a.fp32 = h->precision == PYGBE_PRECISION_MIXED; a.stream = st;
+    typedef int (*fn_t)(const M2PArgs &);
+    static const fn_t table[PYGBE_PMAX + 1] = {nullptr, pygbe_m2p_launch_1, pygbe_m2p_launch_2, pygbe_m2p_launch_3,
+        pygbe_m2p_launch_4, pygbe_m2p_launch_5, pygbe_m2p_launch_6, pygbe_m2p_launch_7, pygbe_m2p_launch_8,
+        pygbe_m2p_launch_9, pygbe_m2p_launch_10, pygbe_m2p_launch_11, pygbe_m2p_launch_12};
+    if (h->P < 1 || h->P > PYGBE_PMAX) { pygbe_set_error("P = %d not instantiated", h->P); return PYGBE_EINVAL; }
+    table[h->P](a);
+    h->launches++;
+    return PYGBE_OK;
+}
+
+template <typename T>
+static void launch_p2p(pygbe_handle *h, Region &A, Region *B, const int *skip)
+{
+    typedef typename Real<T>::vec4 V4;
+    const V4 *pos = sizeof(T) == 4 ? (const V4 *)A.sposf : (const V4 *)A.spos;
+    const V4 *chg = sizeof(T) == 4 ? (const V4 *)A.schgf : (const V4 *)A.schg;
+    const double kA = A.kappa, kB = B ? B->kappa : 0.0, rV = A.twin_rV;
+    double *oA = A.out, *oB = B ? B->out : nullptr;
+#define P2P_GO(YA, TW, YB)                                                                                     \
+    do { auto kern = k_p2p<T, YA, TW, YB>;                                                                     \
+    LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, h->K, A.np, A.tpos,              \
+           A.cgeo, pos, chg, kA, kB, rV, oA, oB); } while (0)
+    if (!B) { if (A.yukawa) P2P_GO(true, false, false); else P2P_GO(false, false, false); }
+    else if (A.yukawa) { if (B->yukawa) P2P_GO(true, true, true); else P2P_GO(true, true, false); }
+    else { if (B->yukawa) P2P_GO(false, true, true); else P2P_GO(false, true, false); }
+#undef P2P_GO
+}
+
+// Everything of one tree owner A (and its twin B, if any) except the final combination.
+static int region_sum(pygbe_handle *h, Region &A, Region *B, const double *x, const int *skip)
+{
+    if (A.np == 0) return PYGBE_OK;
+    const bool mixed = h->precision == PYGBE_PRECISION_MIXED;
+    const bool far = A.n_m2p_items > 0;
+    const bool fork = far && h->overlap && !h->profile && h->side != nullptr;
+    STAGE(h, PYGBE_STAGE_PREP);
+    LAUNCH(h, k_prep, cdiv(A.np, 128), 128, 0, skip, A.np, h->K, x, A.phi_idx, A.dphi_idx, A.cV, A.cK, A.pnrm, A.spos,
+           A.schg, mixed ? A.schgf : (float4 *)nullptr, A.pphi, A.pdphi, A.out, B ? B->out : (double *)nullptr);
+    STAGE_END(h, PYGBE_STAGE_PREP);
+    cudaStream_t main_st = h->stream, fs = fork ? h->side : h->stream;
+    if (far) {
+        if (fork) { cudaEventRecord(h->ev_fork, main_st); cudaStreamWaitEvent(fs, h->ev_fork, 0); }
+        cudaStream_t keep = h->stream;
+        h->stream = fs;                      // LAUNCH issues on h->stream
+        STAGE(h, PYGBE_STAGE_P2M);
+        LAUNCH(h, k_p2m, A.nleaves, P2M_THREADS, 0, skip, h->P, h->Nc, h->K, h->itab, A.leaf_cell, A.cgeo, A.crange,
+               A.spos, A.schg, A.mom);
+        STAGE_END(h, PYGBE_STAGE_P2M);
+        STAGE(h, PYGBE_STAGE_M2M);
+        for (int l = A.depth - 2; l >= 0; l--) {
+            int b = A.level_begin[l], e = A.level_begin[l + 1];
+            LAUNCH(h, k_m2m, e - b, M2M_THREADS, 0, skip, h->P, h->Nc, b, e, h->itab, A.cgeo, A.cchild, A.mom);
+        }
+        STAGE_END(h, PYGBE_STAGE_M2M);
+        STAGE(h, PYGBE_STAGE_M2P);
+        TRY(launch_m2p(h, A, A, 1.0, -1.0, skip, fs));
+        if (B) TRY(launch_m2p(h, A, *B, A.twin_rV, 1.0, skip, fs));
+        STAGE_END(h, PYGBE_STAGE_M2P);
+        h->stream = keep;
+        if (fork) cudaEventRecord(h->ev_join, fs);
+    }
+    if (A.n_p2p_items > 0) {
+        STAGE(h, PYGBE_STAGE_P2P);
+        if (mixed) launch_p2p<float>(h, A, B, skip); else launch_p2p<double>(h, A, B, skip);
+        STAGE_END(h, PYGBE_STAGE_P2P);
+    }
+    if (fork) cudaStreamWaitEvent(main_st, h->ev_join, 0);
+    STAGE(h, PYGBE_STAGE_NEAR);
+    LAUNCH(h, k_near_apply, cdiv(A.np, 128), 128, 0, skip, A.np, A.corr_off, A.corr_col, A.corr_val, A.pphi, A.pdphi, A.out);
+    if (B) LAUNCH(h, k_near_apply, cdiv(A.np, 128), 128, 0, skip, A.np, B->corr_off, B->corr_col, B->corr_val, A.pphi, A.pdphi, B->out);
+    STAGE_END(h, PYGBE_STAGE_NEAR);
+    return PYGBE_OK;
+}
+
+static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *skip)
+{
+    long before = h->launches;
+    for (Region &R : h->regions) {
+        if (R.np == 0 || R.twin_of >= 0) continue;
+        Region *B = R.twin >= 0 ? &h->regions[R.twin] : nullptr;
+        TRY(region_sum(h, R, B, x, skip));
+        STAGE(h, PYGBE_STAGE_COMBINE);
+        LAUNCH(h, k_combine, cdiv(R.np, 256), 256, 0, skip, R.np, R.row_idx, R.pphi, R.out, y);
+        if (B) LAUNCH(h, k_combine, cdiv(R.np, 256), 256, 0, skip, R.np, B->row_idx, R.pphi, B->out, y);
+        STAGE_END(h, PYGBE_STAGE_COMBINE);
+    }
+    stage_mark(h, -1);
+    h->kernels_per_matvec = h->launches - before;
+    h->n_matvec++;
+    return PYGBE_OK;
+}

@@ -27,23 +27,6 @@ __device__ __forceinline__ double pair_f64(double dx, double dy, double dz, doub
     }
 }
 
-template <bool YUKAWA>
-__device__ __forceinline__ float pair_f32(float dx, float dy, float dz, float mV, float mKx, float mKy,
-                                          float mKz, float kappa_log2e, float kappa)
-{
-    float r2 = dx * dx + dy * dy + dz * dz;
-    float rinv = r2 > 0.0f ? rsqrtf(r2) : 0.0f;
-    float mKd = mKx * dx + mKy * dy + mKz * dz;
-    float rinv2 = rinv * rinv;
-    if (!YUKAWA) {
-        return (mV - mKd * rinv2) * rinv;
-    } else {
-        float r = r2 * rinv;
-        float e = exp2f(-kappa_log2e * r);
-        return (mV - mKd * fmaf(kappa, r, 1.0f) * rinv2) * (rinv * e);
-    }
-}
-
 // ------------------------------------------------------------------------------- per-matvec weighting
 // Gather the densities of the region's panels from x and turn them into point "charges":
 //   mV_g = w_g A_j/(4pi) sigma_S c_S dphi_j,   mK_g = w_g A_j/(4pi) sigma_S phi_j n_j     (reading A4)
@@ -53,7 +36,7 @@ __global__ void k_prep(const int *__restrict__ skip, int np, int K, const double
                        const double *__restrict__ cK, const double4 *__restrict__ pnrm,
                        const double4 *__restrict__ spos, double4 *__restrict__ schg,
                        float4 *__restrict__ schgf, double *__restrict__ pphi, double *__restrict__ pdphi,
-                       double *__restrict__ out)
+                       double *__restrict__ out, double *__restrict__ out_twin)
 {
     if (skip && *skip) return;
     int p = blockIdx.x * blockDim.x + threadIdx.x;
@@ -61,6 +44,7 @@ __global__ void k_prep(const int *__restrict__ skip, int np, int K, const double
     double phi = x[phi_idx[p]], dphi = x[dphi_idx[p]];
     pphi[p] = phi; pdphi[p] = dphi;
     out[p] = 0.0;
+    if (out_twin) out_twin[p] = 0.0;
     double qV = cV[p] * dphi, qK = cK[p] * phi;
     double4 n = pnrm[p];
     for (int g = 0; g < K; g++) {
@@ -81,51 +65,6 @@ __global__ void k_combine(const int *__restrict__ skip, int np, const int *__res
     y[row_idx[p]] = 0.5 * pphi[p] - out[p];
 }
 
-// ------------------------------------------------------------------------------------------ P2P fp64
-// Work item = (target group, a run of chunked source panel ranges).  One thread per target; source points
-// are staged through shared memory in tiles (both double4 streams: position+weight, charges).
-#define P2P_TILE 256
-template <bool YUKAWA>
-__global__ void __launch_bounds__(PYGBE_TG)
-k_p2p_f64(const int *__restrict__ skip, const int4 *__restrict__ items, const int2 *__restrict__ sub, int K, int np,
-          const double4 *__restrict__ tpos, const double4 *__restrict__ spos,
-          const double4 *__restrict__ schg, double kappa, double *__restrict__ out)
-{
-    __shared__ double4 s_pos[P2P_TILE];
-    __shared__ double4 s_chg[P2P_TILE];
-    if (skip && *skip) return;
-    const int4 it = items[blockIdx.x];
-    const int t = it.x * PYGBE_TG + threadIdx.x;
-    const bool ok = t < np;
-    double4 X = ok ? tpos[t] : make_double4(0, 0, 0, 0);
-    double acc0 = 0.0, acc1 = 0.0;
-    for (int r = it.y; r < it.z; r++) {
-        int2 rg = sub[r];
-        long p0 = (long)rg.x * K, p1 = (long)rg.y * K;
-        for (long base = p0; base < p1; base += P2P_TILE) {
-            int n = (int)min((long)P2P_TILE, p1 - base);
-            __syncthreads();
-            for (int i = threadIdx.x; i < n; i += PYGBE_TG) {
-                s_pos[i] = spos[base + i];
-                s_chg[i] = schg[base + i];
-            }
-            __syncthreads();
-            int i = 0;
-            for (; i + 1 < n; i += 2) {
-                double4 a = s_pos[i], c = s_chg[i];
-                double4 a2 = s_pos[i + 1], c2 = s_chg[i + 1];
-                acc0 += pair_f64<YUKAWA>(X.x - a.x, X.y - a.y, X.z - a.z, c.x, c.y, c.z, c.w, kappa);
-                acc1 += pair_f64<YUKAWA>(X.x - a2.x, X.y - a2.y, X.z - a2.z, c2.x, c2.y, c2.z, c2.w, kappa);
-            }
-            if (i < n) {
-                double4 a = s_pos[i], c = s_chg[i];
-                acc0 += pair_f64<YUKAWA>(X.x - a.x, X.y - a.y, X.z - a.z, c.x, c.y, c.z, c.w, kappa);
-            }
-        }
-    }
-    if (ok) atomicAdd(out + t, acc0 + acc1);
-}
-
 // ------------------------------------------------------------------- singular / near-singular panels
 // Step 1: for each target, find the source panels of its group's P2P ranges that are the target's own
 // panel or lie inside the near-singular region |x_i - c_j|^2 < thres^2 * 2 A_j  (
@@ -133,7 +72,7 @@ k_p2p_f64(const int *__restrict__ skip, const int4 *__restrict__ items, const in
 __global__ void __launch_bounds__(PYGBE_TG)
 k_near_find(int np, const double4 *__restrict__ tpos, const double4 *__restrict__ pnrm,
             const int *__restrict__ p2p_off,
-            const int2 *__restrict__ p2p_rng, double thres2, int fill, int *__restrict__ cnt,
+            const int4 *__restrict__ p2p_rng, double thres2, int fill, int *__restrict__ cnt,
             const int *__restrict__ off, int *__restrict__ col)
 {
     int g = blockIdx.x;
@@ -143,7 +82,7 @@ k_near_find(int np, const double4 *__restrict__ tpos, const double4 *__restrict_
     int n = 0;
     int base = fill ? off[t] : 0;
     for (int r = p2p_off[g]; r < p2p_off[g + 1]; r++) {
-        int2 rg = p2p_rng[r];
+        int4 rg = p2p_rng[r];
         for (int j = rg.x; j < rg.y; j++) {
             double4 c = tpos[j];
             double dx = X.x - c.x, dy = X.y - c.y, dz = X.z - c.z;

@@ -1,0 +1,195 @@
+// solve.cuh -- right-hand side (a10), device-resident restarted GMRES driver (a11), energies (a12, a13).
+#pragma once
+#include "matvec.cuh"
+#include "gmres.cuh"
+
+static int ensure_host_staging(pygbe_handle *h)
+{
+    if (!h->xh) { TRY(h->mem.alloc(&h->xh, 2 * h->npan)); TRY(h->mem.alloc(&h->yh, 2 * h->npan)); }
+    return PYGBE_OK;
+}
+
+
+// ---------------------------------------------------------------------------------------------- rhs
+extern "C" int pygbe_rhs(pygbe_handle *h, double *b_dev)
+{
+    if (!h || !b_dev) { pygbe_set_error("rhs: null pointer"); return PYGBE_EINVAL; }
+    CUDA_TRY(cudaSetDevice(h->device));
+    CUDA_TRY(cudaMemsetAsync(b_dev, 0, 2 * h->npan * sizeof(double), h->stream));
+    const double inv4pi = 0.07957747154594767;
+    for (Region &R : h->regions) {
+        if (R.nq == 0 || R.np == 0) continue;
+        if (R.yukawa)
+            LAUNCH(h, k_rhs<true>, cdiv(R.np, 128), 128, 0, R.np, R.tpos, R.row_idx, R.nq, R.qpos, R.kappa, inv4pi / R.eps, b_dev);
+        else
+            LAUNCH(h, k_rhs<false>, cdiv(R.np, 128), 128, 0, R.np, R.tpos, R.row_idx, R.nq, R.qpos, R.kappa, inv4pi / R.eps, b_dev);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return PYGBE_OK;
+}
+
+// -------------------------------------------------------------------------------------------- gmres
+static int ensure_gmres(pygbe_handle *h, int m)
+{
+    GmresWork &G = h->gm;
+    long n = 2 * h->npan;
+    if (G.V && G.m >= m) return PYGBE_OK;
+    if (G.V) {
+        for (void *q : {(void *)G.V, (void *)G.H, (void *)G.h1, (void *)G.h2, (void *)G.cs, (void *)G.sn, (void *)G.g, (void *)G.yk})
+            h->mem.release_one(q);
+    }
+    G.m = m; G.n = n;
+    TRY(h->mem.alloc(&G.V, (size_t)(m + 1) * n));
+    TRY(h->mem.alloc(&G.H, (size_t)(m + 1) * m));
+    TRY(h->mem.alloc(&G.h1, m + 2)); TRY(h->mem.alloc(&G.h2, m + 2)); TRY(h->mem.alloc(&G.cs, m + 1));
+    TRY(h->mem.alloc(&G.sn, m + 1)); TRY(h->mem.alloc(&G.g, m + 2)); TRY(h->mem.alloc(&G.yk, m + 1));
+    if (!G.w) {
+        TRY(h->mem.alloc(&G.w, n)); TRY(h->mem.alloc(&G.b, n)); TRY(h->mem.alloc(&G.scal, 8)); TRY(h->mem.alloc(&G.flags, 4));
+    }
+    return PYGBE_OK;
+}
+
+extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t max_iter, double *x_dev,
+                           int32_t *iters, double *rel_resid)
+{
+    if (!h || !x_dev) { pygbe_set_error("solve: null pointer"); return PYGBE_EINVAL; }
+    if (!(tol > 0.0) || restart < 1 || max_iter < 1) { pygbe_set_error("solve: bad tol / restart / max_iter"); return PYGBE_EINVAL; }
+    CUDA_TRY(cudaSetDevice(h->device));
+    double t0 = now_ms();
+    const long n = 2 * h->npan;
+    const int m = std::min(restart, max_iter);
+    TRY(ensure_gmres(h, m));
+    GmresWork &G = h->gm;
+    const int ldh = G.m + 1;     // H was sized with G.m
+    (void)ldh;
+    cudaStream_t st = h->stream;
+    const int gridn = cdiv(n, GM_THREADS), gridd = cdiv(n, GM_ROWS_PER_CTA);
+    TRY(pygbe_rhs(h, G.b));
+    CUDA_TRY(cudaMemsetAsync(x_dev, 0, n * sizeof(double), st));
+    CUDA_TRY(cudaMemsetAsync(G.flags, 0, 4 * sizeof(int), st));
+    CUDA_TRY(cudaMemsetAsync(G.scal, 0, 8 * sizeof(double), st));
+    const int poll = n < 200000 ? 4 : 1;
+    int total = 0, done = 0;
+    bool first = true;
+    while (total < max_iter && !done) {
+        const int mc = std::min(m, max_iter - total);
+        if (!first) TRY(matvec_impl(h, x_dev, G.w, G.flags));
+        LAUNCH(h, k_gm_residual, gridn, GM_THREADS, 0, G.flags, n, G.b, G.w, first ? 0 : 1, G.V, G.scal);
+        LAUNCH(h, k_gm_begin, 1, 1, 0, G.flags, G.scal, G.g, G.m, first ? 1 : 0, tol);
+        LAUNCH(h, k_gm_scale, gridn, GM_THREADS, 0, G.flags, n, G.V, G.scal + 1, 0, G.V);
+        first = false;
+        int j = 0;
+        for (; j < mc; j++) {
+            double *vj = G.V + (size_t)j * n, *vn = G.V + (size_t)(j + 1) * n;
+            TRY(matvec_impl(h, vj, G.w, G.flags));
+            LAUNCH(h, k_gm_zero, cdiv(j + 2, 128), 128, 0, G.flags, G.h1, j + 1, G.h2, j + 1, G.scal + 3, 1);
+            LAUNCH(h, k_gm_dots, gridd, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.w, G.h1);
+            LAUNCH(h, k_gm_axpys, gridn, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.h1, G.w);
+            LAUNCH(h, k_gm_dots, gridd, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.w, G.h2);
+            LAUNCH(h, k_gm_axpys, gridn, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.h2, G.w);
+            LAUNCH(h, k_gm_dots, gridd, GM_THREADS, 0, G.flags, G.w, n, 1, G.w, G.scal + 3);
+            LAUNCH(h, k_gm_scale, gridn, GM_THREADS, 0, G.flags, n, G.w, G.scal + 3, 1, vn);
+            LAUNCH(h, k_gm_givens, 1, 1, 0, G.flags, j, G.m, G.h1, G.h2, G.scal + 3, G.H, G.cs, G.sn, G.g, G.scal, tol);
+            if ((j + 1) % poll == 0 || j + 1 == mc) {
+                CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+                CUDA_TRY(cudaStreamSynchronize(st));
+                if (h->pinned_flags[0]) { done = 1; break; }
+            }
+        }
+        LAUNCH(h, k_gm_solve_small, 1, 1, 0, G.flags, G.m, G.H, G.g, G.yk);
+        LAUNCH(h, k_gm_update, gridn, GM_THREADS, 0, G.flags, n, G.V, G.yk, x_dev);
+        CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaMemcpyAsync(h->pinned_scal, G.scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        done = h->pinned_flags[0];
+        total = h->pinned_flags[2];
+        if (!done) {
+            // new cycle: rotations and g restart; flags[1] is rewritten by the next givens
+            CUDA_TRY(cudaMemsetAsync(G.scal + 3, 0, sizeof(double), st));
+        }
+    }
+    CUDA_TRY(cudaGetLastError());
+    h->last_iters = total;
+    h->last_solve_ms = now_ms() - t0;
+    if (iters) *iters = total;
+    if (rel_resid) *rel_resid = h->pinned_scal[2];
+    if (!done) { pygbe_set_error("GMRES: %d iterations, relative residual %.3e > tol %.3e", total, h->pinned_scal[2], tol); return PYGBE_ENOCONV; }
+    return PYGBE_OK;
+}
+
+// ------------------------------------------------------------------------------------------- energy
+extern "C" int pygbe_reaction_potential(pygbe_handle *h, const double *x_dev, double *phi_dev)
+{
+    if (!h || !x_dev || !phi_dev) { pygbe_set_error("reaction_potential: null pointer"); return PYGBE_EINVAL; }
+    CUDA_TRY(cudaSetDevice(h->device));
+    if (h->nq == 0) return PYGBE_OK;
+    CUDA_TRY(cudaMemsetAsync(phi_dev, 0, h->nq * sizeof(double), h->stream));
+    for (Region &R : h->regions) {
+        if (R.nq == 0) continue;
+        LAUNCH(h, k_prep, cdiv(R.np, 128), 128, 0, nullptr, R.np, h->K, x_dev, R.phi_idx, R.dphi_idx, R.cV, R.cK, R.pnrm,
+               R.spos, R.schg, (float4 *)nullptr, R.pphi, R.pdphi, R.out, (double *)nullptr);
+        dim3 grid(cdiv(R.npts, EN_CHUNK), R.nq);
+        if (R.yukawa) LAUNCH(h, k_reaction<true>, grid, EN_THREADS, 0, R.npts, R.spos, R.schg, R.nq, R.qpos, R.qid, R.kappa, phi_dev);
+        else LAUNCH(h, k_reaction<false>, grid, EN_THREADS, 0, R.npts, R.spos, R.schg, R.nq, R.qpos, R.qid, R.kappa, phi_dev);
+    }
+    CUDA_TRY(cudaGetLastError());
+    return PYGBE_OK;
+}
+
+static double unit_C0()
+{   // reading A17: qe^2 N_A 1e-3 1e10 / eps0 in kJ Angstrom / (mol e^2); reproduces PAPER.md:229
+    const double qe = 1.60217646e-19, NA = 6.0221415e23, eps0 = 8.854187818e-12;
+    return qe * qe * NA * 1e7 / eps0;
+}
+
+extern "C" int pygbe_energy(pygbe_handle *h, const double *x_dev, double *E_solv, double *E_coul)
+{
+    if (!h || !x_dev) { pygbe_set_error("energy: null pointer"); return PYGBE_EINVAL; }
+    CUDA_TRY(cudaSetDevice(h->device));
+    const double C0 = unit_C0();
+    if (E_solv) *E_solv = 0.0;
+    if (E_coul) *E_coul = 0.0;
+    if (h->nq == 0) return PYGBE_OK;
+    if (E_solv) {
+        TRY(pygbe_reaction_potential(h, x_dev, h->phi_reac));
+        double *d_q;
+        TRY(h->mem.alloc(&d_q, h->nq));
+        CUDA_TRY(cudaMemcpyAsync(d_q, h->qq.data(), h->nq * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+        LAUNCH(h, k_dot_q, 1, 256, 0, (int)h->nq, d_q, h->phi_reac, h->scratch);
+        CUDA_TRY(cudaMemcpyAsync(h->pinned_scal, h->scratch, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+        h->mem.release_one(d_q);
+        *E_solv = 0.5 * C0 * h->pinned_scal[0];
+    }
+    if (E_coul) {
+        double tot = 0.0;
+        for (Region &R : h->regions) {
+            if (R.nq < 2) continue;
+            CUDA_TRY(cudaMemsetAsync(h->scratch + 1, 0, sizeof(double), h->stream));
+            LAUNCH(h, k_coulomb, cdiv(R.nq, 128), 128, 0, R.nq, R.qpos, h->scratch + 1);
+            CUDA_TRY(cudaMemcpyAsync(h->pinned_scal + 1, h->scratch + 1, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+            CUDA_TRY(cudaStreamSynchronize(h->stream));
+            tot += h->pinned_scal[1] / (4.0 * 3.14159265358979323846 * R.eps);
+        }
+        *E_coul = 0.5 * C0 * tot;
+    }
+    CUDA_TRY(cudaGetLastError());
+    return PYGBE_OK;
+}
+
+extern "C" int pygbe_solve_host(pygbe_handle *h, double tol, int32_t restart, int32_t max_iter, double *x_host,
+                                int32_t *iters, double *rel_resid, double *E_solv, double *E_coul)
+{
+    if (!h) { pygbe_set_error("solve_host: null handle"); return PYGBE_EINVAL; }
+    CUDA_TRY(cudaSetDevice(h->device));
+    TRY(ensure_host_staging(h));
+    int rc = pygbe_solve(h, tol, restart, max_iter, h->xh, iters, rel_resid);
+    if (rc != PYGBE_OK && rc != PYGBE_ENOCONV) return rc;
+    if (x_host) {
+        CUDA_TRY(cudaMemcpyAsync(x_host, h->xh, 2 * h->npan * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+    }
+    TRY(pygbe_energy(h, h->xh, E_solv, E_coul));
+    return rc;
+}
+

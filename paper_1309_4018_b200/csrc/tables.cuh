@@ -109,36 +109,27 @@ static int make_quad_tables(int K, int Kfine, int Nk, QuadTables *q)
 // ---------------------------------------------------------------------------------------------------
 // Multi-index tables.  Canonical order of the coefficients k = (kx,ky,kz), |k| <= P: by total order n,
 // then kx descending, then ky descending.  The first Nc(P') entries are the set for any P' <= PMAX.
-__constant__ unsigned char c_kxyz[PYGBE_NCMAX][4];                              // kx, ky, kz, n
-__constant__ short c_idx3[PYGBE_PMAX + 1][PYGBE_PMAX + 1][PYGBE_PMAX + 1];       // -> canonical index
-__constant__ double c_binom[PYGBE_PMAX + 1][PYGBE_PMAX + 1];
+// One copy lives in device memory per handle; kernels stage what they need into shared memory.
+struct IndexTables {
+    unsigned char kxyz[PYGBE_NCMAX][4];                              // kx, ky, kz, n
+    short idx3[PYGBE_PMAX + 1][PYGBE_PMAX + 1][PYGBE_PMAX + 1];       // -> canonical index (or -1)
+    double binom[PYGBE_PMAX + 1][PYGBE_PMAX + 1];
+};
 
-static int upload_index_tables()
+static void fill_index_tables(IndexTables *t)
 {
-    static bool done[64] = {false};
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (dev >= 0 && dev < 64 && done[dev]) return PYGBE_OK;
-    static unsigned char kxyz[PYGBE_NCMAX][4];
-    static short idx3[PYGBE_PMAX + 1][PYGBE_PMAX + 1][PYGBE_PMAX + 1];
-    static double binom[PYGBE_PMAX + 1][PYGBE_PMAX + 1];
-    memset(idx3, 0xff, sizeof(idx3));
+    memset(t->idx3, 0xff, sizeof(t->idx3));
     int at = 0;
     for (int n = 0; n <= PYGBE_PMAX; n++)
         for (int kx = n; kx >= 0; kx--)
             for (int ky = n - kx; ky >= 0; ky--) {
                 int kz = n - kx - ky;
-                kxyz[at][0] = kx; kxyz[at][1] = ky; kxyz[at][2] = kz; kxyz[at][3] = n;
-                idx3[kx][ky][kz] = (short)at++;
+                t->kxyz[at][0] = kx; t->kxyz[at][1] = ky; t->kxyz[at][2] = kz; t->kxyz[at][3] = n;
+                t->idx3[kx][ky][kz] = (short)at++;
             }
     for (int n = 0; n <= PYGBE_PMAX; n++)
         for (int m = 0; m <= PYGBE_PMAX; m++) {
-            if (m > n) { binom[n][m] = 0; continue; }
-            binom[n][m] = (m == 0 || m == n) ? 1.0 : binom[n - 1][m - 1] + binom[n - 1][m];
+            if (m > n) { t->binom[n][m] = 0; continue; }
+            t->binom[n][m] = (m == 0 || m == n) ? 1.0 : t->binom[n - 1][m - 1] + t->binom[n - 1][m];
         }
-    CUDA_TRY(cudaMemcpyToSymbol(c_kxyz, kxyz, sizeof(kxyz)));
-    CUDA_TRY(cudaMemcpyToSymbol(c_idx3, idx3, sizeof(idx3)));
-    CUDA_TRY(cudaMemcpyToSymbol(c_binom, binom, sizeof(binom)));
-    if (dev >= 0 && dev < 64) done[dev] = true;
-    return PYGBE_OK;
 }

@@ -196,7 +196,7 @@ k_group_geometry(const double4 *__restrict__ tpos, int np, double4 *__restrict__
 // the near-singular region is always contained in an area where the MAC criterion is not met"), when
 // additionally every panel centroid of the cell is farther than thres * Lmax from every target:
 //      |c_grp - y_c| - r_grp - (sqrt(3)/2) r_b > thres * Lmax.
-// Accepted cells go to the M2P list; leaves that fail go to the P2P list as panel ranges; other cells
+// Accepted cells go to the M2P list; leaves that fail go to the P2P list (as cell ids); other cells
 // are opened.  Pass 1 (fill == 0) counts, pass 2 writes.  The lane that owns child d of the popped
 // cell tests it; ballots keep the output order deterministic (Morton order).
 #define TRAV_WARPS 4
@@ -206,7 +206,7 @@ k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__
            const int2 *__restrict__ crange, const int2 *__restrict__ cchild, double theta,
            double near_dist, int fill, int *__restrict__ m2p_cnt, int *__restrict__ p2p_cnt,
            const int *__restrict__ m2p_off, const int *__restrict__ p2p_off, int *__restrict__ m2p_cell,
-           int2 *__restrict__ p2p_rng, int *overflow)
+           int *__restrict__ p2p_leaf, int *overflow)
 {
     __shared__ int s_stack[TRAV_WARPS][TRAV_STACK];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -221,7 +221,6 @@ k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__
     while (true) {
         int c = (lane < count) ? first + lane : -1;
         bool acc = false, leaf = false, open = false;
-        int2 rng = make_int2(0, 0);
         if (c >= 0) {
             double4 cg = cgeo[c];
             double dx = G.x - cg.x, dy = G.y - cg.y, dz = G.z - cg.z;
@@ -230,7 +229,6 @@ k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__
             if (!acc) {
                 leaf = cchild[c].y == 0;
                 open = !leaf;
-                if (leaf) rng = crange[c];
             }
         }
         unsigned ma = __ballot_sync(0xffffffffu, acc);
@@ -238,7 +236,7 @@ k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__
         unsigned mo = __ballot_sync(0xffffffffu, open);
         unsigned below = (1u << lane) - 1u;
         if (acc && fill) m2p_cell[mbase + nm + __popc(ma & below)] = c;
-        if (leaf && fill) p2p_rng[pbase + npp + __popc(ml & below)] = rng;
+        if (leaf && fill) p2p_leaf[pbase + npp + __popc(ml & below)] = c;
         nm += __popc(ma);
         npp += __popc(ml);
         // push the cells to open in reverse so that they pop in Morton order
