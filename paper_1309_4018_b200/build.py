@@ -17,6 +17,7 @@ LIB = os.path.join(HERE, "libpygbe.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+FLAGS += os.environ.get("PYGBE_CFLAGS", "").split()      # e.g. -DPYGBE_TG=64 for tuning experiments
 PMAX = 12
 
 
@@ -31,9 +32,9 @@ def _newest_source():
 def _compile(job):
     src, obj, extra = job
     if src.endswith("m2p_inst.cu"):
-        deps = [src, os.path.join(CSRC, "m2p.cuh")]
+        deps = [src, os.path.join(CSRC, "m2p.cuh"), os.path.join(CSRC, "mathx.cuh")]
     else:
-        deps = [src] + [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")]
+        deps = [src] + [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".inc"))]
         deps.append(os.path.join(HERE, "..", "include", "pygbe.h"))
     if os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(d) for d in deps):
         return obj, ""
@@ -53,8 +54,15 @@ def build(force=False, verbose=False):
             os.remove(os.path.join(OBJ, f))
     jobs = [(os.path.join(CSRC, "pygbe.cu"), os.path.join(OBJ, "pygbe.o"), [])]
     # the largest orders first: they take longest
+    # PYGBE_FAST_BUILD=<n>: development shortcut, orders above n are compiled as stubs that refuse to run
+    fast = int(os.environ.get("PYGBE_FAST_BUILD", "0"))
     for p in range(PMAX, 0, -1):
-        jobs.append((os.path.join(CSRC, "m2p_inst.cu"), os.path.join(OBJ, "m2p_%d.o" % p), ["-DM2P_P=%d" % p]))
+        extra = ["-DM2P_P=%d" % p]
+        name = "m2p_%d.o" % p
+        if fast and p > fast:
+            extra.append("-DM2P_STUB")
+            name = "m2p_%d_stub.o" % p
+        jobs.append((os.path.join(CSRC, "m2p_inst.cu"), os.path.join(OBJ, name), extra))
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         objs = [o for o, _ in ex.map(_compile, jobs)]
     if (not os.path.exists(LIB)) or os.path.getmtime(LIB) < max(os.path.getmtime(o) for o in objs):

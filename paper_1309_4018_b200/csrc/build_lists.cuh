@@ -90,7 +90,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
 
     // ---- target groups + traversal (count, offsets, fill)
     R.ng = cdiv(R.np, PYGBE_TG);
-    TRY(h->mem.alloc(&R.ggeo, R.ng));
+    TRY(h->mem.alloc(&R.ggeo, 2 * (size_t)R.ng));
     LAUNCH(h, k_group_geometry, R.ng, PYGBE_TG, 0, R.tpos, R.np, R.ggeo);
     int *d_mcnt, *d_pcnt, *d_over;
     TRY(h->mem.alloc(&d_mcnt, R.ng)); TRY(h->mem.alloc(&d_pcnt, R.ng)); TRY(h->mem.alloc(&d_over, 1));
@@ -110,6 +110,25 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
            h->theta, near_dist, 1, d_mcnt, d_pcnt, R.m2p_off, d_poff_raw, R.m2p_cell, d_pleaf_raw, d_over);
     std::vector<int> pleaf;
     TRY(download(h, pleaf, d_pleaf_raw, (size_t)poff[R.ng]));
+    {   // multipoles are needed for the listed cells and, to build those by M2M, for all their descendants
+        std::vector<int> mcell;
+        TRY(download(h, mcell, R.m2p_cell, (size_t)moff[R.ng]));
+        std::vector<char> need(ncells, 0);
+        for (int c : mcell) need[c] = 1;
+        for (int c = 1; c < ncells; c++)                  // parents precede children in the numbering
+            if (need[cparent_h[c]]) need[c] = 1;
+        std::vector<int> p2m_cells, m2m_cells;
+        for (int c : leaves) if (need[c]) p2m_cells.push_back(c);
+        R.m2m_off.assign(R.depth + 1, 0);
+        for (int l = 0; l < R.depth; l++) {
+            R.m2m_off[l] = (int)m2m_cells.size();
+            for (int c = R.level_begin[l]; c < R.level_begin[l + 1]; c++)
+                if (need[c] && cchild_h[c].y > 0) m2m_cells.push_back(c);
+        }
+        R.m2m_off[R.depth] = (int)m2m_cells.size();
+        R.n_p2m = (int)p2m_cells.size();
+        TRY(upload(h, &R.p2m_cells, p2m_cells)); TRY(upload(h, &R.m2m_cells, m2m_cells));
+    }
     int over = 0;
     CUDA_TRY(cudaMemcpy(&over, d_over, sizeof(int), cudaMemcpyDeviceToHost));
     if (over) { pygbe_set_error("traversal stack overflow"); return PYGBE_ECUDA; }
@@ -147,7 +166,8 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     // ---- work items of bounded size, enough of them to fill 148 SMs several times over
     const long want_items = 148L * 16;
     int p2p_item = (int)std::min(512L, std::max(32L, total_src_panels / want_items));
-    int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[R.ng] / want_items));
+    // M2P CTAs keep only 8-16 warps per SM resident (72-127 registers): finer items even out the tail
+    int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[R.ng] / (3 * want_items)));
     m2p_item = (m2p_item + 3) / 4 * 4;
     std::vector<int4> sub, pitems, mitems;
     for (int g = 0; g < R.ng; g++) {

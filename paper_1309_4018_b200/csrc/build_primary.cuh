@@ -63,7 +63,10 @@ static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<do
         h->mem.release_one(q);
     TRY(build_tree_and_lists(h, R));
     TRY(build_corrections(h, R, qt, nullptr));
-    if (R.n_m2p_items > 0) TRY(h->mem.alloc(&R.mom, (size_t)R.ncells * 2 * h->Nc));
+    if (R.n_m2p_items > 0) {
+        TRY(h->mem.alloc(&R.mom, (size_t)R.ncells * 2 * h->Nc));
+        TRY(h->mem.alloc((char **)&R.momc, (size_t)R.ncells * ((h->Nc + 3) / 4 * 4) * sizeof(double)));
+    }
     CUDA_TRY(cudaGetLastError());
     return PYGBE_OK;
 }

@@ -14,7 +14,9 @@
 
 #define PYGBE_PMAX 12
 #define PYGBE_NCMAX 455              // (P+1)(P+2)(P+3)/6 at P = 12
-#define PYGBE_TG 128                 // targets per group = threads per CTA of the P2P / M2P kernels
+#ifndef PYGBE_TG
+#define PYGBE_TG 64                  // targets per group = threads per CTA of the P2P / M2P kernels
+#endif
 #define PYGBE_MAXLEVEL 21            // 21 bits per dimension in the 63-bit Morton key
 
 void pygbe_set_error(const char *fmt, ...);
@@ -114,6 +116,10 @@ struct Region {
     unsigned long long *ckey = nullptr;
     std::vector<int> level_begin;   // host: cells of level l are [level_begin[l], level_begin[l+1])
     int *leaf_cell = nullptr;       // leaves in Morton order
+    // cells whose multipoles are needed: those in some M2P list and all their descendants
+    int *p2m_cells = nullptr; int n_p2m = 0;        // needed leaves (P2M)
+    int *m2m_cells = nullptr;                       // needed internal cells, grouped by level
+    std::vector<int> m2m_off;                       // host: level l -> [m2m_off[l], m2m_off[l+1])
     double Lmax = 0;                // max panel length sqrt(2A) on this region's boundary
     double root_c[3] = {0, 0, 0}, root_edge = 1;
     // target groups and interaction lists -----------------------------------------------------------
@@ -128,7 +134,8 @@ struct Region {
     int4 *m2p_items = nullptr;      // (group, first list slot, last slot+1, unused)
     long p2p_pairs = 0, m2p_evals = 0;
     // multipoles ------------------------------------------------------------------------------------
-    double *mom = nullptr;          // [ncells][2][Nc]: MV, MK (farfield.cuh)
+    double *mom = nullptr;          // [ncells][2][Nc]: MV, MK (farfield.cuh), shared by twin regions
+    void *momc = nullptr;           // [ncells][m2p_stride(Nc)]: this region's ca MV + cb MK in float or double
     // singular / near-singular corrections (CSR over targets) ----------------------------------------
     int *corr_off = nullptr, *corr_col = nullptr;
     double2 *corr_val = nullptr;    // (sigma c (fine - coarse)_V, sigma (fine - coarse)_K)

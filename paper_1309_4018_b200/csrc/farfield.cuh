@@ -82,83 +82,71 @@ k_p2m(const int *__restrict__ skip, int P, int Nc, int K, const IndexTables *__r
 // Parent moments from the children's ("shifted and added"), for both sets:
 //   M_p^k = sum_children sum_{l <= k} C(k,l) s^(k-l) M_c^l,   s = y_child - y_parent.
 // The shift factorises over the axes, so it is applied as three one-dimensional shifts (x, then y, then z)
-// through two shared-memory buffers: O(Nc P) work per child instead of O(Nc P^3).  The index tables are
-// staged in shared memory (the first version read them from constant memory with divergent indices and
-// was latency-bound: 62 us per launch, profiles/r1a_first_path.md).  One CTA per non-leaf cell of the
-// level; launched level by level from the deepest upward.
-#define M2M_THREADS 256
-#define M2M_SLOTS ((2 * PYGBE_NCMAX + M2M_THREADS - 1) / M2M_THREADS)
+// through two shared-memory buffers: O(Nc P) work per child instead of O(Nc P^3).  All children of a parent
+// are shifted concurrently (work item = (child, coefficient)), then summed.  The index tables are staged
+// in shared memory (the first version read them from constant memory with divergent indices and was
+// latency-bound: 62 us per launch, profiles/r1a_first_path.md).  One CTA per listed parent cell; launched
+// level by level from the deepest upward, and only for the cells whose multipoles are used: those in
+// some M2P list and, to build those, all their descendants (build_lists.cuh).
+// Dynamic shared memory: 2 buffers x 8 children x 2 Nc doubles.
+#define M2M_THREADS 512
+static inline size_t m2m_smem_bytes(int Nc) { return (size_t)2 * 8 * 2 * Nc * sizeof(double); }
 __global__ void __launch_bounds__(M2M_THREADS)
-k_m2m(const int *__restrict__ skip, int P, int Nc, int cell_begin, int cell_end,
-      const IndexTables *__restrict__ tab, const double4 *__restrict__ cgeo, const int2 *__restrict__ cchild,
-      double *__restrict__ mom)
+k_m2m(const int *__restrict__ skip, int P, int Nc, const int *__restrict__ cells, const IndexTables *__restrict__ tab,
+      const double4 *__restrict__ cgeo, const int2 *__restrict__ cchild, double *__restrict__ mom)
 {
-    __shared__ double s_a[2 * PYGBE_NCMAX], s_b[2 * PYGBE_NCMAX];
-    __shared__ double s_pw[3][PYGBE_PMAX + 1];
+    extern __shared__ double s_dyn[];
+    __shared__ double s_pw[8][3][PYGBE_PMAX + 1];
     __shared__ double s_binom[PYGBE_PMAX + 1][PYGBE_PMAX + 1];
     __shared__ short s_idx3[PYGBE_PMAX + 1][PYGBE_PMAX + 1][PYGBE_PMAX + 1];
+    __shared__ __align__(16) unsigned char s_k[PYGBE_NCMAX][4];
     if (skip && *skip) return;
-    const int cell = cell_begin + blockIdx.x;
-    if (cell >= cell_end) return;
+    const int cell = cells[blockIdx.x];
     const int2 ch = cchild[cell];
-    if (ch.y == 0) return;                       // leaf: filled by P2M
+    const int n2 = 2 * Nc, nch = ch.y, nw = nch * n2;
+    double *s_a = s_dyn, *s_b = s_dyn + 8 * n2;
     for (int i = threadIdx.x; i < (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1); i += M2M_THREADS)
         (&s_binom[0][0])[i] = (&tab->binom[0][0])[i];
     for (int i = threadIdx.x; i < (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1); i += M2M_THREADS)
         (&s_idx3[0][0][0])[i] = (&tab->idx3[0][0][0])[i];
-    const double4 pg = cgeo[cell];
-    const int n2 = 2 * Nc;
-    double acc[M2M_SLOTS];
-    int kx[M2M_SLOTS], ky[M2M_SLOTS], kz[M2M_SLOTS], so[M2M_SLOTS];
-#pragma unroll
-    for (int s = 0; s < M2M_SLOTS; s++) {
-        acc[s] = 0.0;
-        int e = threadIdx.x + s * M2M_THREADS;
-        int k = e < Nc ? e : e - Nc;
-        so[s] = e < Nc ? 0 : Nc;
-        if (e < n2) { kx[s] = tab->kxyz[k][0]; ky[s] = tab->kxyz[k][1]; kz[s] = tab->kxyz[k][2]; }
-        else { kx[s] = ky[s] = kz[s] = 0; }
+    for (int i = threadIdx.x; i < Nc; i += M2M_THREADS)
+        *(uchar4 *)s_k[i] = *(const uchar4 *)tab->kxyz[i];
+    for (int w = threadIdx.x; w < nw; w += M2M_THREADS) s_a[w] = mom[(long)ch.x * n2 + w];   // children are contiguous
+    if (threadIdx.x < nch * 3) {
+        const int c = threadIdx.x / 3, a = threadIdx.x - 3 * c;
+        const double4 g = cgeo[ch.x + c], pg = cgeo[cell];
+        const double sft = a == 0 ? g.x - pg.x : (a == 1 ? g.y - pg.y : g.z - pg.z);
+        double pw = 1.0;
+        for (int e = 0; e <= P; e++) { s_pw[c][a][e] = pw; pw *= sft; }
     }
-    for (int c = ch.x; c < ch.x + ch.y; c++) {
-        __syncthreads();
-        for (int i = threadIdx.x; i < n2; i += M2M_THREADS) s_a[i] = mom[(long)c * n2 + i];
-        if (threadIdx.x < 3) {
-            double4 g = cgeo[c];
-            double sft = threadIdx.x == 0 ? g.x - pg.x : (threadIdx.x == 1 ? g.y - pg.y : g.z - pg.z);
-            double pw = 1.0;
-            for (int e = 0; e <= P; e++) { s_pw[threadIdx.x][e] = pw; pw *= sft; }
-        }
-        __syncthreads();
-#pragma unroll
-        for (int s = 0; s < M2M_SLOTS; s++) {            // shift along x: s_a -> s_b
-            int e = threadIdx.x + s * M2M_THREADS;
-            if (e >= n2) break;
-            double a = 0.0;
-            for (int l = 0; l <= kx[s]; l++) a += s_binom[kx[s]][l] * s_pw[0][kx[s] - l] * s_a[so[s] + s_idx3[l][ky[s]][kz[s]]];
-            s_b[e] = a;
-        }
-        __syncthreads();
-#pragma unroll
-        for (int s = 0; s < M2M_SLOTS; s++) {            // shift along y: s_b -> s_a
-            int e = threadIdx.x + s * M2M_THREADS;
-            if (e >= n2) break;
-            double a = 0.0;
-            for (int l = 0; l <= ky[s]; l++) a += s_binom[ky[s]][l] * s_pw[1][ky[s] - l] * s_b[so[s] + s_idx3[kx[s]][l][kz[s]]];
-            s_a[e] = a;
-        }
-        __syncthreads();
-#pragma unroll
-        for (int s = 0; s < M2M_SLOTS; s++) {            // shift along z: s_a -> accumulator
-            int e = threadIdx.x + s * M2M_THREADS;
-            if (e >= n2) break;
-            double a = 0.0;
-            for (int l = 0; l <= kz[s]; l++) a += s_binom[kz[s]][l] * s_pw[2][kz[s] - l] * s_a[so[s] + s_idx3[kx[s]][ky[s]][l]];
-            acc[s] += a;
-        }
+    __syncthreads();
+    for (int w = threadIdx.x; w < nw; w += M2M_THREADS) {          // shift along x: s_a -> s_b
+        const int c = w / n2, e = w - c * n2, so = c * n2 + (e < Nc ? 0 : Nc), k = e < Nc ? e : e - Nc;
+        const int kx = s_k[k][0], ky = s_k[k][1], kz = s_k[k][2];
+        double a = 0.0;
+        for (int l = 0; l <= kx; l++) a += s_binom[kx][l] * s_pw[c][0][kx - l] * s_a[so + s_idx3[l][ky][kz]];
+        s_b[w] = a;
     }
-#pragma unroll
-    for (int s = 0; s < M2M_SLOTS; s++) {
-        int e = threadIdx.x + s * M2M_THREADS;
-        if (e < n2) mom[(long)cell * n2 + e] = acc[s];
+    __syncthreads();
+    for (int w = threadIdx.x; w < nw; w += M2M_THREADS) {          // shift along y: s_b -> s_a
+        const int c = w / n2, e = w - c * n2, so = c * n2 + (e < Nc ? 0 : Nc), k = e < Nc ? e : e - Nc;
+        const int kx = s_k[k][0], ky = s_k[k][1], kz = s_k[k][2];
+        double a = 0.0;
+        for (int l = 0; l <= ky; l++) a += s_binom[ky][l] * s_pw[c][1][ky - l] * s_b[so + s_idx3[kx][l][kz]];
+        s_a[w] = a;
+    }
+    __syncthreads();
+    for (int w = threadIdx.x; w < nw; w += M2M_THREADS) {          // shift along z: s_a -> s_b
+        const int c = w / n2, e = w - c * n2, so = c * n2 + (e < Nc ? 0 : Nc), k = e < Nc ? e : e - Nc;
+        const int kx = s_k[k][0], ky = s_k[k][1], kz = s_k[k][2];
+        double a = 0.0;
+        for (int l = 0; l <= kz; l++) a += s_binom[kz][l] * s_pw[c][2][kz - l] * s_a[so + s_idx3[kx][ky][l]];
+        s_b[w] = a;
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < n2; e += M2M_THREADS) {          // sum over the children
+        double a = 0.0;
+        for (int c = 0; c < nch; c++) a += s_b[c * n2 + e];
+        mom[(long)cell * n2 + e] = a;
     }
 }

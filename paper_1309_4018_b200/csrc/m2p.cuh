@@ -3,15 +3,30 @@
 #pragma once
 #include <cuda_runtime.h>
 #include "mathx.cuh"
-#define PYGBE_TG_M2P 128
+#ifndef PYGBE_TG
+#define PYGBE_TG 64
+#endif
+#define PYGBE_TG_M2P PYGBE_TG
+
+// Row stride of the combined moments momc[cell][stride] (elements of T): Nc padded to a multiple of 4 so
+// that every row starts on a 16-byte boundary and can be moved with 16-byte cp.async.
+static inline __host__ __device__ int m2p_stride(int Nc) { return (Nc + 3) / 4 * 4; }
 
 struct M2PArgs {
     const int *skip; const int4 *items; const int *m2p_cell; int n_items; int np;
-    const double4 *tpos; const double4 *cgeo; const double *mom;   // mom[cell][2][Nc]: MV, MK (farfield.cuh)
-    double ca, cb;             // the region's multipole is ca * MV + cb * MK
+    const double4 *tpos; const double4 *cgeo;
+    const void *momc;          // the region's multipoles ca * MV + cb * MK, already in T (k_mom_combine)
     double kappa; double *out;
     int yukawa; int fp32; cudaStream_t stream;
 };
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // Taylor coefficients by recurrence ("recursive relations for the Green's function of
 // the Poisson equation [20] and linearized Poisson-Boltzmann equation [21]"; reading A13), d = x - y_c,
@@ -82,37 +97,66 @@ __device__ __forceinline__ T m2p_eval(T dx, T dy, T dz, T kappa, T kscaled, cons
 // at a time are staged in shared memory (combined ca MV + cb MK, converted to T) and read by all threads
 // as broadcasts.  The target offset d = x - y_c is always formed in fp64 and then rounded to T, so the
 // fp32 path never subtracts large absolute coordinates; accumulation over cells is fp64.
+// The batches are double-buffered with cp.async (LDGSTS): while the threads evaluate the recurrences of one
+// batch, the moments and centres of the next one stream from L2 into the other buffer (capture r1b showed
+// 7-9 % barrier + 5-9 % long-scoreboard stalls with synchronous staging at 2 warps per CTA).
 #define M2P_CB 4
 template <int P, bool YUKAWA, typename T>
 __global__ void __launch_bounds__(PYGBE_TG_M2P)
 k_m2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
-      const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const double *__restrict__ mom,
-      double ca, double cb, double kappa, double kscaled, double *__restrict__ out)
+      const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const T *__restrict__ momc,
+      double kappa, double kscaled, double *__restrict__ out)
 {
     constexpr int Nc = (P + 1) * (P + 2) * (P + 3) / 6;
-    __shared__ T s_M[M2P_CB][Nc];
-    __shared__ double4 s_c[M2P_CB];
+    constexpr int NCS = (Nc + 3) / 4 * 4;                    // = m2p_stride(Nc)
+    constexpr int EPC = 16 / (int)sizeof(T);                 // elements per 16-byte chunk
+    constexpr int CH = NCS / EPC;                            // chunks per cell
+    __shared__ __align__(16) T s_M[2][M2P_CB][NCS];
+    __shared__ __align__(16) double4 s_c[2][M2P_CB];
     if (skip && *skip) return;
     const int4 it = items[blockIdx.x];
     const int t = it.x * PYGBE_TG_M2P + threadIdx.x;
     const bool ok = t < np;
-    double4 X = ok ? tpos[t] : make_double4(1e30, 1e30, 1e30, 0);
+    const double4 X = ok ? tpos[t] : make_double4(1e30, 1e30, 1e30, 0);
     double acc = 0.0;
-    for (int s0 = it.y; s0 < it.z; s0 += M2P_CB) {
-        int nb = min(M2P_CB, it.z - s0);
-        __syncthreads();
-        for (int i = threadIdx.x; i < nb * Nc; i += PYGBE_TG_M2P) {
-            int cb_ = i / Nc, k = i - cb_ * Nc;
-            const double *m = mom + (long)m2p_cell[s0 + cb_] * 2 * Nc;
-            s_M[cb_][k] = (T)(ca * m[k] + cb * m[Nc + k]);
+    auto stage = [&](int buf, int s0) {
+        const int nb = min(M2P_CB, it.z - s0);
+        for (int i = threadIdx.x; i < nb * CH; i += PYGBE_TG_M2P) {
+            const int c_ = i / CH, j = i - c_ * CH;
+            cp_async16(&s_M[buf][c_][j * EPC], momc + (long)m2p_cell[s0 + c_] * NCS + j * EPC);
         }
-        if (threadIdx.x < nb) s_c[threadIdx.x] = cgeo[m2p_cell[s0 + threadIdx.x]];
+        if (threadIdx.x < nb * 2) {
+            const int c_ = threadIdx.x >> 1, hf = threadIdx.x & 1;
+            cp_async16((char *)&s_c[buf][c_] + 16 * hf, (const char *)(cgeo + m2p_cell[s0 + c_]) + 16 * hf);
+        }
+        cp_async_commit();
+    };
+    stage(0, it.y);
+    int buf = 0;
+    for (int s0 = it.y; s0 < it.z; s0 += M2P_CB, buf ^= 1) {
+        const int nb = min(M2P_CB, it.z - s0);
+        const bool more = s0 + M2P_CB < it.z;
+        if (more) { stage(buf ^ 1, s0 + M2P_CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
         __syncthreads();
         for (int c_ = 0; c_ < nb; c_++) {
-            double4 c = s_c[c_];
+            const double4 c = s_c[buf][c_];
             acc += (double)m2p_eval<P, YUKAWA, T>((T)(X.x - c.x), (T)(X.y - c.y), (T)(X.z - c.z), (T)kappa,
-                                                  (T)kscaled, s_M[c_]);
+                                                  (T)kscaled, s_M[buf][c_]);
         }
+        __syncthreads();                                     // buf is refilled two iterations from now
     }
     if (ok) atomicAdd(out + t, acc);
+}
+
+// momc[cell][k] = (T)(ca MV^k + cb MK^k): the multipoles of one region in the arithmetic type of its M2P.
+template <typename T>
+__global__ void k_mom_combine(const int *__restrict__ skip, long ncells, int Nc, int stride,
+                              const double *__restrict__ mom, double ca, double cb, T *__restrict__ momc)
+{
+    if (skip && *skip) return;
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (i >= ncells * stride) return;
+    long cell = i / stride;
+    int k = (int)(i - cell * stride);
+    momc[i] = k < Nc ? (T)(ca * mom[cell * 2 * Nc + k] + cb * mom[(cell * 2 + 1) * Nc + k]) : T(0);
 }

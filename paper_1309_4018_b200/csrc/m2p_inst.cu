@@ -6,10 +6,13 @@
 #define CAT_(a, b) a##b
 #define CAT(a, b) CAT_(a, b)
 
+#ifdef M2P_STUB
+int CAT(pygbe_m2p_launch_, M2P_P)(const M2PArgs &) { return -1; }
+#else
 template <bool Y, typename T> static void launch(const M2PArgs &a)
 {
-    k_m2p<M2P_P, Y, T><<<a.n_items, PYGBE_TG_M2P, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo, a.mom,
-                                                                 a.ca, a.cb, a.kappa, Real<T>::kscale(a.kappa), a.out);
+    k_m2p<M2P_P, Y, T><<<a.n_items, PYGBE_TG_M2P, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo,
+                                                                 (const T *)a.momc, a.kappa, Real<T>::kscale(a.kappa), a.out);
 }
 
 int CAT(pygbe_m2p_launch_, M2P_P)(const M2PArgs &a)
@@ -18,3 +21,4 @@ int CAT(pygbe_m2p_launch_, M2P_P)(const M2PArgs &a)
     else { if (a.yukawa) launch<true, double>(a); else launch<false, double>(a); }
     return 0;
 }
+#endif

@@ -35,17 +35,23 @@ M2P_DECL(7) M2P_DECL(8) M2P_DECL(9) M2P_DECL(10) M2P_DECL(11) M2P_DECL(12)
 // M2P of region R with the multipoles ca MV + cb MK of the tree owner T, on stream st.
 static int launch_m2p(pygbe_handle *h, Region &T, Region &R, double ca, double cb, const int *skip, cudaStream_t st)
 {
+    const bool fp32 = h->precision == PYGBE_PRECISION_MIXED;
+    const int stride = m2p_stride(h->Nc);
+    const long nel = (long)T.ncells * stride;
+    // the region's multipoles in the arithmetic type of its M2P (LAUNCH issues on h->stream == st here)
+    if (fp32) LAUNCH(h, k_mom_combine<float>, cdiv(nel, 256), 256, 0, skip, (long)T.ncells, h->Nc, stride, T.mom, ca, cb, (float *)R.momc);
+    else LAUNCH(h, k_mom_combine<double>, cdiv(nel, 256), 256, 0, skip, (long)T.ncells, h->Nc, stride, T.mom, ca, cb, (double *)R.momc);
     M2PArgs a;
     memset(&a, 0, sizeof(a));
     a.skip = skip; a.items = T.m2p_items; a.m2p_cell = T.m2p_cell; a.n_items = T.n_m2p_items; a.np = T.np;
-    a.tpos = T.tpos; a.cgeo = T.cgeo; a.mom = T.mom; a.ca = ca; a.cb = cb; a.kappa = R.kappa; a.out = R.out;
-    a.yukawa = R.yukawa; a.fp32 = h->precision == PYGBE_PRECISION_MIXED; a.stream = st;
+    a.tpos = T.tpos; a.cgeo = T.cgeo; a.momc = R.momc; a.kappa = R.kappa; a.out = R.out;
+    a.yukawa = R.yukawa; a.fp32 = fp32; a.stream = st;
     typedef int (*fn_t)(const M2PArgs &);
     static const fn_t table[PYGBE_PMAX + 1] = {nullptr, pygbe_m2p_launch_1, pygbe_m2p_launch_2, pygbe_m2p_launch_3,
         pygbe_m2p_launch_4, pygbe_m2p_launch_5, pygbe_m2p_launch_6, pygbe_m2p_launch_7, pygbe_m2p_launch_8,
         pygbe_m2p_launch_9, pygbe_m2p_launch_10, pygbe_m2p_launch_11, pygbe_m2p_launch_12};
     if (h->P < 1 || h->P > PYGBE_PMAX) { pygbe_set_error("P = %d not instantiated", h->P); return PYGBE_EINVAL; }
-    table[h->P](a);
+    if (table[h->P](a) != 0) { pygbe_set_error("M2P order %d was compiled as a stub (PYGBE_FAST_BUILD)", h->P); return PYGBE_EINVAL; }
     h->launches++;
     return PYGBE_OK;
 }
@@ -68,8 +74,8 @@ static void launch_p2p(pygbe_handle *h, Region &A, Region *B, const int *skip)
 #undef P2P_GO
 }
 
-// Everything of one tree owner A (and its twin B, if any) except the final combination.
-static int region_sum(pygbe_handle *h, Region &A, Region *B, const double *x, const int *skip)
+// The rows of one tree owner A (and of its twin B, if any).
+static int region_sum(pygbe_handle *h, Region &A, Region *B, const double *x, double *y, const int *skip)
 {
     if (A.np == 0) return PYGBE_OK;
     const bool mixed = h->precision == PYGBE_PRECISION_MIXED;
@@ -85,13 +91,16 @@ static int region_sum(pygbe_handle *h, Region &A, Region *B, const double *x, co
         cudaStream_t keep = h->stream;
         h->stream = fs;                      // LAUNCH issues on h->stream
         STAGE(h, PYGBE_STAGE_P2M);
-        LAUNCH(h, k_p2m, A.nleaves, P2M_THREADS, 0, skip, h->P, h->Nc, h->K, h->itab, A.leaf_cell, A.cgeo, A.crange,
-               A.spos, A.schg, A.mom);
+        if (A.n_p2m > 0)
+            LAUNCH(h, k_p2m, A.n_p2m, P2M_THREADS, 0, skip, h->P, h->Nc, h->K, h->itab, A.p2m_cells, A.cgeo, A.crange,
+                   A.spos, A.schg, A.mom);
         STAGE_END(h, PYGBE_STAGE_P2M);
         STAGE(h, PYGBE_STAGE_M2M);
-        for (int l = A.depth - 2; l >= 0; l--) {
-            int b = A.level_begin[l], e = A.level_begin[l + 1];
-            LAUNCH(h, k_m2m, e - b, M2M_THREADS, 0, skip, h->P, h->Nc, b, e, h->itab, A.cgeo, A.cchild, A.mom);
+        for (int l = A.depth - 2; l >= 0; l--) {           // only the cells some M2P list depends on
+            int b = A.m2m_off[l], e = A.m2m_off[l + 1];
+            if (e > b)
+                LAUNCH(h, k_m2m, e - b, M2M_THREADS, m2m_smem_bytes(h->Nc), skip, h->P, h->Nc, A.m2m_cells + b, h->itab,
+                       A.cgeo, A.cchild, A.mom);
         }
         STAGE_END(h, PYGBE_STAGE_M2M);
         STAGE(h, PYGBE_STAGE_M2P);
@@ -108,8 +117,9 @@ static int region_sum(pygbe_handle *h, Region &A, Region *B, const double *x, co
     }
     if (fork) cudaStreamWaitEvent(main_st, h->ev_join, 0);
     STAGE(h, PYGBE_STAGE_NEAR);
-    LAUNCH(h, k_near_apply, cdiv(A.np, 128), 128, 0, skip, A.np, A.corr_off, A.corr_col, A.corr_val, A.pphi, A.pdphi, A.out);
-    if (B) LAUNCH(h, k_near_apply, cdiv(A.np, 128), 128, 0, skip, A.np, B->corr_off, B->corr_col, B->corr_val, A.pphi, A.pdphi, B->out);
+    LAUNCH(h, k_near_combine, cdiv(A.np, 128), 128, 0, skip, A.np, A.corr_off, A.corr_col, A.corr_val,
+           B ? B->corr_val : (const double2 *)nullptr, A.pphi, A.pdphi, A.out, B ? B->out : (const double *)nullptr,
+           A.row_idx, B ? B->row_idx : (const int *)nullptr, y);
     STAGE_END(h, PYGBE_STAGE_NEAR);
     return PYGBE_OK;
 }
@@ -120,11 +130,7 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
     for (Region &R : h->regions) {
         if (R.np == 0 || R.twin_of >= 0) continue;
         Region *B = R.twin >= 0 ? &h->regions[R.twin] : nullptr;
-        TRY(region_sum(h, R, B, x, skip));
-        STAGE(h, PYGBE_STAGE_COMBINE);
-        LAUNCH(h, k_combine, cdiv(R.np, 256), 256, 0, skip, R.np, R.row_idx, R.pphi, R.out, y);
-        if (B) LAUNCH(h, k_combine, cdiv(R.np, 256), 256, 0, skip, R.np, B->row_idx, R.pphi, B->out, y);
-        STAGE_END(h, PYGBE_STAGE_COMBINE);
+        TRY(region_sum(h, R, B, x, y, skip));
     }
     stage_mark(h, -1);
     h->kernels_per_matvec = h->launches - before;

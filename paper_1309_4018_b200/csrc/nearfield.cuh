@@ -198,6 +198,40 @@ __global__ void k_near_apply(const int *__restrict__ skip, int np, const int *__
     out[t] += acc;
 }
 
+// Correction SpMV (a8) fused with the block combination (a9) for a region and, optionally, its twin (same
+// sparsity pattern, own values):  y[row] = 1/2 phi - ( out + sum_e [ val.x dphi_j - val.y phi_j ] ).
+__global__ void k_near_combine(const int *__restrict__ skip, int np, const int *__restrict__ off,
+                               const int *__restrict__ col, const double2 *__restrict__ valA,
+                               const double2 *__restrict__ valB, const double *__restrict__ pphi,
+                               const double *__restrict__ pdphi, const double *__restrict__ outA,
+                               const double *__restrict__ outB, const int *__restrict__ rowA,
+                               const int *__restrict__ rowB, double *__restrict__ y)
+{
+    if (skip && *skip) return;
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= np) return;
+    double accA = 0.0, accB = 0.0;
+    const int e0 = off[t], e1 = off[t + 1];
+    if (valB) {
+        for (int e = e0; e < e1; e++) {
+            int j = col[e];
+            double ph = pphi[j], dp = pdphi[j];
+            double2 a = valA[e], b = valB[e];
+            accA += a.x * dp - a.y * ph;
+            accB += b.x * dp - b.y * ph;
+        }
+    } else {
+        for (int e = e0; e < e1; e++) {
+            int j = col[e];
+            double2 a = valA[e];
+            accA += a.x * pdphi[j] - a.y * pphi[j];
+        }
+    }
+    const double half_phi = 0.5 * pphi[t];
+    y[rowA[t]] = half_phi - (outA[t] + accA);
+    if (valB) y[rowB[t]] = half_phi - (outB[t] + accB);
+}
+
 // ------------------------------------------------------------------------------------------------ RHS
 // b[row(Omega,T,i)] = sum_{k in Omega} q_k G_Omega(x_i, r_k) / eps_Omega   (eq. 9 / 11).
 #define RHS_TILE 256

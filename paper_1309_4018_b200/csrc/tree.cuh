@@ -160,7 +160,8 @@ k_split_level(const unsigned long long *__restrict__ keys, int level, int lvl_be
 
 // ------------------------------------------------------------------------------------ target groups
 // A group = PYGBE_TG Morton-consecutive collocation points (reading A9: the MAC is tested for the
-// whole group against its bounding sphere, which is stricter than the per-target test of eq. 15).
+// whole group against its bounding sphere and bounding box, which is stricter than the per-target test
+// of eq. 15).  ggeo[2g] = (centre, radius), ggeo[2g+1] = half extents of the box about the same centre.
 __global__ void __launch_bounds__(PYGBE_TG)
 k_group_geometry(const double4 *__restrict__ tpos, int np, double4 *__restrict__ ggeo)
 {
@@ -185,17 +186,21 @@ k_group_geometry(const double4 *__restrict__ tpos, int np, double4 *__restrict__
     double dx = x.x - s_c[0], dy = x.y - s_c[1], dz = x.z - s_c[2];
     double r = ok ? sqrt(dx * dx + dy * dy + dz * dz) : 0.0;
     double rmax = Red(tmp).Reduce(r, cub::Max());
-    if (threadIdx.x == 0) ggeo[g] = make_double4(s_c[0], s_c[1], s_c[2], rmax);
+    if (threadIdx.x == 0) {
+        ggeo[2 * g] = make_double4(s_c[0], s_c[1], s_c[2], rmax);
+        ggeo[2 * g + 1] = make_double4(0.5 * (mx[0] - mn[0]), 0.5 * (mx[1] - mn[1]), 0.5 * (mx[2] - mn[2]), 0.0);
+    }
 }
 
 // ---------------------------------------------------------------------------------------- traversal
 // One warp per target group walks the tree from the root.  A cell is accepted for the
-// Taylor expansion when the MAC of eq. (15) holds for every point of the group's bounding sphere:
-//      theta * (|c_grp - y_c| - r_grp) > r_b          (reading A8: r_b = cell edge, y_c = cell centre)
+// Taylor expansion when the MAC of eq. (15) holds for every point of the group's bounding volume
+// (dist = lower bound of |x - y_c| over the group, from its bounding sphere and box):
+//      theta * dist > r_b                             (reading A8: r_b = cell edge, y_c = cell centre)
 // and, so that the near-singular region is always inside the direct list ("in practice,
 // the near-singular region is always contained in an area where the MAC criterion is not met"), when
 // additionally every panel centroid of the cell is farther than thres * Lmax from every target:
-//      |c_grp - y_c| - r_grp - (sqrt(3)/2) r_b > thres * Lmax.
+//      dist - (sqrt(3)/2) r_b > thres * Lmax.
 // Accepted cells go to the M2P list; leaves that fail go to the P2P list (as cell ids); other cells
 // are opened.  Pass 1 (fill == 0) counts, pass 2 writes.  The lane that owns child d of the popped
 // cell tests it; ballots keep the output order deterministic (Morton order).
@@ -213,7 +218,7 @@ k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__
     const int g = blockIdx.x * TRAV_WARPS + warp;
     if (g >= ng) return;
     int *stack = s_stack[warp];
-    const double4 G = ggeo[g];
+    const double4 G = ggeo[2 * g], H = ggeo[2 * g + 1];
     int nm = 0, npp = 0, sp = 0;
     const int mbase = fill ? m2p_off[g] : 0, pbase = fill ? p2p_off[g] : 0;
     // the root is tested like a child of a virtual parent
@@ -224,7 +229,10 @@ k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__
         if (c >= 0) {
             double4 cg = cgeo[c];
             double dx = G.x - cg.x, dy = G.y - cg.y, dz = G.z - cg.z;
-            double dist = sqrt(dx * dx + dy * dy + dz * dz) - G.w;
+            // lower bound of the distance from the cell centre to any target of the group: the better of
+            // the bounding sphere and the bounding box
+            double bx = fmax(fabs(dx) - H.x, 0.0), by = fmax(fabs(dy) - H.y, 0.0), bz = fmax(fabs(dz) - H.z, 0.0);
+            double dist = fmax(sqrt(dx * dx + dy * dy + dz * dz) - G.w, sqrt(bx * bx + by * by + bz * bz));
             acc = (theta * dist > cg.w) && (dist - 0.8660254037844387 * cg.w > near_dist);
             if (!acc) {
                 leaf = cchild[c].y == 0;

@@ -7,10 +7,13 @@ the MSMS / pdb2pqr molecules of PAPER.md:195, Tables 1-6, which are not availabl
 """
 from .spheres import icosphere, born_problem, kirkwood_problem, stern_sphere_problem, cavity_sphere_problem
 from .problem import Problem, Surface, concat_problem_arrays
+from .molecule import (saw_molecule, density_surface, marching_tetrahedra, validate_closed_mesh,
+                       protein_problem, multisurface_problem, binding_problems)
 
 SEED0 = 13094018
 
 __all__ = [
     "icosphere", "born_problem", "kirkwood_problem", "stern_sphere_problem", "cavity_sphere_problem",
-    "Problem", "Surface", "concat_problem_arrays", "SEED0",
+    "Problem", "Surface", "concat_problem_arrays", "saw_molecule", "density_surface", "marching_tetrahedra",
+    "validate_closed_mesh", "protein_problem", "multisurface_problem", "binding_problems", "SEED0",
 ]
