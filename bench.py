@@ -135,6 +135,20 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------------------------- our arm
+def max_over_ranks(v, dist, device):
+    """Timing of the slowest rank (the job is as slow as its slowest replica)."""
+    import torch
+    t = torch.tensor([float(v)], dtype=torch.float64, device=device)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, units_per_step, steps, seconds):
+    """Aggregate throughput of `world` independent replicas ("replicas only": no data-path collective)."""
+    return world * units_per_step * steps / seconds
+
+
 def run_ours(args):
     import torch
     import paper_1309_4018_b200 as pg
@@ -205,12 +219,9 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
         h.matvec(x, y)
     torch.cuda.synchronize()
     stop.set(); th.join()
-    tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms = float(tmax.item())
+    ms = max_over_ranks(ms, dist, "cuda")
     ms_per_step = ms / args.steps
-    value = world * st["direct_equiv"] * args.steps / (ms * 1e-3)
+    value = whole_job_value(world, st["direct_equiv"], args.steps, ms * 1e-3)
 
     # ---- e2e: host buffers through pygbe_matvec_host (pinned), copies inside the timed region
     xh = torch.empty(n, dtype=torch.float64).pin_memory(); xh.copy_(x.cpu())
@@ -219,16 +230,14 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
     for _ in range(3):
         h.matvec_host(xn, yn)
     barrier()
-    t = time.perf_counter()
+    e2e_s = 0.0
     for _ in range(args.steps):
         flush.zero_()
         torch.cuda.synchronize()
-        h.matvec_host(xn, yn)
-    e2e_s = time.perf_counter() - t
-    te = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e = world * st["direct_equiv"] * args.steps / float(te.item())
+        t = time.perf_counter()
+        h.matvec_host(xn, yn)            # synchronous: H2D copy, matvec, D2H copy, stream sync
+        e2e_s += time.perf_counter() - t
+    e2e = whole_job_value(world, st["direct_equiv"], args.steps, max_over_ranks(e2e_s, dist, "cuda"))
 
     line = None
     if rank == 0:
