@@ -191,8 +191,16 @@ def density_surface(centres, radii, spacing, probe=1.4, B=2.3, max_tries=4):
     """Closed outward-oriented triangulation of {rho = 1}.  If the grid happens to produce a non-manifold
     edge (isosurface through a grid vertex), the grid is shifted by a fraction of the spacing and redone."""
     R = np.asarray(radii) + probe
-    for attempt in range(max_tries):
-        rho, lo, n = _density_grid(np.asarray(centres) + 0.37 * spacing * attempt, R, spacing, B, pad=2 * spacing)
+    pad = 2 * spacing
+    for attempt in range(max_tries + 4):
+        rho, lo, n = _density_grid(np.asarray(centres) + 0.37 * spacing * attempt, R, spacing, B, pad=pad)
+        # where many atoms overlap the tails add up and the isosurface lies outside every R_i: the grid must
+        # contain it with a margin, otherwise the mesh would be cut open at the box
+        edge_max = max(rho[:2].max(), rho[-2:].max(), rho[:, :2].max(), rho[:, -2:].max(), rho[:, :, :2].max(),
+                       rho[:, :, -2:].max())
+        if edge_max >= 1.0:
+            pad += 0.5 * R.max()
+            continue
         v, t = marching_tetrahedra(rho - 1.0, lo, spacing)
         v = v - 0.37 * spacing * attempt
         v, t = _outer_component(v, t)
