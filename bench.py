@@ -270,11 +270,16 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
         nominal = {"f64": 148 * 64 * 2 * sm_max * 1e6 / 1e12, "f32": 148 * 128 * 2 * sm_max * 1e6 / 1e12}
         dt = "f32" if precision == pg.PRECISION_MIXED else "f64"
         achieved = flops / (stage_ms[dom] * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "k_%s<%s> (%d launches/matvec)" % (dom, "float" if dt == "f32" else "double", round(nreg_launch[dom])),
+        # dram__bytes_read.sum + dram__bytes_write.sum of the stage's launches from the ncu --set full capture of this
+        # command (profiles/r1b_mixed_path.md, config kirkwood_l5): bytes per matvec, both regions; else null
+        traffic = {("kirkwood_l5", "f32", "m2p"): 1.64e6 + 1.65e6, ("kirkwood_l5", "f32", "p2p"): 3.77e6}.get((args.config, dt, dom))
+        kname = {"m2p": "k_m2p<%d,*,%s> x %d regions (+ k_mom_combine)" % (kw["P"], "float" if dt == "f32" else "double", nreg),
+                 "p2p": "k_p2p<%s,%s>" % ("float" if dt == "f32" else "double", "twin regions fused" if nreg == 2 else "per region")}[dom]
+        roofline = {"bound": "alu", "kernel": "%s, %d launches/matvec" % (kname, round(nreg_launch[dom])),
                     "achieved": achieved, "peak": nominal[dt], "unit": "TFLOP/s", "frac": achieved / nominal[dt],
                     "peak_kind": "derived: 148 SM x %d lanes x 2 x %.0f MHz (DESIGN.md); FMA micro-benchmark in this run: %.1f TFLOP/s"
                                  % (64 if dt == "f64" else 128, sm_max, peaks["fp64_tflops" if dt == "f64" else "fp32_tflops"]),
-                    "traffic": None, "stage_ms": stage_ms, "alu_peaks_measured": peaks,
+                    "traffic": traffic, "stage_ms": stage_ms, "alu_peaks_measured": peaks,
                     "flops_per_launchset": flops,
                     "hbm_peak_gbs": mp.get("hbm_gbs")}
         # ---- time-to-solution (second half of the metric): create + rhs + GMRES + energy, host buffers
