@@ -288,7 +288,19 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
         xs, iters, rr, es, ec = h.solve_host(tol=tol)
         solve_ms = 1e3 * (time.perf_counter() - t)
         solve = {"create_ms": create_ms, "solve_ms": solve_ms, "time_to_solution_ms": create_ms + solve_ms,
-                 "gmres_iters": iters, "rel_resid": rr, "tol": tol, "E_solv_kJ_mol": es, "E_coul_kJ_mol": ec}
+                 "gmres_iters": iters, "rel_resid": rr, "tol": tol, "E_solv_kJ_mol": es, "E_coul_kJ_mol": ec,
+                 "preconditioner": "none (reading A16)"}
+        # the same with the optional block-diagonal right preconditioner (pygbe_options.precond = 1)
+        t = time.perf_counter()
+        h2 = pg.Handle.from_problem(prob, precision=precision, device=local, precond=1, **kw)
+        torch.cuda.synchronize()
+        c2 = 1e3 * (time.perf_counter() - t)
+        t = time.perf_counter()
+        _, it2, rr2, es2, ec2 = h2.solve_host(tol=tol, want_x=False)
+        s2 = 1e3 * (time.perf_counter() - t)
+        h2.close()
+        solve["block_diagonal"] = {"create_ms": c2, "solve_ms": s2, "time_to_solution_ms": c2 + s2, "gmres_iters": it2,
+                                   "rel_resid": rr2, "E_solv_kJ_mol": es2}
         # ---- oracle on the host cores, bounded sample
         cv, cores, sample = (None, None, None)
         if full:

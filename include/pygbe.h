@@ -85,7 +85,11 @@ typedef struct {
     int32_t device;     /* CUDA device ordinal [0]                                                     */
     void   *stream;     /* cudaStream_t [NULL]                                                         */
     int32_t check_mesh; /* 1: verify closedness / orientation on the host in create [0]                */
-    int32_t reserved[7];
+    int32_t precond;    /* GMRES right preconditioner: 0 none (the paper names none) [0];        */
+                        /* 1 block-diagonal: per panel the 2x2 block [[1/2, -V_ii^in], [1/2, c V_ii^out]] of   */
+                        /* its two rows and two unknowns (self integrals only).  Same stopping test, since a   */
+                        /* right preconditioner leaves the residual b - A x unchanged                          */
+    int32_t reserved[6];
 } pygbe_options;
 
 /* Counters and timings filled by pygbe_stats. */

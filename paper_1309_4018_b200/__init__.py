@@ -38,7 +38,7 @@ class pygbe_charges(C.Structure):
 class pygbe_options(C.Structure):
     _fields_ = [("K_fine", C.c_int32), ("thres", C.c_double), ("N_k", C.c_int32), ("ncrit", C.c_int32),
                 ("precision", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p),
-                ("check_mesh", C.c_int32), ("reserved", C.c_int32 * 7)]
+                ("check_mesh", C.c_int32), ("precond", C.c_int32), ("reserved", C.c_int32 * 6)]
 
 
 class pygbe_stats_t(C.Structure):
@@ -103,7 +103,7 @@ class Handle:
     """Owner of a pygbe_handle.  Methods mirror the C entry points one to one."""
 
     def __init__(self, surfaces, charges, eps, kappa, K=4, P=6, theta=0.5, K_fine=0, thres=0.0, N_k=0, ncrit=0,
-                 precision=PRECISION_FP64, device=0, stream=None, check_mesh=False):
+                 precision=PRECISION_FP64, device=0, stream=None, check_mesh=False, precond=0):
         """surfaces: list of (vertices [nv,3] f64, triangles [nt,3] i32, region_in, region_out);
         charges: (xyz [nq,3], q [nq], region [nq] or None) or None."""
         import torch
@@ -133,7 +133,7 @@ class Handle:
         if stream is None:
             stream = torch.cuda.current_stream(device).cuda_stream
         opt = pygbe_options(K_fine=K_fine, thres=thres, N_k=N_k, ncrit=ncrit, precision=precision, device=device,
-                            stream=C.c_void_p(stream), check_mesh=int(check_mesh))
+                            stream=C.c_void_p(stream), check_mesh=int(check_mesh), precond=int(precond))
         h = C.c_void_p()
         _check(L.pygbe_create(arr, len(surfaces), C.byref(ch) if ch is not None else None,
                               eps.ctypes.data_as(C.POINTER(C.c_double)), kappa.ctypes.data_as(C.POINTER(C.c_double)),

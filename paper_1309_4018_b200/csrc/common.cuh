@@ -179,6 +179,11 @@ struct pygbe_handle {
     cudaStream_t side = nullptr;    // far-field chain (P2M, M2M, M2P) runs here, concurrently with P2P
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     bool overlap = true;
+    // optional block-diagonal right preconditioner of GMRES (pygbe_options.precond)
+    int precond = 0;
+    double4 *pinv = nullptr;        // per global panel: inverse of [[1/2, -V_in], [1/2, c V_out]] as (a, b, c, d)
+    int2 *pidx = nullptr;           // per global panel: positions of (phi, dphi) = (row_in, row_out) in x / y
+    double *zbuf = nullptr;         // [2 npan] scratch
     double *scratch = nullptr;      // small device scratch (16 doubles)
     double *xh = nullptr, *yh = nullptr;   // device staging for the *_host entry points
     int *pinned_flags = nullptr;    // host pinned, 4 ints

@@ -5,6 +5,8 @@
 // immediately once flags[0] ("done") is set, so the host can queue iterations ahead and only polls.
 #pragma once
 #include "common.cuh"
+#include "tables.cuh"
+#include "nearfield.cuh"
 #include <cub/cub.cuh>
 
 #define GM_THREADS 256
@@ -153,4 +155,37 @@ k_gm_update(const int *__restrict__ flags, long n, const double *__restrict__ V,
     double acc = x[r];
     for (int i = 0; i < k; i++) acc += yk[i] * V[(long)i * n + r];
     x[r] = acc;
+}
+
+// ---------------------------------------------------------------------------------- block-diagonal M^-1
+// Per panel the 2x2 block that couples its two unknowns (phi, dphi/dn) with its two rows (equation of
+// region_in, equation of region_out) through the self integrals only:
+//     M_j = [[1/2, -V_in,jj], [1/2, c V_out,jj]],   c = eps_in/eps_out,   K_jj = 0.
+// pinv[j] = M_j^-1 = (a, b; c, d).  Built once in create.
+__global__ void k_precond_build(long npan, QuadTables q, const double *__restrict__ tri,
+                                const double4 *__restrict__ pk, double4 *__restrict__ pinv)
+{
+    long j = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    if (j >= npan) return;
+    const double inv4pi = 0.07957747154594767;
+    const double4 k = pk[j];                     // kappa_in, kappa_out, eps_in / eps_out
+    const double vin = self_integral(tri + 9 * j, k.x, q) * inv4pi;
+    const double vout = self_integral(tri + 9 * j, k.y, q) * inv4pi * k.z;
+    const double det = 0.5 * vout + 0.5 * vin;
+    pinv[j] = make_double4(vout / det, vin / det, -0.5 / det, 0.5 / det);
+}
+
+// z (= or +=) M^-1 u, panel by panel.
+__global__ void __launch_bounds__(GM_THREADS)
+k_precond_apply(const int *__restrict__ flags, int respect_done, long npan, const double4 *__restrict__ pinv,
+                const int2 *__restrict__ pidx, const double *__restrict__ u, int add, double *__restrict__ z)
+{
+    if (respect_done && flags[0]) return;
+    long j = (long)blockIdx.x * GM_THREADS + threadIdx.x;
+    if (j >= npan) return;
+    const int2 ix = pidx[j];
+    const double4 m = pinv[j];
+    const double u0 = u[ix.x], u1 = u[ix.y];
+    const double z0 = m.x * u0 + m.y * u1, z1 = m.z * u0 + m.w * u1;
+    if (add) { z[ix.x] += z0; z[ix.y] += z1; } else { z[ix.x] = z0; z[ix.y] = z1; }
 }

@@ -69,6 +69,7 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
     CUDA_TRY(cudaMemsetAsync(G.flags, 0, 4 * sizeof(int), st));
     CUDA_TRY(cudaMemsetAsync(G.scal, 0, 8 * sizeof(double), st));
     const int poll = n < 200000 ? 4 : 1;
+    const bool pc = h->precond == 1 && h->pinv != nullptr;
     int total = 0, done = 0;
     bool first = true;
     while (total < max_iter && !done) {
@@ -81,7 +82,12 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
         int j = 0;
         for (; j < mc; j++) {
             double *vj = G.V + (size_t)j * n, *vn = G.V + (size_t)(j + 1) * n;
-            TRY(matvec_impl(h, vj, G.w, G.flags));
+            if (pc) {           // right preconditioning: w = A (M^-1 v_j)
+                LAUNCH(h, k_precond_apply, cdiv(h->npan, GM_THREADS), GM_THREADS, 0, G.flags, 1, h->npan, h->pinv, h->pidx, vj, 0, h->zbuf);
+                TRY(matvec_impl(h, h->zbuf, G.w, G.flags));
+            } else {
+                TRY(matvec_impl(h, vj, G.w, G.flags));
+            }
             LAUNCH(h, k_gm_zero, cdiv(j + 2, 128), 128, 0, G.flags, G.h1, j + 1, G.h2, j + 1, G.scal + 3, 1);
             LAUNCH(h, k_gm_dots, gridd, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.w, G.h1);
             LAUNCH(h, k_gm_axpys, gridn, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.h1, G.w);
@@ -97,7 +103,13 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
             }
         }
         LAUNCH(h, k_gm_solve_small, 1, 1, 0, G.flags, G.m, G.H, G.g, G.yk);
-        LAUNCH(h, k_gm_update, gridn, GM_THREADS, 0, G.flags, n, G.V, G.yk, x_dev);
+        if (pc) {               // x += M^-1 (V y)
+            CUDA_TRY(cudaMemsetAsync(h->zbuf, 0, n * sizeof(double), st));
+            LAUNCH(h, k_gm_update, gridn, GM_THREADS, 0, G.flags, n, G.V, G.yk, h->zbuf);
+            LAUNCH(h, k_precond_apply, cdiv(h->npan, GM_THREADS), GM_THREADS, 0, G.flags, 0, h->npan, h->pinv, h->pidx, h->zbuf, 1, x_dev);
+        } else {
+            LAUNCH(h, k_gm_update, gridn, GM_THREADS, 0, G.flags, n, G.V, G.yk, x_dev);
+        }
         CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(cudaMemcpyAsync(h->pinned_scal, G.scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(cudaStreamSynchronize(st));
