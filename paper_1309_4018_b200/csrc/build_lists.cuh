@@ -96,8 +96,11 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     TRY(h->mem.alloc(&d_mcnt, R.ng)); TRY(h->mem.alloc(&d_pcnt, R.ng)); TRY(h->mem.alloc(&d_over, 1));
     CUDA_TRY(cudaMemsetAsync(d_over, 0, sizeof(int), h->stream));
     const double near_dist = h->thres > 0 ? h->thres * R.Lmax : 0.0;
+    // break-even between one Taylor evaluation and the direct sum over a leaf's points, from the SASS
+    // instruction counts (profiles/r1b_mixed_path.md): ~50 points in fp32, ~18 in fp64 at P = 6 (Nc = 84)
+    const int small_leaf = (int)((mixed ? 50.0 : 18.0) * h->Nc / 84.0 / K);
     LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.ggeo, R.cgeo, R.crange, R.cchild,
-           h->theta, near_dist, 0, d_mcnt, d_pcnt, nullptr, nullptr, nullptr, nullptr, d_over);
+           h->theta, near_dist, small_leaf, 0, d_mcnt, d_pcnt, nullptr, nullptr, nullptr, nullptr, d_over);
     std::vector<int> mcnt, pcnt;
     TRY(download(h, mcnt, d_mcnt, (size_t)R.ng));
     TRY(download(h, pcnt, d_pcnt, (size_t)R.ng));
@@ -107,7 +110,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     TRY(upload(h, &R.m2p_off, moff)); TRY(upload(h, &d_poff_raw, poff));
     TRY(h->mem.alloc(&R.m2p_cell, moff[R.ng])); TRY(h->mem.alloc(&d_pleaf_raw, poff[R.ng]));
     LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.ggeo, R.cgeo, R.crange, R.cchild,
-           h->theta, near_dist, 1, d_mcnt, d_pcnt, R.m2p_off, d_poff_raw, R.m2p_cell, d_pleaf_raw, d_over);
+           h->theta, near_dist, small_leaf, 1, d_mcnt, d_pcnt, R.m2p_off, d_poff_raw, R.m2p_cell, d_pleaf_raw, d_over);
     std::vector<int> pleaf;
     TRY(download(h, pleaf, d_pleaf_raw, (size_t)poff[R.ng]));
     {   // multipoles are needed for the listed cells and, to build those by M2M, for all their descendants

@@ -209,7 +209,7 @@ k_group_geometry(const double4 *__restrict__ tpos, int np, double4 *__restrict__
 __global__ void __launch_bounds__(TRAV_WARPS * 32)
 k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__ cgeo,
            const int2 *__restrict__ crange, const int2 *__restrict__ cchild, double theta,
-           double near_dist, int fill, int *__restrict__ m2p_cnt, int *__restrict__ p2p_cnt,
+           double near_dist, int small_leaf, int fill, int *__restrict__ m2p_cnt, int *__restrict__ p2p_cnt,
            const int *__restrict__ m2p_off, const int *__restrict__ p2p_off, int *__restrict__ m2p_cell,
            int *__restrict__ p2p_leaf, int *overflow)
 {
@@ -234,7 +234,12 @@ k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__
             double bx = fmax(fabs(dx) - H.x, 0.0), by = fmax(fabs(dy) - H.y, 0.0), bz = fmax(fabs(dz) - H.z, 0.0);
             double dist = fmax(sqrt(dx * dx + dy * dy + dz * dz) - G.w, sqrt(bx * bx + by * by + bz * bz));
             acc = (theta * dist > cg.w) && (dist - 0.8660254037844387 * cg.w > near_dist);
-            if (!acc) {
+            if (acc && cchild[c].y == 0) {
+                // an accepted leaf with so few panels that summing its points directly (exact) costs fewer
+                // instructions than one Taylor evaluation goes to the direct list instead
+                int2 r = crange[c];
+                if (r.y - r.x <= small_leaf) { acc = false; leaf = true; }
+            } else if (!acc) {
                 leaf = cchild[c].y == 0;
                 open = !leaf;
             }

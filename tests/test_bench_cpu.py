@@ -30,6 +30,15 @@ def test_whole_job_value_and_flop_model():
     assert bench.P2P_FLOPS_FUSED < bench.P2P_FLOPS[False] + bench.P2P_FLOPS[True]
 
 
+def test_richardson_formulas():
+    """eq. (16)-(17), on a manufactured sequence f(h) = f* + C h^p."""
+    from paper_1309_4018_b200.richardson import observed_order, extrapolate
+    fstar, C, p, r = -41.2465, 0.8, 1.013, 4.0
+    f = [fstar + C * h ** p for h in (1.0 / 16, 1.0 / 4, 1.0)]          # fine, medium, coarse
+    assert abs(observed_order(f[0], f[1], f[2], r) - p) < 1e-12
+    assert abs(extrapolate(f[0], f[1], r, p) - fstar) < 1e-12
+
+
 def test_max_over_ranks_gloo_world2(tmp_path):
     """Two processes, gloo: every rank must get the slowest rank's time; the aggregate counts both replicas."""
     script = tmp_path / "w.py"

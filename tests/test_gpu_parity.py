@@ -370,6 +370,19 @@ def test_multisurface_molecule(env):
     h.close()
 
 
+def test_paper_sphere_convergence_study(env):
+    """The paper's own sphere experiment (section 3.1, Table 3: kappa = 0, K = 3, P = 12, tol 1e-6) through the
+    CUDA path: PAPER.md:229 prints the analytic value -41.2465 and PyGBe's Richardson value -41.2467 kJ/mol,
+    PAPER.md:231 the observed order 1.013 with respect to panel area."""
+    pg, torch, orc = env
+    from paper_1309_4018_b200.richardson import sphere_refinement_study
+    r = sphere_refinement_study(levels=(3, 4, 5))
+    assert abs(r["extrapolated"] - (-41.2465)) < 2e-3
+    assert abs(r["order_wrt_area"] - 1.013) < 0.03
+    e = r["E_solv_kJ_mol"]
+    assert e[0] < e[1] < e[2] < -41.2465                  # converging from below, like Fig. 5a
+
+
 def test_block_diagonal_preconditioner(env):
     """pygbe_options.precond = 1: same solution (right preconditioning leaves b - A x unchanged), fewer
     iterations on a sliver-rich multi-surface mesh; the true residual is checked through the oracle."""
