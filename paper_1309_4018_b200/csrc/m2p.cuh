@@ -100,9 +100,14 @@ __device__ __forceinline__ T m2p_eval(T dx, T dy, T dz, T kappa, T kscaled, cons
 // The batches are double-buffered with cp.async (LDGSTS): while the threads evaluate the recurrences of one
 // batch, the moments and centres of the next one stream from L2 into the other buffer (capture r1b showed
 // 7-9 % barrier + 5-9 % long-scoreboard stalls with synchronous staging at 2 warps per CTA).
+#ifndef M2P_CB
 #define M2P_CB 4
+#endif
+#ifndef M2P_MINB
+#define M2P_MINB 1       // min CTAs per SM asked of ptxas (register cap); tuning knob
+#endif
 template <int P, bool YUKAWA, typename T>
-__global__ void __launch_bounds__(PYGBE_TG_M2P)
+__global__ void __launch_bounds__(PYGBE_TG_M2P, M2P_MINB)
 k_m2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
       const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const T *__restrict__ momc,
       double kappa, double kscaled, double *__restrict__ out)

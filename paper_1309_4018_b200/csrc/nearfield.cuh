@@ -55,16 +55,6 @@ __global__ void k_prep(const int *__restrict__ skip, int np, int K, const double
     }
 }
 
-// Row of region Omega collocated on the panel (eq. 10):  y = 1/2 phi - out.
-__global__ void k_combine(const int *__restrict__ skip, int np, const int *__restrict__ row_idx, const double *__restrict__ pphi,
-                          const double *__restrict__ out, double *__restrict__ y)
-{
-    if (skip && *skip) return;
-    int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= np) return;
-    y[row_idx[p]] = 0.5 * pphi[p] - out[p];
-}
-
 // ------------------------------------------------------------------- singular / near-singular panels
 // Step 1: for each target, find the source panels of its group's P2P ranges that are the target's own
 // panel or lie inside the near-singular region |x_i - c_j|^2 < thres^2 * 2 A_j  (
@@ -179,23 +169,6 @@ __global__ void k_near_values(int np, QuadTables q, bool yukawa, double kappa, c
         }
         val[e] = make_double2(cV[j] * (fv - cv), cK[j] * (fk - ck));
     }
-}
-
-// Per-matvec application: out_i += sum_e [ val.x dphi_j - val.y phi_j ]  (CSR SpMV, fp64 always).
-__global__ void k_near_apply(const int *__restrict__ skip, int np, const int *__restrict__ off, const int *__restrict__ col,
-                             const double2 *__restrict__ val, const double *__restrict__ pphi,
-                             const double *__restrict__ pdphi, double *__restrict__ out)
-{
-    if (skip && *skip) return;
-    int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= np) return;
-    double acc = 0.0;
-    for (int e = off[t]; e < off[t + 1]; e++) {
-        int j = col[e];
-        double2 v = val[e];
-        acc += v.x * pdphi[j] - v.y * pphi[j];
-    }
-    out[t] += acc;
 }
 
 // Correction SpMV (a8) fused with the block combination (a9) for a region and, optionally, its twin (same

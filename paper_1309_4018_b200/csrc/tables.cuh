@@ -1,5 +1,5 @@
 // tables.cuh -- quadrature rules (host side, handed to kernels by value) and the multi-index tables of
-// the Cartesian Taylor expansion (constant memory, valid for every P <= PYGBE_PMAX).
+// the Cartesian Taylor expansion (one device-memory copy per handle, valid for every P <= PYGBE_PMAX).
 #pragma once
 #include "common.cuh"
 

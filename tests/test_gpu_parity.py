@@ -232,6 +232,22 @@ def test_treecode_leaf_sizes(env, ncrit):
     h.close()
 
 
+@pytest.mark.parametrize("kw", [dict(K=4, thres=3.0, ncrit=8, theta=0.6), dict(K=7, thres=1.25, ncrit=16, theta=0.5),
+                                dict(K=1, thres=2.0, ncrit=12, theta=0.66), dict(K=3, K_fine=7, ncrit=500, theta=0.3)])
+def test_treecode_near_field_inside_direct_lists(env, kw):
+    """Tiny leaves + a wide near-singular region + loose theta: the traversal's guard must keep every
+    near-singular pair in the direct lists, otherwise the K_fine rule would be lost."""
+    pg, torch, orc = env
+    prob = W.cavity_sphere_problem(2)
+    okw = {k: v for k, v in kw.items() if k in ("K", "K_fine", "thres")}
+    o = orc.Oracle(prob, **okw)
+    x = np.random.default_rng(17).normal(size=o.n)
+    for prec in (pg.PRECISION_FP64, pg.PRECISION_MIXED):
+        h, y = gpu_matvec(pg, torch, prob, x, P=8, precision=prec, **kw)
+        assert rel(y, o.matvec(x)) <= TOL_TREE
+        h.close()
+
+
 def test_kirkwood_full_size_sampled_rows(env):
     """BASELINE.json config 1 at full size (20480 panels, the configuration bench.py times): oracle rows
     computed one by one on a seeded sample; plus the Gauss identity as a size-independent property."""
