@@ -272,7 +272,7 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
         achieved = flops / (stage_ms[dom] * 1e-3) / 1e12
         # dram__bytes_read.sum + dram__bytes_write.sum of the stage's launches from the ncu --set full capture of this
         # command (profiles/r1b_mixed_path.md, config kirkwood_l5): bytes per matvec, both regions; else null
-        traffic = {("kirkwood_l5", "f32", "m2p"): 1.64e6 + 1.65e6, ("kirkwood_l5", "f32", "p2p"): 3.77e6}.get((args.config, dt, dom))
+        traffic = {("kirkwood_l5", "f32", "m2p"): 1.50e6 + 1.51e6, ("kirkwood_l5", "f32", "p2p"): 3.86e6}.get((args.config, dt, dom))
         kname = {"m2p": "k_m2p<%d,*,%s> x %d regions (+ k_mom_combine)" % (kw["P"], "float" if dt == "f32" else "double", nreg),
                  "p2p": "k_p2p<%s,%s>" % ("float" if dt == "f32" else "double", "twin regions fused" if nreg == 2 else "per region")}[dom]
         roofline = {"bound": "alu", "kernel": "%s, %d launches/matvec" % (kname, round(nreg_launch[dom])),
