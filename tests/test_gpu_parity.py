@@ -386,6 +386,26 @@ def test_multisurface_molecule(env):
     h.close()
 
 
+def test_multisurface_full_size_sampled_rows(env):
+    """BASELINE.json config 3 at its full size (3000 atoms, two cavities, Stern surface, ~157 k panels, four
+    regions): oracle rows one by one on a seeded sample, both precisions; Gauss identity as a property."""
+    pg, torch, orc = env
+    prob = W.multisurface_problem(3000, spacing=1.12)
+    assert 140_000 < prob.n_panels < 175_000 and len(prob.surfaces) == 4
+    o = orc.Oracle(prob)
+    rng = np.random.default_rng(33)
+    x = rng.normal(size=o.n)
+    rows = np.sort(rng.choice(o.n, 120, replace=False))
+    yo = o.matvec(x, rows)
+    for prec in (pg.PRECISION_FP64, pg.PRECISION_MIXED):
+        h = pg.Handle.from_problem(prob, K=4, P=6, theta=0.5, precision=prec, check_mesh=True)
+        y = h.matvec(torch.tensor(x, device="cuda")).cpu().numpy()
+        assert rel(y[rows], yo) <= TOL_TREE
+        st = h.stats()
+        assert st["p2p_pairs"] < 0.05 * st["direct_equiv"]
+        h.close()
+
+
 def test_paper_sphere_convergence_study(env):
     """The paper's own sphere experiment (section 3.1, Table 3: kappa = 0, K = 3, P = 12, tol 1e-6) through the
     CUDA path: PAPER.md:229 prints the analytic value -41.2465 and PyGBe's Richardson value -41.2467 kJ/mol,
