@@ -293,6 +293,10 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
                     "traffic": traffic, "stage_ms": stage_ms, "alu_peaks_measured": peaks,
                     "flops_per_launchset": flops, "flop_model": "exact for twin regions" if nreg == 2 else "regions weighted equally (approximate)",
                     "hbm_peak_gbs": mp.get("hbm_gbs")}
+        if dt == "f32" and peaks.get("fp32_mix_tflops"):
+            # context, not the denominator: what the FP32 pipe delivers on a register-resident FMUL + 3-register
+            # FFMA mix (pygbe_alu_peaks out[3]), the practical ceiling of the recurrences' mix
+            roofline["frac_of_mix_ceiling"] = achieved / peaks["fp32_mix_tflops"]
         # ---- time-to-solution (second half of the metric): create + rhs + GMRES + energy, host buffers
         t = time.perf_counter()
         tol = 1e-6 if dt == "f64" else 1e-5

@@ -187,8 +187,10 @@ int pygbe_stage_times(pygbe_handle *h, double *ms, int64_t *launches);
 const char *pygbe_last_error(void);
 
 /* ALU roofline denominators measured on `device` with dependent-FMA / MUFU micro-kernels (synchronous,
- * ~50 ms): out3[0] = fp32 FMA TFLOP/s, out3[1] = fp64 FMA TFLOP/s, out3[2] = MUFU.RSQ Gop/s.  HOST. */
-int pygbe_alu_peaks(int32_t device, double *out3);
+ * ~80 ms): out4[0] = fp32 FMA TFLOP/s, out4[1] = fp64 FMA TFLOP/s, out4[2] = MUFU.RSQ Gop/s, out4[3] = TFLOP/s
+ * of an fp32 FMUL + three-register FFMA mix over 24 live registers (the practical ceiling of the
+ * recurrence-like instruction mix of M2P / P2P; FMA = 2 flops, MUL = 1).  out4: HOST, 4 doubles. */
+int pygbe_alu_peaks(int32_t device, double *out4);
 
 /* Library / build identification, e.g. "pygbe-b200 0.1 sm_100a". */
 const char *pygbe_version(void);

@@ -232,12 +232,12 @@ class Handle:
 
 
 def alu_peaks(device=0):
-    """Measured ALU peaks of the device: dict(fp32_tflops, fp64_tflops, mufu_gops)."""
+    """Measured ALU peaks of the device: dict(fp32_tflops, fp64_tflops, mufu_gops, fp32_mix_tflops)."""
     L = lib()
     L.pygbe_alu_peaks.argtypes = [C.c_int32, C.POINTER(C.c_double)]
-    out = (C.c_double * 3)()
+    out = (C.c_double * 4)()
     _check(L.pygbe_alu_peaks(device, out))
-    return dict(fp32_tflops=out[0], fp64_tflops=out[1], mufu_gops=out[2])
+    return dict(fp32_tflops=out[0], fp64_tflops=out[1], mufu_gops=out[2], fp32_mix_tflops=out[3])
 
 
 def pygbe_version():

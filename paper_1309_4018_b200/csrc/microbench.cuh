@@ -33,7 +33,27 @@ __global__ void __launch_bounds__(256) k_mufu_peak(int iters, float *out)
     if (s == -12345.f) out[0] = s;
 }
 
-// out[0] = fp32 FMA TFLOP/s, out[1] = fp64 FMA TFLOP/s, out[2] = MUFU.RSQ Gop/s (best of 5 launches each)
+// A register-resident mix that looks like the Taylor recurrences: per element one FMUL and one three-register
+// FFMA over 24 live values with scattered operand indices (3 flops per 2 instructions).  It measures what the
+// FP32 pipe delivers once operands come from three different registers (bank conflicts in the operand
+// collector), i.e. the practical ceiling of the M2P / P2P instruction mix, below the pure-FMA peak.
+__global__ void __launch_bounds__(128) k_mix_peak(int iters, float *out)
+{
+    float v[24];
+#pragma unroll
+    for (int i = 0; i < 24; i++) v[i] = 1.0f + 1e-3f * (threadIdx.x + i);
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int i = 0; i < 24; i++) v[i] = v[(i + 7) % 24] * v[(i + 13) % 24] + v[i] * 0.5f;
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 24; i++) s += v[i];
+    if (s == -12345.f) out[0] = s;
+}
+
+// out[0] = fp32 FMA TFLOP/s, out[1] = fp64 FMA TFLOP/s, out[2] = MUFU.RSQ Gop/s, out[3] = fp32 FMUL + 3-register
+// FFMA mix TFLOP/s (FMA = 2 flops, MUL = 1); best of 5 launches each
 static int run_alu_peaks(int device, double *out)
 {
     CUDA_TRY(cudaSetDevice(device));
@@ -60,6 +80,20 @@ static int run_alu_peaks(int device, double *out)
             if (rep > 0) best = std::max(best, ops / (ms * 1e-3));
         }
         out[which] = which == 2 ? best * 1e-9 : best * 1e-12;
+    }
+    {
+        const int g2 = prop.multiProcessorCount * 16, iters = 4096;
+        double best = 0.0;
+        for (int rep = 0; rep < 6; rep++) {
+            CUDA_TRY(cudaEventRecord(e0));
+            k_mix_peak<<<g2, 128>>>(iters, (float *)buf);
+            CUDA_TRY(cudaEventRecord(e1));
+            CUDA_TRY(cudaEventSynchronize(e1));
+            float ms = 0;
+            CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+            if (rep > 0) best = std::max(best, (double)g2 * 128 * iters * 24.0 * 3.0 / (ms * 1e-3));
+        }
+        out[3] = best * 1e-12;
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     cudaFree(buf);

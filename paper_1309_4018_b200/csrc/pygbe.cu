@@ -115,8 +115,8 @@ extern "C" int pygbe_stats(const pygbe_handle *h, pygbe_stats_t *s)
     return PYGBE_OK;
 }
 
-extern "C" int pygbe_alu_peaks(int32_t device, double *out3)
+extern "C" int pygbe_alu_peaks(int32_t device, double *out4)
 {
-    if (!out3) { pygbe_set_error("alu_peaks: null pointer"); return PYGBE_EINVAL; }
-    return run_alu_peaks(device, out3);
+    if (!out4) { pygbe_set_error("alu_peaks: null pointer"); return PYGBE_EINVAL; }
+    return run_alu_peaks(device, out4);
 }
