@@ -120,17 +120,23 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
         for (int c : mcell) need[c] = 1;
         for (int c = 1; c < ncells; c++)                  // parents precede children in the numbering
             if (need[cparent_h[c]]) need[c] = 1;
-        std::vector<int> p2m_cells, m2m_cells;
+        std::vector<int> p2m_cells;
+        std::vector<int4> m2m_rec;
         for (int c : leaves) if (need[c]) p2m_cells.push_back(c);
-        R.m2m_off.assign(R.depth + 1, 0);
-        for (int l = 0; l < R.depth; l++) {
-            R.m2m_off[l] = (int)m2m_cells.size();
+        for (int l = R.depth - 1; l >= 0; l--)              // deepest level first: children before parents
             for (int c = R.level_begin[l]; c < R.level_begin[l + 1]; c++)
-                if (need[c] && cchild_h[c].y > 0) m2m_cells.push_back(c);
-        }
-        R.m2m_off[R.depth] = (int)m2m_cells.size();
+                if (need[c] && cchild_h[c].y > 0) {
+                    int mask = 0;
+                    for (int k = 0; k < cchild_h[c].y; k++)
+                        if (cchild_h[cchild_h[c].x + k].y > 0) mask |= 1 << k;
+                    m2m_rec.push_back(make_int4(c, cchild_h[c].x, cchild_h[c].y, mask));
+                }
+        R.n_m2m = (int)m2m_rec.size();
         R.n_p2m = (int)p2m_cells.size();
-        TRY(upload(h, &R.p2m_cells, p2m_cells)); TRY(upload(h, &R.m2m_cells, m2m_cells));
+        TRY(upload(h, &R.p2m_cells, p2m_cells)); TRY(upload(h, &R.m2m_rec, m2m_rec));
+        TRY(h->mem.alloc(&R.up_sync, 2)); TRY(h->mem.alloc(&R.cready, (size_t)ncells));
+        CUDA_TRY(cudaMemsetAsync(R.up_sync, 0, 2 * sizeof(int), h->stream));
+        CUDA_TRY(cudaMemsetAsync(R.cready, 0, (size_t)ncells * sizeof(int), h->stream));
     }
     int over = 0;
     CUDA_TRY(cudaMemcpy(&over, d_over, sizeof(int), cudaMemcpyDeviceToHost));

@@ -1,6 +1,7 @@
 // build_primary.cuh -- build of a region that owns its tree (see build_region.cuh for the twin case).
 #pragma once
 #include "build_region.cuh"
+#include "farfield.cuh"
 
 static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<double> &tri_host, const QuadTables &qt)
 {
@@ -65,7 +66,13 @@ static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<do
     TRY(build_corrections(h, R, qt, nullptr));
     if (R.n_m2p_items > 0) {
         TRY(h->mem.alloc(&R.mom, (size_t)R.ncells * 2 * h->Nc));
-        TRY(h->mem.alloc((char **)&R.momc, (size_t)R.ncells * ((h->Nc + 3) / 4 * 4) * sizeof(double)));
+        TRY(h->mem.alloc(&R.pmom, (size_t)R.np * 2 * h->Nc));
+        if (R.n_p2m > 0)
+            LAUNCH(h, k_panel_moments, R.n_p2m, PMOM_THREADS, 0, h->P, h->Nc, h->K, h->itab, R.p2m_cells, R.cgeo, R.crange,
+                   R.spos, R.pnrm, R.pmom);
+        const size_t mc_bytes = (size_t)R.ncells * ((h->Nc + 3) / 4 * 4) * sizeof(double);
+        TRY(h->mem.alloc((char **)&R.momc, mc_bytes));
+        CUDA_TRY(cudaMemsetAsync(R.momc, 0, mc_bytes, h->stream));       // row padding stays zero
     }
     CUDA_TRY(cudaGetLastError());
     return PYGBE_OK;

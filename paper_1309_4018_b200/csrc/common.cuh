@@ -118,8 +118,10 @@ struct Region {
     int *leaf_cell = nullptr;       // leaves in Morton order
     // cells whose multipoles are needed: those in some M2P list and all their descendants
     int *p2m_cells = nullptr; int n_p2m = 0;        // needed leaves (P2M)
-    int *m2m_cells = nullptr;                       // needed internal cells, grouped by level
-    std::vector<int> m2m_off;                       // host: level l -> [m2m_off[l], m2m_off[l+1])
+    int4 *m2m_rec = nullptr; int n_m2m = 0;         // needed internal cells, deepest level first: (cell, first child, n children, internal-child mask)
+    double *pmom = nullptr;                         // [np][2][Nc] geometry-only panel moments about the panel's leaf centre (P2M)
+    int *up_sync = nullptr;                         // [2] ticket and exit counters of the upward pass
+    int *cready = nullptr;                          // [ncells] matvec number at which the cell's multipoles were built
     double Lmax = 0;                // max panel length sqrt(2A) on this region's boundary
     double root_c[3] = {0, 0, 0}, root_edge = 1;
     // target groups and interaction lists -----------------------------------------------------------
@@ -158,7 +160,7 @@ struct GmresWork {
 };
 
 struct pygbe_handle {
-    int device = 0;
+    int device = 0, n_sm = 148;
     cudaStream_t stream = nullptr;
     int K = 4, P = 6, Nc = 84, Kfine = 19, Nk = 5, ncrit = 0, precision = 0;
     double theta = 0.5, thres = 2.0;

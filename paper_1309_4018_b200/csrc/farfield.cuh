@@ -13,140 +13,257 @@
 #include "common.cuh"
 #include "tables.cuh"
 
-// ------------------------------------------------------------------------------------------------ P2M
-// One CTA per leaf; thread k owns coefficient k of both sets; the leaf's points go through shared memory
-// as tables of powers d^0..d^P per axis (HBM traffic: each point read once, 64 B).
-#define P2M_THREADS 128
-#define P2M_TILE 64
-#define P2M_SLOTS ((PYGBE_NCMAX + P2M_THREADS - 1) / P2M_THREADS)
-__global__ void __launch_bounds__(P2M_THREADS)
-k_p2m(const int *__restrict__ skip, int P, int Nc, int K, const IndexTables *__restrict__ tab,
-      const int *__restrict__ leaf_cell, const double4 *__restrict__ cgeo, const int2 *__restrict__ crange,
-      const double4 *__restrict__ spos, const double4 *__restrict__ schg, double *__restrict__ mom)
+// Where a finished cell's multipoles go besides mom: the combinations ca MV + cb MK that the M2P of the tree
+// owner (A) and of its twin region (B, or null) read, in the arithmetic type of the M2P, row stride padded to
+// a multiple of 4 (m2p.cuh).  Written by the kernel that finishes the cell (P2M for leaves, M2M otherwise).
+struct MomOut {
+    void *A, *B;
+    double caA, cbA, caB, cbB;
+    int fp32, stride;
+};
+__device__ __forceinline__ void momc_store(const MomOut &o, long cell, int k, double mv, double mk)
 {
-    __shared__ double s_pw[P2M_TILE][3][PYGBE_PMAX + 1];
-    __shared__ double4 s_chg[P2M_TILE];
-    if (skip && *skip) return;
+    const long i = cell * o.stride + k;
+    if (o.fp32) {
+        ((float *)o.A)[i] = (float)(o.caA * mv + o.cbA * mk);
+        if (o.B) ((float *)o.B)[i] = (float)(o.caB * mv + o.cbB * mk);
+    } else {
+        ((double *)o.A)[i] = o.caA * mv + o.cbA * mk;
+        if (o.B) ((double *)o.B)[i] = o.caB * mv + o.cbB * mk;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ P2M
+// The densities are constant per panel, so a leaf's multipoles are linear in the panel values
+// with geometry-only coefficients, computed once at create (k_panel_moments) about the centre of the panel's
+// leaf, K-point rule:
+//     GV_j^k = sum_g w_g d_g^k,     GK_j^k = sum_g w_g sum_i n_j,i k_i d_g^(k - e_i),     d_g = y_jg - y_c
+//     MV^k(leaf) = sum_{j in leaf} (cV_j dphi_j) GV_j^k,      MK^k(leaf) = sum_{j in leaf} (cK_j phi_j) GK_j^k
+// (cV, cK: the per-region constants folded into the densities, nearfield.cuh k_prep).  Each matvec the P2M is
+// then a streaming product: 2 Nc doubles read per panel, coalesced, two FMAs per 16 bytes -- HBM / L2 bound
+// as SURVEY 8(d) puts it (27.5 MB at 20 480 panels and P = 6) instead of the ALU- and latency-bound
+// monomial loop over the Gauss points of the first versions (29 us -> see profiles/r2a_upward.md).
+// pmom[panel][set][Nc], panels in the region's Morton order.
+#define PMOM_THREADS 128
+__global__ void __launch_bounds__(PMOM_THREADS)
+k_panel_moments(int P, int Nc, int K, const IndexTables *__restrict__ tab, const int *__restrict__ leaf_cell,
+                const double4 *__restrict__ cgeo, const int2 *__restrict__ crange,
+                const double4 *__restrict__ spos, const double4 *__restrict__ pnrm, double *__restrict__ pmom)
+{
     const int cell = leaf_cell[blockIdx.x];
     const double4 cg = cgeo[cell];
     const int2 rg = crange[cell];
-    const long p0 = (long)rg.x * K, p1 = (long)rg.y * K;
-    double accV[P2M_SLOTS], accK[P2M_SLOTS];
-    int kk[P2M_SLOTS][3];
-#pragma unroll
-    for (int s = 0; s < P2M_SLOTS; s++) {
-        accV[s] = accK[s] = 0.0;
-        int k = threadIdx.x + s * P2M_THREADS;
-        if (k < Nc) { kk[s][0] = tab->kxyz[k][0]; kk[s][1] = tab->kxyz[k][1]; kk[s][2] = tab->kxyz[k][2]; }
-        else { kk[s][0] = kk[s][1] = kk[s][2] = 0; }
-    }
-    for (long base = p0; base < p1; base += P2M_TILE) {
-        int n = (int)min((long)P2M_TILE, p1 - base);
-        __syncthreads();
-        for (int i = threadIdx.x; i < n * 3; i += P2M_THREADS) {
-            int pt = i / 3, a = i - 3 * pt;
-            double4 s = spos[base + pt];
-            double d = (a == 0 ? s.x - cg.x : (a == 1 ? s.y - cg.y : s.z - cg.z));
-            double pw = 1.0;
-            for (int e = 0; e <= P; e++) { s_pw[pt][a][e] = pw; pw *= d; }
+    const long nitem = (long)(rg.y - rg.x) * Nc;
+    for (long it = threadIdx.x; it < nitem; it += PMOM_THREADS) {
+        const int j = rg.x + (int)(it / Nc), k = (int)(it % Nc);
+        const int kx = tab->kxyz[k][0], ky = tab->kxyz[k][1], kz = tab->kxyz[k][2];
+        const double4 n = pnrm[j];
+        double gv = 0.0, gk = 0.0;
+        for (int g = 0; g < K; g++) {
+            const double4 s = spos[(long)j * K + g];
+            const double dx = s.x - cg.x, dy = s.y - cg.y, dz = s.z - cg.z;
+            // X1 = dx^(kx-1) (or 0), X = dx^kx, likewise for y and z
+            double X1 = 0.0, X = 1.0, Y1 = 0.0, Y = 1.0, Z1 = 0.0, Z = 1.0;
+            for (int e = 0; e < kx; e++) { X1 = X; X *= dx; }
+            for (int e = 0; e < ky; e++) { Y1 = Y; Y *= dy; }
+            for (int e = 0; e < kz; e++) { Z1 = Z; Z *= dz; }
+            gv += s.w * X * Y * Z;
+            gk += s.w * (n.x * kx * X1 * Y * Z + n.y * ky * X * Y1 * Z + n.z * kz * X * Y * Z1);
         }
-        for (int i = threadIdx.x; i < n; i += P2M_THREADS) s_chg[i] = schg[base + i];
-        __syncthreads();
-#pragma unroll
-        for (int s = 0; s < P2M_SLOTS; s++) {
-            int k = threadIdx.x + s * P2M_THREADS;
-            if (k >= Nc) break;
-            const int kx = kk[s][0], ky = kk[s][1], kz = kk[s][2];
-            double aV = 0.0, aK = 0.0;
-            for (int pt = 0; pt < n; pt++) {
-                double X = s_pw[pt][0][kx], Y = s_pw[pt][1][ky], Z = s_pw[pt][2][kz];
-                double4 c = s_chg[pt];
-                aV += c.x * X * Y * Z;
-                double t = 0.0;
-                if (kx) t += c.y * kx * s_pw[pt][0][kx - 1] * Y * Z;
-                if (ky) t += c.z * ky * X * s_pw[pt][1][ky - 1] * Z;
-                if (kz) t += c.w * kz * X * Y * s_pw[pt][2][kz - 1];
-                aK += t;
-            }
-            accV[s] += aV; accK[s] += aK;
-        }
+        pmom[((long)j * 2) * Nc + k] = gv;
+        pmom[((long)j * 2 + 1) * Nc + k] = gk;
     }
-#pragma unroll
-    for (int s = 0; s < P2M_SLOTS; s++) {
-        int k = threadIdx.x + s * P2M_THREADS;
-        if (k < Nc) { mom[((long)cell * 2) * Nc + k] = accV[s]; mom[((long)cell * 2 + 1) * Nc + k] = accK[s]; }
+}
+
+// One CTA per needed leaf, one work item (split s, coefficient k) per thread: split s takes every nsplit-th
+// panel of the leaf; the partial sums meet in shared memory in a fixed order (deterministic).
+#define P2M_MAXT 512
+static inline int p2m_nsplit(int Nc) { return Nc >= 192 ? 1 : (Nc >= 96 ? 2 : (256 / Nc > 8 ? 8 : 256 / Nc)); }
+static inline int p2m_threads(int Nc) { return (p2m_nsplit(Nc) * Nc + 31) / 32 * 32; }
+__global__ void __launch_bounds__(P2M_MAXT)
+k_p2m(const int *__restrict__ skip, int Nc, int nsplit, const int *__restrict__ leaf_cell,
+      const int2 *__restrict__ crange, const double *__restrict__ cV, const double *__restrict__ cK,
+      const double *__restrict__ pphi, const double *__restrict__ pdphi, const double *__restrict__ pmom,
+      double *__restrict__ mom, MomOut mo)
+{
+    __shared__ double s_part[2][P2M_MAXT];
+    if (skip && *skip) return;
+    const int cell = leaf_cell[blockIdx.x];
+    const int2 rg = crange[cell];
+    const int t = threadIdx.x;
+    const int sp = t / Nc, k = t - sp * Nc;
+    const bool active = sp < nsplit;
+    double aV = 0.0, aK = 0.0;
+    if (active) {
+#pragma unroll 4
+        for (int j = rg.x + sp; j < rg.y; j += nsplit) {
+            const double qV = cV[j] * pdphi[j], qK = cK[j] * pphi[j];
+            aV += qV * pmom[((long)j * 2) * Nc + k];
+            aK += qK * pmom[((long)j * 2 + 1) * Nc + k];
+        }
+        if (sp > 0) { s_part[0][t] = aV; s_part[1][t] = aK; }
+    }
+    if (nsplit > 1) __syncthreads();
+    if (active && sp == 0) {
+        for (int j = 1; j < nsplit; j++) { aV += s_part[0][t + j * Nc]; aK += s_part[1][t + j * Nc]; }
+        mom[((long)cell * 2) * Nc + k] = aV;
+        mom[((long)cell * 2 + 1) * Nc + k] = aK;
+        momc_store(mo, cell, k, aV, aK);
     }
 }
 
 // ------------------------------------------------------------------------------------------------ M2M
 // Parent moments from the children's ("shifted and added"), for both sets:
 //   M_p^k = sum_children sum_{l <= k} C(k,l) s^(k-l) M_c^l,   s = y_child - y_parent.
-// The shift factorises over the axes, so it is applied as three one-dimensional shifts (x, then y, then z)
-// through two shared-memory buffers: O(Nc P) work per child instead of O(Nc P^3).  All children of a parent
-// are shifted concurrently (work item = (child, coefficient)), then summed.  The index tables are staged
-// in shared memory (the first version read them from constant memory with divergent indices and was
-// latency-bound: 62 us per launch, profiles/r1a_first_path.md).  One CTA per listed parent cell; launched
-// level by level from the deepest upward, and only for the cells whose multipoles are used: those in
-// some M2P list and, to build those, all their descendants (build_lists.cuh).
-// Dynamic shared memory: 2 buffers x 8 children x 2 Nc doubles.
+// The shift factorises over the axes: three one-dimensional passes (x, then y, then z).  In a pass the
+// coefficients split into independent lines along the axis (all k with the other two indices (u, v) fixed,
+// u + v <= P, length L = P - u - v + 1), and on a line the shift is the binomial transform
+//   b_m <- sum_{l <= m} C(m,l) s^(m-l) b_l,
+// computed in registers without binomials or powers by L - 1 sweeps  b_m += s b_(m-1), m = L-1 .. i  (i = 1 ..
+// L-1).  One thread owns one line of one (child, set): it loads the line, sweeps, and stores it back in
+// place; a __syncthreads separates the passes; then the children are summed.  (The first version looped
+// over binomial terms through shared-memory tables per coefficient: ~1100 dependent instructions per warp
+// and cell, 12 us per level.)
+//
+// The whole upward pass is ONE launch of persistent CTAs.  Cells are listed deepest level first -- only those
+// whose multipoles are used: the ones in some M2P list and, to build those, all their descendants
+// (build_lists.cuh) -- and handed out by an atomic ticket; a parent waits for the ready flag of each internal
+// child.  A child's ticket is always smaller than its parent's, so the CTA holding it is already running: no
+// deadlock whatever the residency.  Ready flags hold the matvec number (never reset); the last CTA to leave
+// resets the ticket.  Children are read with ld.global.cg (written by other SMs during this launch).
+// rec[i] = (cell, first child, number of children, bit c set if child c is internal).
+// Dynamic shared memory: 8 children x 2 Nc doubles.
 #define M2M_THREADS 512
-static inline size_t m2m_smem_bytes(int Nc) { return (size_t)2 * 8 * 2 * Nc * sizeof(double); }
-__global__ void __launch_bounds__(M2M_THREADS)
-k_m2m(const int *__restrict__ skip, int P, int Nc, const int *__restrict__ cells, const IndexTables *__restrict__ tab,
-      const double4 *__restrict__ cgeo, const int2 *__restrict__ cchild, double *__restrict__ mom)
+#define M2M_SLOTS 3                      // 16 (P+1)(P+2)/2 lines <= 3 x 512 at P = 12
+static inline size_t m2m_smem_bytes(int Nc) { return (size_t)8 * 2 * Nc * sizeof(double); }
+
+__device__ __forceinline__ int ld_acquire(const int *p)
 {
-    extern __shared__ double s_dyn[];
-    __shared__ double s_pw[8][3][PYGBE_PMAX + 1];
-    __shared__ double s_binom[PYGBE_PMAX + 1][PYGBE_PMAX + 1];
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(int *p, int v)
+{
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// one pass over the lines this thread owns; AXIS = 0, 1, 2
+template <int PM, int AXIS>
+__device__ __forceinline__ void m2m_pass(int P, int Nc, int nch, const int *line, double *s_m,
+                                         const short (*s_idx3)[PYGBE_PMAX + 1][PYGBE_PMAX + 1], const double (*s_sh)[3])
+{
+#pragma unroll
+    for (int sl = 0; sl < M2M_SLOTS; sl++) {
+        const int q = line[sl];                                      // packed (child, set, u, v) or -1
+        if (q < 0) continue;
+        const int c = q >> 16, set = (q >> 8) & 1, u = (q >> 4) & 15, v = q & 15;
+        if (c >= nch) continue;
+        const int L = P - u - v + 1;
+        double *m = s_m + (c * 2 + set) * Nc;
+        const double s = s_sh[c][AXIS];
+        double b[PM + 1];
+        short id[PM + 1];
+#pragma unroll
+        for (int l = 0; l <= PM; l++) {
+            id[l] = l < L ? (AXIS == 0 ? s_idx3[l][u][v] : (AXIS == 1 ? s_idx3[u][l][v] : s_idx3[u][v][l])) : (short)0;
+            b[l] = l < L ? m[id[l]] : 0.0;
+        }
+#pragma unroll
+        for (int i = 1; i <= PM; i++)
+#pragma unroll
+            for (int mm = PM; mm >= i; mm--) b[mm] = fma(s, b[mm - 1], b[mm]);
+#pragma unroll
+        for (int l = 1; l <= PM; l++)
+            if (l < L) m[id[l]] = b[l];
+    }
+}
+
+template <int PM>
+__global__ void __launch_bounds__(M2M_THREADS)
+k_m2m(const int *__restrict__ skip, int P, int Nc, int n_cells, const int4 *__restrict__ rec,
+      const IndexTables *__restrict__ tab, const double4 *__restrict__ cgeo, double *mom, MomOut mo,
+      int *sync, int *ready, int epoch)
+{
+    extern __shared__ double s_m[];
     __shared__ short s_idx3[PYGBE_PMAX + 1][PYGBE_PMAX + 1][PYGBE_PMAX + 1];
-    __shared__ __align__(16) unsigned char s_k[PYGBE_NCMAX][4];
+    __shared__ double s_sh[8][3];
+    __shared__ int s_ticket;
     if (skip && *skip) return;
-    const int cell = cells[blockIdx.x];
-    const int2 ch = cchild[cell];
-    const int n2 = 2 * Nc, nch = ch.y, nw = nch * n2;
-    double *s_a = s_dyn, *s_b = s_dyn + 8 * n2;
-    for (int i = threadIdx.x; i < (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1); i += M2M_THREADS)
-        (&s_binom[0][0])[i] = (&tab->binom[0][0])[i];
+    const int n2 = 2 * Nc, nl = (P + 1) * (P + 2) / 2;
     for (int i = threadIdx.x; i < (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1); i += M2M_THREADS)
         (&s_idx3[0][0][0])[i] = (&tab->idx3[0][0][0])[i];
-    for (int i = threadIdx.x; i < Nc; i += M2M_THREADS)
-        *(uchar4 *)s_k[i] = *(const uchar4 *)tab->kxyz[i];
-    for (int w = threadIdx.x; w < nw; w += M2M_THREADS) s_a[w] = mom[(long)ch.x * n2 + w];   // children are contiguous
-    if (threadIdx.x < nch * 3) {
-        const int c = threadIdx.x / 3, a = threadIdx.x - 3 * c;
-        const double4 g = cgeo[ch.x + c], pg = cgeo[cell];
-        const double sft = a == 0 ? g.x - pg.x : (a == 1 ? g.y - pg.y : g.z - pg.z);
-        double pw = 1.0;
-        for (int e = 0; e <= P; e++) { s_pw[c][a][e] = pw; pw *= sft; }
+    // the lines this thread owns: the same for every cell
+    int line[M2M_SLOTS];
+#pragma unroll
+    for (int sl = 0; sl < M2M_SLOTS; sl++) {
+        const int w = threadIdx.x + sl * M2M_THREADS;
+        line[sl] = -1;
+        if (w < 16 * nl) {
+            const int cs = w / nl;
+            int j = w - cs * nl, u = 0;
+            while (j >= P - u + 1) { j -= P - u + 1; u++; }           // line j -> (u, v), u + v <= P
+            line[sl] = ((cs >> 1) << 16) | ((cs & 1) << 8) | (u << 4) | j;
+        }
     }
-    __syncthreads();
-    for (int w = threadIdx.x; w < nw; w += M2M_THREADS) {          // shift along x: s_a -> s_b
-        const int c = w / n2, e = w - c * n2, so = c * n2 + (e < Nc ? 0 : Nc), k = e < Nc ? e : e - Nc;
-        const int kx = s_k[k][0], ky = s_k[k][1], kz = s_k[k][2];
-        double a = 0.0;
-        for (int l = 0; l <= kx; l++) a += s_binom[kx][l] * s_pw[c][0][kx - l] * s_a[so + s_idx3[l][ky][kz]];
-        s_b[w] = a;
+    for (;;) {
+        __syncthreads();                                             // previous cell is done with shared memory
+        if (threadIdx.x == 0) s_ticket = atomicAdd(&sync[0], 1);
+        __syncthreads();
+        if (s_ticket >= n_cells) break;
+        const int4 rc = rec[s_ticket];
+        const int cell = rc.x, ch0 = rc.y, nch = rc.z;
+        if (threadIdx.x < nch && ((rc.w >> threadIdx.x) & 1))        // internal child: wait until it is built
+            while (ld_acquire(ready + ch0 + threadIdx.x) != epoch) __nanosleep(32);
+        if (threadIdx.x >= 32 && threadIdx.x < 32 + nch * 3) {
+            const int c = (threadIdx.x - 32) / 3, a = (threadIdx.x - 32) - 3 * c;
+            const double4 g = cgeo[ch0 + c], pg = cgeo[cell];
+            s_sh[c][a] = a == 0 ? g.x - pg.x : (a == 1 ? g.y - pg.y : g.z - pg.z);
+        }
+        __syncthreads();
+        for (int w = threadIdx.x; w < nch * n2; w += M2M_THREADS) s_m[w] = __ldcg(mom + (long)ch0 * n2 + w);   // children are contiguous
+        __syncthreads();
+        m2m_pass<PM, 0>(P, Nc, nch, line, s_m, s_idx3, s_sh);
+        __syncthreads();
+        m2m_pass<PM, 1>(P, Nc, nch, line, s_m, s_idx3, s_sh);
+        __syncthreads();
+        m2m_pass<PM, 2>(P, Nc, nch, line, s_m, s_idx3, s_sh);
+        __syncthreads();
+        for (int k = threadIdx.x; k < Nc; k += M2M_THREADS) {          // sum over the children
+            double mv = 0.0, mk = 0.0;
+            for (int c = 0; c < nch; c++) { mv += s_m[c * n2 + k]; mk += s_m[c * n2 + Nc + k]; }
+            mom[(long)cell * n2 + k] = mv;
+            mom[(long)cell * n2 + Nc + k] = mk;
+            momc_store(mo, cell, k, mv, mk);
+        }
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) st_release(ready + cell, epoch);
     }
-    __syncthreads();
-    for (int w = threadIdx.x; w < nw; w += M2M_THREADS) {          // shift along y: s_b -> s_a
-        const int c = w / n2, e = w - c * n2, so = c * n2 + (e < Nc ? 0 : Nc), k = e < Nc ? e : e - Nc;
-        const int kx = s_k[k][0], ky = s_k[k][1], kz = s_k[k][2];
-        double a = 0.0;
-        for (int l = 0; l <= ky; l++) a += s_binom[ky][l] * s_pw[c][1][ky - l] * s_b[so + s_idx3[kx][l][kz]];
-        s_a[w] = a;
+    if (threadIdx.x == 0) {
+        const int d = atomicAdd(&sync[1], 1);
+        if (d == (int)gridDim.x - 1) { sync[1] = 0; __threadfence(); sync[0] = 0; }
     }
-    __syncthreads();
-    for (int w = threadIdx.x; w < nw; w += M2M_THREADS) {          // shift along z: s_a -> s_b
-        const int c = w / n2, e = w - c * n2, so = c * n2 + (e < Nc ? 0 : Nc), k = e < Nc ? e : e - Nc;
-        const int kx = s_k[k][0], ky = s_k[k][1], kz = s_k[k][2];
-        double a = 0.0;
-        for (int l = 0; l <= kz; l++) a += s_binom[kz][l] * s_pw[c][2][kz - l] * s_a[so + s_idx3[kx][ky][l]];
-        s_b[w] = a;
-    }
-    __syncthreads();
-    for (int e = threadIdx.x; e < n2; e += M2M_THREADS) {          // sum over the children
-        double a = 0.0;
-        for (int c = 0; c < nch; c++) a += s_b[c * n2 + e];
-        mom[(long)cell * n2 + e] = a;
-    }
+}
+
+struct M2MLaunch {
+    const int *skip; int P, Nc, n_cells, grid; const int4 *rec; const IndexTables *tab; const double4 *cgeo;
+    double *mom; MomOut mo; int *sync, *ready; int epoch; cudaStream_t stream;
+};
+template <int PM> static void m2m_go(const M2MLaunch &a)
+{
+    k_m2m<PM><<<a.grid, M2M_THREADS, m2m_smem_bytes(a.Nc), a.stream>>>(a.skip, a.P, a.Nc, a.n_cells, a.rec, a.tab, a.cgeo,
+                                                                      a.mom, a.mo, a.sync, a.ready, a.epoch);
+}
+static void m2m_launch(const M2MLaunch &a)
+{
+    if (a.P <= 4) m2m_go<4>(a);
+    else if (a.P <= 6) m2m_go<6>(a);
+    else if (a.P <= 8) m2m_go<8>(a);
+    else m2m_go<PYGBE_PMAX>(a);
+}
+static cudaError_t m2m_configure()
+{
+    cudaError_t e = cudaFuncSetAttribute(k_m2m<PYGBE_PMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m2m_smem_bytes(PYGBE_NCMAX));
+    return e;
 }

@@ -15,7 +15,7 @@ static inline __host__ __device__ int m2p_stride(int Nc) { return (Nc + 3) / 4 *
 struct M2PArgs {
     const int *skip; const int4 *items; const int *m2p_cell; int n_items; int np;
     const double4 *tpos; const double4 *cgeo;
-    const void *momc;          // the region's multipoles ca * MV + cb * MK, already in T (k_mom_combine)
+    const void *momc;          // the region's multipoles ca * MV + cb * MK, already in T (written by P2M / M2M, farfield.cuh)
     double kappa; double *out;
     int yukawa; int fp32; cudaStream_t stream;
 };
@@ -153,15 +153,3 @@ k_m2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int *_
     if (ok) atomicAdd(out + t, acc);
 }
 
-// momc[cell][k] = (T)(ca MV^k + cb MK^k): the multipoles of one region in the arithmetic type of its M2P.
-template <typename T>
-__global__ void k_mom_combine(const int *__restrict__ skip, long ncells, int Nc, int stride,
-                              const double *__restrict__ mom, double ca, double cb, T *__restrict__ momc)
-{
-    if (skip && *skip) return;
-    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
-    if (i >= ncells * stride) return;
-    long cell = i / stride;
-    int k = (int)(i - cell * stride);
-    momc[i] = k < Nc ? (T)(ca * mom[cell * 2 * Nc + k] + cb * mom[(cell * 2 + 1) * Nc + k]) : T(0);
-}

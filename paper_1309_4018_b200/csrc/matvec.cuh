@@ -32,15 +32,10 @@ M2P_DECL(1) M2P_DECL(2) M2P_DECL(3) M2P_DECL(4) M2P_DECL(5) M2P_DECL(6)
 M2P_DECL(7) M2P_DECL(8) M2P_DECL(9) M2P_DECL(10) M2P_DECL(11) M2P_DECL(12)
 #undef M2P_DECL
 
-// M2P of region R with the multipoles ca MV + cb MK of the tree owner T, on stream st.
-static int launch_m2p(pygbe_handle *h, Region &T, Region &R, double ca, double cb, const int *skip, cudaStream_t st)
+// M2P of region R over the lists of the tree owner T, on stream st; R.momc was written by P2M / M2M.
+static int launch_m2p(pygbe_handle *h, Region &T, Region &R, const int *skip, cudaStream_t st)
 {
     const bool fp32 = h->precision == PYGBE_PRECISION_MIXED;
-    const int stride = m2p_stride(h->Nc);
-    const long nel = (long)T.ncells * stride;
-    // the region's multipoles in the arithmetic type of its M2P (LAUNCH issues on h->stream == st here)
-    if (fp32) LAUNCH(h, k_mom_combine<float>, cdiv(nel, 256), 256, 0, skip, (long)T.ncells, h->Nc, stride, T.mom, ca, cb, (float *)R.momc);
-    else LAUNCH(h, k_mom_combine<double>, cdiv(nel, 256), 256, 0, skip, (long)T.ncells, h->Nc, stride, T.mom, ca, cb, (double *)R.momc);
     M2PArgs a;
     memset(&a, 0, sizeof(a));
     a.skip = skip; a.items = T.m2p_items; a.m2p_cell = T.m2p_cell; a.n_items = T.n_m2p_items; a.np = T.np;
@@ -86,26 +81,32 @@ static int region_sum(pygbe_handle *h, Region &A, Region *B, const double *x, do
            A.schg, mixed ? A.schgf : (float4 *)nullptr, A.pphi, A.pdphi, A.out, B ? B->out : (double *)nullptr);
     STAGE_END(h, PYGBE_STAGE_PREP);
     cudaStream_t main_st = h->stream, fs = fork ? h->side : h->stream;
+    if (fork) { cudaEventRecord(h->ev_fork, main_st); cudaStreamWaitEvent(fs, h->ev_fork, 0); }
     if (far) {
-        if (fork) { cudaEventRecord(h->ev_fork, main_st); cudaStreamWaitEvent(fs, h->ev_fork, 0); }
         cudaStream_t keep = h->stream;
         h->stream = fs;                      // LAUNCH issues on h->stream
+        // multipoles leave P2M / M2M already combined for the M2P of A (MV - MK) and of its twin (rV MV + MK)
+        MomOut mo;
+        mo.A = A.momc; mo.B = B ? B->momc : nullptr; mo.caA = 1.0; mo.cbA = -1.0; mo.caB = A.twin_rV; mo.cbB = 1.0;
+        mo.fp32 = mixed ? 1 : 0; mo.stride = m2p_stride(h->Nc);
         STAGE(h, PYGBE_STAGE_P2M);
         if (A.n_p2m > 0)
-            LAUNCH(h, k_p2m, A.n_p2m, P2M_THREADS, 0, skip, h->P, h->Nc, h->K, h->itab, A.p2m_cells, A.cgeo, A.crange,
-                   A.spos, A.schg, A.mom);
+            LAUNCH(h, k_p2m, A.n_p2m, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.p2m_cells, A.crange, A.cV, A.cK,
+                   A.pphi, A.pdphi, A.pmom, A.mom, mo);
         STAGE_END(h, PYGBE_STAGE_P2M);
         STAGE(h, PYGBE_STAGE_M2M);
-        for (int l = A.depth - 2; l >= 0; l--) {           // only the cells some M2P list depends on
-            int b = A.m2m_off[l], e = A.m2m_off[l + 1];
-            if (e > b)
-                LAUNCH(h, k_m2m, e - b, M2M_THREADS, m2m_smem_bytes(h->Nc), skip, h->P, h->Nc, A.m2m_cells + b, h->itab,
-                       A.cgeo, A.cchild, A.mom);
+        if (A.n_m2m > 0) {
+            M2MLaunch ml;
+            ml.skip = skip; ml.P = h->P; ml.Nc = h->Nc; ml.n_cells = A.n_m2m; ml.grid = std::min(A.n_m2m, 3 * h->n_sm);
+            ml.rec = A.m2m_rec; ml.tab = h->itab; ml.cgeo = A.cgeo; ml.mom = A.mom; ml.mo = mo; ml.sync = A.up_sync;
+            ml.ready = A.cready; ml.epoch = (int)(h->n_matvec + 1); ml.stream = h->stream;
+            m2m_launch(ml);
+            h->launches++;
         }
         STAGE_END(h, PYGBE_STAGE_M2M);
         STAGE(h, PYGBE_STAGE_M2P);
-        TRY(launch_m2p(h, A, A, 1.0, -1.0, skip, fs));
-        if (B) TRY(launch_m2p(h, A, *B, A.twin_rV, 1.0, skip, fs));
+        TRY(launch_m2p(h, A, A, skip, fs));
+        if (B) TRY(launch_m2p(h, A, *B, skip, fs));
         STAGE_END(h, PYGBE_STAGE_M2P);
         h->stream = keep;
         if (fork) cudaEventRecord(h->ev_join, fs);
