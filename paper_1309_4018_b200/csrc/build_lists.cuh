@@ -134,6 +134,9 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
         R.n_m2m = (int)m2m_rec.size();
         R.n_p2m = (int)p2m_cells.size();
         TRY(upload(h, &R.p2m_cells, p2m_cells)); TRY(upload(h, &R.m2m_rec, m2m_rec));
+        std::vector<int4> p2m_rec;
+        for (int c : p2m_cells) p2m_rec.push_back(make_int4(c, crange_h[c].x, crange_h[c].y, 0));
+        TRY(upload(h, &R.p2m_rec, p2m_rec));
         TRY(h->mem.alloc(&R.up_sync, 2)); TRY(h->mem.alloc(&R.cready, (size_t)ncells));
         CUDA_TRY(cudaMemsetAsync(R.up_sync, 0, 2 * sizeof(int), h->stream));
         CUDA_TRY(cudaMemsetAsync(R.cready, 0, (size_t)ncells * sizeof(int), h->stream));

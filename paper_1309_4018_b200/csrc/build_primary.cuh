@@ -54,7 +54,7 @@ static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<do
     TRY(h->mem.alloc(&R.row_idx, R.np)); TRY(h->mem.alloc(&R.cV, R.np)); TRY(h->mem.alloc(&R.cK, R.np));
     TRY(h->mem.alloc(&R.tpos, R.np)); TRY(h->mem.alloc(&R.pnrm, R.np));
     TRY(h->mem.alloc(&R.spos, R.npts)); TRY(h->mem.alloc(&R.schg, R.npts));
-    TRY(h->mem.alloc(&R.pphi, R.np)); TRY(h->mem.alloc(&R.pdphi, R.np)); TRY(h->mem.alloc(&R.out, R.np));
+    TRY(h->mem.alloc(&R.pphi, R.np)); TRY(h->mem.alloc(&R.pdphi, R.np)); TRY(h->mem.alloc(&R.out, R.np)); TRY(h->mem.alloc(&R.corr, R.np)); TRY(h->mem.alloc(&R.pq, R.np));
     LAUNCH(h, k_region_gather, cdiv(R.np, 128), 128, 0, R.np, K, qt, R.perm, d_gid_u, d_phi_u, d_dphi_u, d_row_u,
            d_cV_u, d_cK_u, h->tri, h->gcen, h->gnrm, R.gid, R.phi_idx, R.dphi_idx, R.row_idx, R.cV, R.cK, R.tpos,
            R.pnrm, R.spos);

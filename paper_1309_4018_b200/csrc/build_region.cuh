@@ -89,7 +89,7 @@ static int build_region_twin(pygbe_handle *h, Region &B, Region &A, const QuadTa
     int *d_row_u; double *d_cV_u, *d_cK_u;
     TRY(upload(h, &d_row_u, b.row)); TRY(upload(h, &d_cV_u, b.cV)); TRY(upload(h, &d_cK_u, b.cK));
     TRY(h->mem.alloc(&B.row_idx, B.np)); TRY(h->mem.alloc(&B.cV, B.np)); TRY(h->mem.alloc(&B.cK, B.np));
-    TRY(h->mem.alloc(&B.out, B.np));
+    TRY(h->mem.alloc(&B.out, B.np)); TRY(h->mem.alloc(&B.corr, B.np));
     B.momc = nullptr;
     if (A.n_m2p_items > 0) {
         const size_t mc_bytes = (size_t)A.ncells * ((h->Nc + 3) / 4 * 4) * sizeof(double);

@@ -105,7 +105,9 @@ struct Region {
     float4 *sposf = nullptr;        // mixed precision: position relative to the anchor cell centre, weight
     float4 *schgf = nullptr;
     double *pphi = nullptr, *pdphi = nullptr;   // per matvec: gathered densities
+    double2 *pq = nullptr;          // per matvec: (cV dphi, cK phi) per panel, the weights of the panel moments (P2M)
     double *out = nullptr;          // per matvec: sum_S sigma_S [c_S V dphi - K phi] at each target
+    double *corr = nullptr;         // per matvec: the singular / near-singular correction of that sum (k_near)
     // octree ----------------------------------------------------------------------------------------
     unsigned long long *keys = nullptr;
     int ncells = 0, nleaves = 0, depth = 0;
@@ -118,6 +120,7 @@ struct Region {
     int *leaf_cell = nullptr;       // leaves in Morton order
     // cells whose multipoles are needed: those in some M2P list and all their descendants
     int *p2m_cells = nullptr; int n_p2m = 0;        // needed leaves (P2M)
+    int4 *p2m_rec = nullptr;                        // per needed leaf: (cell, first panel, end panel, 0)
     int4 *m2m_rec = nullptr; int n_m2m = 0;         // needed internal cells, deepest level first: (cell, first child, n children, internal-child mask)
     double *pmom = nullptr;                         // [np][2][Nc] geometry-only panel moments about the panel's leaf centre (P2M)
     int *up_sync = nullptr;                         // [2] ticket and exit counters of the upward pass
@@ -179,7 +182,8 @@ struct pygbe_handle {
     double *phi_reac = nullptr;     // [nq]
     struct IndexTables *itab = nullptr;   // device copy of the multi-index tables
     cudaStream_t side = nullptr;    // far-field chain (P2M, M2M, M2P) runs here, concurrently with P2P
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaStream_t side2 = nullptr;   // near-field correction SpMV runs here
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_join2 = nullptr;
     bool overlap = true;
     // optional block-diagonal right preconditioner of GMRES (pygbe_options.precond)
     int precond = 0;

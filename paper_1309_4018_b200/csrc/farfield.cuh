@@ -39,7 +39,7 @@ __device__ __forceinline__ void momc_store(const MomOut &o, long cell, int k, do
 // leaf, K-point rule:
 //     GV_j^k = sum_g w_g d_g^k,     GK_j^k = sum_g w_g sum_i n_j,i k_i d_g^(k - e_i),     d_g = y_jg - y_c
 //     MV^k(leaf) = sum_{j in leaf} (cV_j dphi_j) GV_j^k,      MK^k(leaf) = sum_{j in leaf} (cK_j phi_j) GK_j^k
-// (cV, cK: the per-region constants folded into the densities, nearfield.cuh k_prep).  Each matvec the P2M is
+// (cV, cK: the per-region constants folded into the densities; k_prep leaves the two products in pq).  Each matvec the P2M is
 // then a streaming product: 2 Nc doubles read per panel, coalesced, two FMAs per 16 bytes -- HBM / L2 bound
 // as SURVEY 8(d) puts it (27.5 MB at 20 480 panels and P = 6) instead of the ALU- and latency-bound
 // monomial loop over the Gauss points of the first versions (29 us -> see profiles/r2a_upward.md).
@@ -81,25 +81,23 @@ k_panel_moments(int P, int Nc, int K, const IndexTables *__restrict__ tab, const
 static inline int p2m_nsplit(int Nc) { return Nc >= 192 ? 1 : (Nc >= 96 ? 2 : (256 / Nc > 8 ? 8 : 256 / Nc)); }
 static inline int p2m_threads(int Nc) { return (p2m_nsplit(Nc) * Nc + 31) / 32 * 32; }
 __global__ void __launch_bounds__(P2M_MAXT)
-k_p2m(const int *__restrict__ skip, int Nc, int nsplit, const int *__restrict__ leaf_cell,
-      const int2 *__restrict__ crange, const double *__restrict__ cV, const double *__restrict__ cK,
-      const double *__restrict__ pphi, const double *__restrict__ pdphi, const double *__restrict__ pmom,
-      double *__restrict__ mom, MomOut mo)
+k_p2m(const int *__restrict__ skip, int Nc, int nsplit, const int4 *__restrict__ rec, const double2 *__restrict__ pq,
+      const double *__restrict__ pmom, double *__restrict__ mom, MomOut mo)
 {
     __shared__ double s_part[2][P2M_MAXT];
     if (skip && *skip) return;
-    const int cell = leaf_cell[blockIdx.x];
-    const int2 rg = crange[cell];
+    const int4 rc = rec[blockIdx.x];                               // (cell, first panel, end panel, -)
+    const int cell = rc.x;
     const int t = threadIdx.x;
     const int sp = t / Nc, k = t - sp * Nc;
     const bool active = sp < nsplit;
     double aV = 0.0, aK = 0.0;
     if (active) {
 #pragma unroll 4
-        for (int j = rg.x + sp; j < rg.y; j += nsplit) {
-            const double qV = cV[j] * pdphi[j], qK = cK[j] * pphi[j];
-            aV += qV * pmom[((long)j * 2) * Nc + k];
-            aK += qK * pmom[((long)j * 2 + 1) * Nc + k];
+        for (int j = rc.y + sp; j < rc.z; j += nsplit) {
+            const double2 q = pq[j];                               // (cV dphi, cK phi) of panel j, from k_prep
+            aV += q.x * pmom[((long)j * 2) * Nc + k];
+            aK += q.y * pmom[((long)j * 2 + 1) * Nc + k];
         }
         if (sp > 0) { s_part[0][t] = aV; s_part[1][t] = aK; }
     }

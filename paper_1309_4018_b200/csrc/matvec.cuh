@@ -1,8 +1,6 @@
 // matvec.cuh -- one evaluation of the treecode, y = A x: kernel launches only.
-//   main stream : prep -> P2P (twin regions fused) ----------------------> near-field corrections -> combine
-//   side stream :      -> P2M -> M2M (per level) -> M2P (per region) ---^   (joined by an event)
-// The far-field chain is latency-bound at small sizes (one launch per tree level); running it beside the
-// compute-bound P2P hides it.  With the stage timers on, everything is issued on the main stream instead.
+// Three streams, joined by events (see matvec_impl); with the stage timers on, everything is issued on the
+// main stream instead.
 #pragma once
 #include "common.cuh"
 #include "nearfield.cuh"
@@ -69,70 +67,103 @@ static void launch_p2p(pygbe_handle *h, Region &A, Region *B, const int *skip)
 #undef P2P_GO
 }
 
-// The rows of one tree owner A (and of its twin B, if any).
-static int region_sum(pygbe_handle *h, Region &A, Region *B, const double *x, double *y, const int *skip)
-{
-    if (A.np == 0) return PYGBE_OK;
-    const bool mixed = h->precision == PYGBE_PRECISION_MIXED;
-    const bool far = A.n_m2p_items > 0;
-    const bool fork = far && h->overlap && !h->profile && h->side != nullptr;
-    STAGE(h, PYGBE_STAGE_PREP);
-    LAUNCH(h, k_prep, cdiv(A.np, 128), 128, 0, skip, A.np, h->K, x, A.phi_idx, A.dphi_idx, A.cV, A.cK, A.pnrm, A.spos,
-           A.schg, mixed ? A.schgf : (float4 *)nullptr, A.pphi, A.pdphi, A.out, B ? B->out : (double *)nullptr);
-    STAGE_END(h, PYGBE_STAGE_PREP);
-    cudaStream_t main_st = h->stream, fs = fork ? h->side : h->stream;
-    if (fork) { cudaEventRecord(h->ev_fork, main_st); cudaStreamWaitEvent(fs, h->ev_fork, 0); }
-    if (far) {
-        cudaStream_t keep = h->stream;
-        h->stream = fs;                      // LAUNCH issues on h->stream
-        // multipoles leave P2M / M2M already combined for the M2P of A (MV - MK) and of its twin (rV MV + MK)
-        MomOut mo;
-        mo.A = A.momc; mo.B = B ? B->momc : nullptr; mo.caA = 1.0; mo.cbA = -1.0; mo.caB = A.twin_rV; mo.cbB = 1.0;
-        mo.fp32 = mixed ? 1 : 0; mo.stride = m2p_stride(h->Nc);
-        STAGE(h, PYGBE_STAGE_P2M);
-        if (A.n_p2m > 0)
-            LAUNCH(h, k_p2m, A.n_p2m, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.p2m_cells, A.crange, A.cV, A.cK,
-                   A.pphi, A.pdphi, A.pmom, A.mom, mo);
-        STAGE_END(h, PYGBE_STAGE_P2M);
-        STAGE(h, PYGBE_STAGE_M2M);
-        if (A.n_m2m > 0) {
-            M2MLaunch ml;
-            ml.skip = skip; ml.P = h->P; ml.Nc = h->Nc; ml.n_cells = A.n_m2m; ml.grid = std::min(A.n_m2m, 3 * h->n_sm);
-            ml.rec = A.m2m_rec; ml.tab = h->itab; ml.cgeo = A.cgeo; ml.mom = A.mom; ml.mo = mo; ml.sync = A.up_sync;
-            ml.ready = A.cready; ml.epoch = (int)(h->n_matvec + 1); ml.stream = h->stream;
-            m2m_launch(ml);
-            h->launches++;
-        }
-        STAGE_END(h, PYGBE_STAGE_M2M);
-        STAGE(h, PYGBE_STAGE_M2P);
-        TRY(launch_m2p(h, A, A, skip, fs));
-        if (B) TRY(launch_m2p(h, A, *B, skip, fs));
-        STAGE_END(h, PYGBE_STAGE_M2P);
-        h->stream = keep;
-        if (fork) cudaEventRecord(h->ev_join, fs);
-    }
-    if (A.n_p2p_items > 0) {
-        STAGE(h, PYGBE_STAGE_P2P);
-        if (mixed) launch_p2p<float>(h, A, B, skip); else launch_p2p<double>(h, A, B, skip);
-        STAGE_END(h, PYGBE_STAGE_P2P);
-    }
-    if (fork) cudaStreamWaitEvent(main_st, h->ev_join, 0);
-    STAGE(h, PYGBE_STAGE_NEAR);
-    LAUNCH(h, k_near_combine, cdiv(A.np, 128), 128, 0, skip, A.np, A.corr_off, A.corr_col, A.corr_val,
-           B ? B->corr_val : (const double2 *)nullptr, A.pphi, A.pdphi, A.out, B ? B->out : (const double *)nullptr,
-           A.row_idx, B ? B->row_idx : (const int *)nullptr, y);
-    STAGE_END(h, PYGBE_STAGE_NEAR);
-    return PYGBE_OK;
-}
-
+// One matvec, phase by phase over the tree owners A (each with its twin B, if any):
+//   main  : prep (all) ........ P2P (all) ............................. combine (all)
+//   side  :            P2M, M2M (all) -> M2P (all) ------------------^
+//   side2 :            near-field corrections (all) -----------------^
+// Issuing every region's latency-bound kernels (prep, P2M, M2M, corrections) first lets them run beside the
+// compute-bound P2P / M2P of the regions before them instead of between them.
 static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *skip)
 {
-    long before = h->launches;
+    const long before = h->launches;
+    const bool mixed = h->precision == PYGBE_PRECISION_MIXED;
+    std::vector<std::pair<Region *, Region *>> work;
+    bool any_far = false;
     for (Region &R : h->regions) {
         if (R.np == 0 || R.twin_of >= 0) continue;
-        Region *B = R.twin >= 0 ? &h->regions[R.twin] : nullptr;
-        TRY(region_sum(h, R, B, x, y, skip));
+        work.push_back({&R, R.twin >= 0 ? &h->regions[R.twin] : nullptr});
+        any_far = any_far || R.n_m2p_items > 0;
     }
+    const bool fork = h->overlap && !h->profile && h->side != nullptr && h->side2 != nullptr;
+    cudaStream_t main_st = h->stream;
+
+    STAGE(h, PYGBE_STAGE_PREP);
+    for (auto &w : work) {
+        Region &A = *w.first; Region *B = w.second;
+        LAUNCH(h, k_prep, cdiv((long)A.np * h->K, 256), 256, 0, skip, A.np, h->K, x, A.phi_idx, A.dphi_idx, A.cV, A.cK, A.pnrm,
+               A.spos, A.schg, mixed ? A.schgf : (float4 *)nullptr, A.pphi, A.pdphi, A.pq, A.out, B ? B->out : (double *)nullptr);
+    }
+    STAGE_END(h, PYGBE_STAGE_PREP);
+    if (fork) {
+        cudaEventRecord(h->ev_fork, main_st);
+        cudaStreamWaitEvent(h->side, h->ev_fork, 0);
+        cudaStreamWaitEvent(h->side2, h->ev_fork, 0);
+    }
+
+    // singular / near-singular corrections: need the gathered densities only
+    h->stream = fork ? h->side2 : main_st;                 // LAUNCH issues on h->stream
+    STAGE(h, PYGBE_STAGE_NEAR);
+    for (auto &w : work) {
+        Region &A = *w.first; Region *B = w.second;
+        LAUNCH(h, k_near, cdiv((long)A.np * NEAR_LANES, 128), 128, 0, skip, A.np, A.corr_off, A.corr_col, A.corr_val,
+               B ? B->corr_val : (const double2 *)nullptr, A.pphi, A.pdphi, A.corr, B ? B->corr : (double *)nullptr);
+    }
+    STAGE_END(h, PYGBE_STAGE_NEAR);
+    if (fork) cudaEventRecord(h->ev_join2, h->side2);
+
+    // far field: upward passes of all trees, then their M2P
+    h->stream = fork ? h->side : main_st;
+    if (any_far) {
+        for (auto &w : work) {
+            Region &A = *w.first; Region *B = w.second;
+            if (A.n_m2p_items == 0) continue;
+            // multipoles leave P2M / M2M already combined for the M2P of A (MV - MK) and of its twin (rV MV + MK)
+            MomOut mo;
+            mo.A = A.momc; mo.B = B ? B->momc : nullptr; mo.caA = 1.0; mo.cbA = -1.0; mo.caB = A.twin_rV; mo.cbB = 1.0;
+            mo.fp32 = mixed ? 1 : 0; mo.stride = m2p_stride(h->Nc);
+            STAGE(h, PYGBE_STAGE_P2M);
+            if (A.n_p2m > 0)
+                LAUNCH(h, k_p2m, A.n_p2m, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.p2m_rec, A.pq, A.pmom, A.mom, mo);
+            STAGE_END(h, PYGBE_STAGE_P2M);
+            STAGE(h, PYGBE_STAGE_M2M);
+            if (A.n_m2m > 0) {
+                M2MLaunch ml;
+                ml.skip = skip; ml.P = h->P; ml.Nc = h->Nc; ml.n_cells = A.n_m2m; ml.grid = std::min(A.n_m2m, 3 * h->n_sm);
+                ml.rec = A.m2m_rec; ml.tab = h->itab; ml.cgeo = A.cgeo; ml.mom = A.mom; ml.mo = mo; ml.sync = A.up_sync;
+                ml.ready = A.cready; ml.epoch = (int)(h->n_matvec + 1); ml.stream = h->stream;
+                m2m_launch(ml);
+                h->launches++;
+            }
+            STAGE_END(h, PYGBE_STAGE_M2M);
+        }
+        STAGE(h, PYGBE_STAGE_M2P);
+        for (auto &w : work) {
+            Region &A = *w.first; Region *B = w.second;
+            if (A.n_m2p_items == 0) continue;
+            int rc = launch_m2p(h, A, A, skip, h->stream);
+            if (rc == PYGBE_OK && B) rc = launch_m2p(h, A, *B, skip, h->stream);
+            if (rc != PYGBE_OK) { h->stream = main_st; return rc; }
+        }
+        STAGE_END(h, PYGBE_STAGE_M2P);
+    }
+    if (fork) cudaEventRecord(h->ev_join, h->side);
+
+    h->stream = main_st;
+    STAGE(h, PYGBE_STAGE_P2P);
+    for (auto &w : work) {
+        Region &A = *w.first; Region *B = w.second;
+        if (A.n_p2p_items == 0) continue;
+        if (mixed) launch_p2p<float>(h, A, B, skip); else launch_p2p<double>(h, A, B, skip);
+    }
+    STAGE_END(h, PYGBE_STAGE_P2P);
+    if (fork) { cudaStreamWaitEvent(main_st, h->ev_join, 0); cudaStreamWaitEvent(main_st, h->ev_join2, 0); }
+    STAGE(h, PYGBE_STAGE_COMBINE);
+    for (auto &w : work) {
+        Region &A = *w.first; Region *B = w.second;
+        LAUNCH(h, k_combine, cdiv(A.np, 256), 256, 0, skip, A.np, A.pphi, A.out, B ? B->out : (const double *)nullptr, A.corr,
+               B ? B->corr : (const double *)nullptr, A.row_idx, B ? B->row_idx : (const int *)nullptr, y);
+    }
+    STAGE_END(h, PYGBE_STAGE_COMBINE);
     stage_mark(h, -1);
     h->kernels_per_matvec = h->launches - before;
     h->n_matvec++;

@@ -36,23 +36,25 @@ __global__ void k_prep(const int *__restrict__ skip, int np, int K, const double
                        const double *__restrict__ cK, const double4 *__restrict__ pnrm,
                        const double4 *__restrict__ spos, double4 *__restrict__ schg,
                        float4 *__restrict__ schgf, double *__restrict__ pphi, double *__restrict__ pdphi,
-                       double *__restrict__ out, double *__restrict__ out_twin)
+                       double2 *__restrict__ pq, double *__restrict__ out, double *__restrict__ out_twin)
 {
     if (skip && *skip) return;
-    int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= np) return;
-    double phi = x[phi_idx[p]], dphi = x[dphi_idx[p]];
-    pphi[p] = phi; pdphi[p] = dphi;
-    out[p] = 0.0;
-    if (out_twin) out_twin[p] = 0.0;
-    double qV = cV[p] * dphi, qK = cK[p] * phi;
-    double4 n = pnrm[p];
-    for (int g = 0; g < K; g++) {
-        double w = spos[(long)p * K + g].w;
-        double4 c = make_double4(w * qV, w * qK * n.x, w * qK * n.y, w * qK * n.z);
-        schg[(long)p * K + g] = c;
-        if (schgf) schgf[(long)p * K + g] = make_float4((float)c.x, (float)c.y, (float)c.z, (float)c.w);
+    const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;      // Gauss point
+    if (i >= (long)np * K) return;
+    const int p = (int)(i / K), g = (int)(i - (long)p * K);
+    const double phi = x[phi_idx[p]], dphi = x[dphi_idx[p]];
+    const double qV = cV[p] * dphi, qK = cK[p] * phi;
+    if (g == 0) {
+        pphi[p] = phi; pdphi[p] = dphi;
+        if (pq) pq[p] = make_double2(qV, qK);
+        out[p] = 0.0;
+        if (out_twin) out_twin[p] = 0.0;
     }
+    const double4 n = pnrm[p];
+    const double w = spos[i].w;
+    const double4 c = make_double4(w * qV, w * qK * n.x, w * qK * n.y, w * qK * n.z);
+    schg[i] = c;
+    if (schgf) schgf[i] = make_float4((float)c.x, (float)c.y, (float)c.z, (float)c.w);
 }
 
 // ------------------------------------------------------------------- singular / near-singular panels
@@ -171,38 +173,60 @@ __global__ void k_near_values(int np, QuadTables q, bool yukawa, double kappa, c
     }
 }
 
-// Correction SpMV (a8) fused with the block combination (a9) for a region and, optionally, its twin (same
-// sparsity pattern, own values):  y[row] = 1/2 phi - ( out + sum_e [ val.x dphi_j - val.y phi_j ] ).
-__global__ void k_near_combine(const int *__restrict__ skip, int np, const int *__restrict__ off,
-                               const int *__restrict__ col, const double2 *__restrict__ valA,
-                               const double2 *__restrict__ valB, const double *__restrict__ pphi,
-                               const double *__restrict__ pdphi, const double *__restrict__ outA,
-                               const double *__restrict__ outB, const int *__restrict__ rowA,
-                               const int *__restrict__ rowB, double *__restrict__ y)
+// Correction SpMV (a8) for a region and, optionally, its twin (same sparsity pattern, own values):
+//   corr[t] = sum_e [ val.x dphi_j - val.y phi_j ].
+// It needs only the gathered densities, so it runs on its own stream beside the P2P / M2P and is
+// latency-bound (~50 entries per row): four lanes share a row, partial sums meet by shuffles in a fixed order.
+#define NEAR_LANES 4
+__global__ void __launch_bounds__(128)
+k_near(const int *__restrict__ skip, int np, const int *__restrict__ off, const int *__restrict__ col,
+       const double2 *__restrict__ valA, const double2 *__restrict__ valB, const double *__restrict__ pphi,
+       const double *__restrict__ pdphi, double *__restrict__ corrA, double *__restrict__ corrB)
 {
     if (skip && *skip) return;
-    int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= np) return;
+    const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+    const int t = gt / NEAR_LANES, lane = gt % NEAR_LANES;
     double accA = 0.0, accB = 0.0;
-    const int e0 = off[t], e1 = off[t + 1];
-    if (valB) {
-        for (int e = e0; e < e1; e++) {
-            int j = col[e];
-            double ph = pphi[j], dp = pdphi[j];
-            double2 a = valA[e], b = valB[e];
-            accA += a.x * dp - a.y * ph;
-            accB += b.x * dp - b.y * ph;
-        }
-    } else {
-        for (int e = e0; e < e1; e++) {
-            int j = col[e];
-            double2 a = valA[e];
-            accA += a.x * pdphi[j] - a.y * pphi[j];
+    if (t < np) {
+        const int e0 = off[t], e1 = off[t + 1];
+        if (valB) {
+#pragma unroll 2
+            for (int e = e0 + lane; e < e1; e += NEAR_LANES) {
+                const int j = col[e];
+                const double ph = pphi[j], dp = pdphi[j];
+                const double2 a = valA[e], b = valB[e];
+                accA += a.x * dp - a.y * ph;
+                accB += b.x * dp - b.y * ph;
+            }
+        } else {
+#pragma unroll 2
+            for (int e = e0 + lane; e < e1; e += NEAR_LANES) {
+                const int j = col[e];
+                const double2 a = valA[e];
+                accA += a.x * pdphi[j] - a.y * pphi[j];
+            }
         }
     }
+#pragma unroll
+    for (int o = 1; o < NEAR_LANES; o <<= 1) {
+        accA += __shfl_xor_sync(0xffffffffu, accA, o);
+        accB += __shfl_xor_sync(0xffffffffu, accB, o);
+    }
+    if (t < np && lane == 0) { corrA[t] = accA; if (valB) corrB[t] = accB; }
+}
+
+// Block combination (a9), eq. (10):  y[row] = 1/2 phi - ( out + corr ).
+__global__ void k_combine(const int *__restrict__ skip, int np, const double *__restrict__ pphi,
+                          const double *__restrict__ outA, const double *__restrict__ outB,
+                          const double *__restrict__ corrA, const double *__restrict__ corrB,
+                          const int *__restrict__ rowA, const int *__restrict__ rowB, double *__restrict__ y)
+{
+    if (skip && *skip) return;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= np) return;
     const double half_phi = 0.5 * pphi[t];
-    y[rowA[t]] = half_phi - (outA[t] + accA);
-    if (valB) y[rowB[t]] = half_phi - (outB[t] + accB);
+    y[rowA[t]] = half_phi - (outA[t] + corrA[t]);
+    if (outB) y[rowB[t]] = half_phi - (outB[t] + corrB[t]);
 }
 
 // ------------------------------------------------------------------------------------------------ RHS

@@ -30,7 +30,9 @@ static void free_handle(pygbe_handle *h)
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->ev_join) cudaEventDestroy(h->ev_join);
+    if (h->ev_join2) cudaEventDestroy(h->ev_join2);
     if (h->side) cudaStreamDestroy(h->side);
+    if (h->side2) cudaStreamDestroy(h->side2);
     delete h;
 }
 
@@ -42,6 +44,7 @@ extern "C" void pygbe_destroy(pygbe_handle *h)
     cudaSetDevice(h->device);
     cudaStreamSynchronize(h->stream);
     if (h->side) cudaStreamSynchronize(h->side);
+    if (h->side2) cudaStreamSynchronize(h->side2);
     free_handle(h);
 }
 
