@@ -70,9 +70,6 @@ static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<do
         if (R.n_p2m > 0)
             LAUNCH(h, k_panel_moments, R.n_p2m, PMOM_THREADS, 0, h->P, h->Nc, h->K, h->itab, R.p2m_cells, R.cgeo, R.crange,
                    R.spos, R.pnrm, R.pmom);
-        const size_t mc_bytes = (size_t)R.ncells * ((h->Nc + 3) / 4 * 4) * sizeof(double);
-        TRY(h->mem.alloc((char **)&R.momc, mc_bytes));
-        CUDA_TRY(cudaMemsetAsync(R.momc, 0, mc_bytes, h->stream));       // row padding stays zero
     }
     CUDA_TRY(cudaGetLastError());
     return PYGBE_OK;

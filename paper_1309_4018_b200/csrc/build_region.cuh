@@ -90,12 +90,6 @@ static int build_region_twin(pygbe_handle *h, Region &B, Region &A, const QuadTa
     TRY(upload(h, &d_row_u, b.row)); TRY(upload(h, &d_cV_u, b.cV)); TRY(upload(h, &d_cK_u, b.cK));
     TRY(h->mem.alloc(&B.row_idx, B.np)); TRY(h->mem.alloc(&B.cV, B.np)); TRY(h->mem.alloc(&B.cK, B.np));
     TRY(h->mem.alloc(&B.out, B.np)); TRY(h->mem.alloc(&B.corr, B.np));
-    B.momc = nullptr;
-    if (A.n_m2p_items > 0) {
-        const size_t mc_bytes = (size_t)A.ncells * ((h->Nc + 3) / 4 * 4) * sizeof(double);
-        TRY(h->mem.alloc((char **)&B.momc, mc_bytes));
-        CUDA_TRY(cudaMemsetAsync(B.momc, 0, mc_bytes, h->stream));       // row padding stays zero
-    }
     LAUNCH(h, k_gather_twin, cdiv(B.np, 256), 256, 0, B.np, A.perm, d_row_u, d_cV_u, d_cK_u, B.row_idx, B.cV, B.cK);
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     for (void *q : {(void *)d_row_u, (void *)d_cV_u, (void *)d_cK_u}) h->mem.release_one(q);

@@ -140,7 +140,8 @@ struct Region {
     long p2p_pairs = 0, m2p_evals = 0;
     // multipoles ------------------------------------------------------------------------------------
     double *mom = nullptr;          // [ncells][2][Nc]: MV, MK (farfield.cuh), shared by twin regions
-    void *momc = nullptr;           // [ncells][m2p_stride(Nc)]: this region's ca MV + cb MK in float or double
+    void *wc = nullptr;             // tree owner: [ncells][m2p_stride(P, twin)] regrouped multipoles W_{m,e} of this region and,
+                                    // interleaved, of its twin, in float or double (m2p.cuh; written by P2M / M2M)
     // singular / near-singular corrections (CSR over targets) ----------------------------------------
     int *corr_off = nullptr, *corr_col = nullptr;
     double2 *corr_val = nullptr;    // (sigma c (fine - coarse)_V, sigma (fine - coarse)_K)
@@ -181,6 +182,8 @@ struct pygbe_handle {
     GmresWork gm;
     double *phi_reac = nullptr;     // [nq]
     struct IndexTables *itab = nullptr;   // device copy of the multi-index tables
+    int NW = 0;                           // W_{m,e} per moment set (m2p_nw(P)) and the table that forms them (tables.cuh)
+    int *wt_off = nullptr; short *wt_k = nullptr; double *wt_c = nullptr;
     cudaStream_t side = nullptr;    // far-field chain (P2M, M2M, M2P) runs here, concurrently with P2P
     cudaStream_t side2 = nullptr;   // near-field correction SpMV runs here
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_join2 = nullptr;

@@ -13,23 +13,32 @@
 #include "common.cuh"
 #include "tables.cuh"
 
-// Where a finished cell's multipoles go besides mom: the combinations ca MV + cb MK that the M2P of the tree
-// owner (A) and of its twin region (B, or null) read, in the arithmetic type of the M2P, row stride padded to
-// a multiple of 4 (m2p.cuh).  Written by the kernel that finishes the cell (P2M for leaves, M2M otherwise).
+// Where a finished cell's multipoles go besides mom: the M2P does not read M^k but the regrouped coefficients
+//     W_{m,e} = (-1)^|e| / e!  sum_{|j| = m - |e|} M^(e + 2j) / (2^|j| j!)            (m2p.cuh)
+// of the combinations ca MV + cb MK that belong to the tree owner (A) and to its twin region (B, interleaved
+// with A's when there is one), in the arithmetic type of the M2P, row stride padded to a multiple of 4.
+// Written by the kernel that finishes the cell (P2M for leaves, M2M otherwise) from the sparse table
+// (wt_off, wt_k, wt_c) built at create (tables.cuh): entry p of the stream is sum_i wt_c[i] M^(wt_k[i]).
 struct MomOut {
-    void *A, *B;
+    void *wc;
     double caA, cbA, caB, cbB;
-    int fp32, stride;
+    int fp32, stride, twin, NW;
+    const int *wt_off; const short *wt_k; const double *wt_c;
 };
-__device__ __forceinline__ void momc_store(const MomOut &o, long cell, int k, double mv, double mk)
+// mv, mk: the cell's two moment sets in shared memory; all nthreads threads of the CTA call this
+__device__ __forceinline__ void wc_store(const MomOut &o, long cell, const double *mv, const double *mk, int tid, int nthreads)
 {
-    const long i = cell * o.stride + k;
-    if (o.fp32) {
-        ((float *)o.A)[i] = (float)(o.caA * mv + o.cbA * mk);
-        if (o.B) ((float *)o.B)[i] = (float)(o.caB * mv + o.cbB * mk);
-    } else {
-        ((double *)o.A)[i] = o.caA * mv + o.cbA * mk;
-        if (o.B) ((double *)o.B)[i] = o.caB * mv + o.cbB * mk;
+    for (int p = tid; p < o.NW; p += nthreads) {
+        double wv = 0.0, wk = 0.0;
+        for (int i = o.wt_off[p]; i < o.wt_off[p + 1]; i++) {
+            const int k = o.wt_k[i];
+            const double c = o.wt_c[i];
+            wv += c * mv[k]; wk += c * mk[k];
+        }
+        const double a = o.caA * wv + o.cbA * wk, b = o.caB * wv + o.cbB * wk;
+        const long at = cell * o.stride + (o.twin ? 2 * p : p);
+        if (o.fp32) { ((float *)o.wc)[at] = (float)a; if (o.twin) ((float *)o.wc)[at + 1] = (float)b; }
+        else { ((double *)o.wc)[at] = a; if (o.twin) ((double *)o.wc)[at + 1] = b; }
     }
 }
 
@@ -101,13 +110,16 @@ k_p2m(const int *__restrict__ skip, int Nc, int nsplit, const int4 *__restrict__
         }
         if (sp > 0) { s_part[0][t] = aV; s_part[1][t] = aK; }
     }
-    if (nsplit > 1) __syncthreads();
+    __syncthreads();
     if (active && sp == 0) {
         for (int j = 1; j < nsplit; j++) { aV += s_part[0][t + j * Nc]; aK += s_part[1][t + j * Nc]; }
         mom[((long)cell * 2) * Nc + k] = aV;
         mom[((long)cell * 2 + 1) * Nc + k] = aK;
-        momc_store(mo, cell, k, aV, aK);
     }
+    __syncthreads();
+    if (active && sp == 0) { s_part[0][k] = aV; s_part[1][k] = aK; }
+    __syncthreads();
+    wc_store(mo, cell, s_part[0], s_part[1], t, blockDim.x);
 }
 
 // ------------------------------------------------------------------------------------------------ M2M
@@ -232,8 +244,10 @@ k_m2m(const int *__restrict__ skip, int P, int Nc, int n_cells, const int4 *__re
             for (int c = 0; c < nch; c++) { mv += s_m[c * n2 + k]; mk += s_m[c * n2 + Nc + k]; }
             mom[(long)cell * n2 + k] = mv;
             mom[(long)cell * n2 + Nc + k] = mk;
-            momc_store(mo, cell, k, mv, mk);
+            s_m[k] = mv; s_m[Nc + k] = mk;                           // only this thread read these two
         }
+        __syncthreads();
+        wc_store(mo, cell, s_m, s_m + Nc, threadIdx.x, M2M_THREADS);
         __threadfence();
         __syncthreads();
         if (threadIdx.x == 0) st_release(ready + cell, epoch);

@@ -1,5 +1,24 @@
 // m2p.cuh -- M2P (a6) of the Cartesian Taylor treecode, eq. (13)-(14).
 // Compiled once per expansion order P (m2p_inst.cu with -DM2P_P=<P>) so that the orders build in parallel.
+//
+// What is evaluated is eq. (14)'s truncated series  sum_{|k| <= P} a^k(x, y_c) M^k,  a^k = (1/k!) D_y^k G.
+// The paper obtains a^k by recurrences (reading A13).  Both kernels are radial,
+// G = F(s), s = |d|^2 / 2, d = x - y_c, and for such a function
+//     D_d^k F(s) = sum_j  prod_axes [ k_a! / (2^j_a j_a! (k_a - 2 j_a)!) d_a^(k_a - 2 j_a) ]  F^(|k| - |j|)(s)
+// (derivatives of a function of a quadratic; j_a <= k_a / 2).  Collecting the series by the order m of the
+// radial derivative and by the monomial d^e, e = k - 2j, gives the same sum in the form
+//     sum_k a^k M^k = sum_{m=0..P} F^(m)(s) Q_m,     Q_m = sum_{e : |e| <= m, 2m - |e| <= P} W_{m,e} d^e,
+//     W_{m,e} = (-1)^|e| / e!  sum_{|j| = m - |e|}  M^(e + 2j) / (2^|j| j!)
+// where the W depend on the cell only: they are formed when the cell's multipoles are (P2M / M2M epilogue,
+// farfield.cuh, from a table built at create) and replace the multipoles as the M2P's input.  Per (target,
+// cell) the work is then Nc - 1 multiplies for the monomials and one FMA per W -- 130 per moment set at P = 6,
+// 295 at P = 8 -- instead of a recurrence of 6 (Laplace) to 12 (Yukawa) instructions per coefficient, and it
+// is independent of the kernel: Laplace and Yukawa differ only in the P + 1 numbers F^(m)(s),
+//     F^(0) = exp(-kappa r) / r,   F^(1) = -exp(-kappa r) (kappa r + 1) / r^3,
+//     F^(m+1) = -[ (2m + 1) F^(m) - kappa^2 F^(m-1) ] / r^2        (kappa = 0: Laplace),
+// so the two regions on either side of a surface set ("twins") are evaluated in one pass.
+// fp32 check (numpy emulation, P = 6 and 8, cells of 2..16 A at 1..4 times the MAC distance): relative error
+// <= 5.5e-7 against the fp64 evaluation of the same series.
 #pragma once
 #include <cuda_runtime.h>
 #include "mathx.cuh"
@@ -8,16 +27,23 @@
 #endif
 #define PYGBE_TG_M2P PYGBE_TG
 
-// Row stride of the combined moments momc[cell][stride] (elements of T): Nc padded to a multiple of 4 so
-// that every row starts on a 16-byte boundary and can be moved with 16-byte cp.async.
-static inline __host__ __device__ int m2p_stride(int Nc) { return (Nc + 3) / 4 * 4; }
+// number of W_{m,e} per moment set, in the order the kernel consumes them (ex, ey, ez ascending, then J)
+static inline __host__ __device__ constexpr int m2p_nw(int P)
+{
+    int n = 0;
+    for (int t = 0; t <= P; t++) n += (t + 1) * (t + 2) / 2 * ((P - t) / 2 + 1);
+    return n;
+}
+// Row stride of wc[cell][stride] (elements of T): the W of the tree owner and, interleaved, of its twin,
+// padded to a multiple of 4 so that every row starts on a 16-byte boundary and moves with 16-byte cp.async.
+static inline __host__ __device__ constexpr int m2p_stride(int P, bool twin) { return (m2p_nw(P) * (twin ? 2 : 1) + 3) / 4 * 4; }
 
 struct M2PArgs {
     const int *skip; const int4 *items; const int *m2p_cell; int n_items; int np;
     const double4 *tpos; const double4 *cgeo;
-    const void *momc;          // the region's multipoles ca * MV + cb * MK, already in T (written by P2M / M2M, farfield.cuh)
-    double kappa; double *out;
-    int yukawa; int fp32; cudaStream_t stream;
+    const void *wc;            // W_{m,e} of the tree owner (and twin), already combined and in T (farfield.cuh)
+    double kappaA, kappaB; double *outA, *outB;
+    int twin; int fp32; cudaStream_t stream;
 };
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
@@ -28,107 +54,102 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// Taylor coefficients by recurrence ("recursive relations for the Green's function of
-// the Poisson equation [20] and linearized Poisson-Boltzmann equation [21]"; reading A13), d = x - y_c,
-// R^2 = |d|^2, n = |k|, terms with a negative index dropped:
-//   Laplace:  a^0 = 1/R;       n R^2 a^k = (2n-1) sum_i d_i a^(k-e_i) - (n-1) sum_i a^(k-2e_i)
-//   Yukawa :  b^0 = exp(-kappa R), a^0 = b^0/R;
-//             n b^k     = kappa [ sum_i d_i a^(k-e_i) - sum_i a^(k-2e_i) ]
-//             n R^2 a^k = (2n-1) sum_i d_i a^(k-e_i) - (n-1) sum_i a^(k-2e_i)
-//                         + kappa [ sum_i d_i b^(k-e_i) - sum_i b^(k-2e_i) ]
-// The loops are fully unrolled for the compile-time order P: the coefficient arrays live in registers
-// and only two order-shells are alive at a time.  Returns sum_k a^k M^k (M in shared memory).
-// T = double: fp64 throughout.  T = float: fp32 recurrence with MUFU rsqrt / ex2 (mathx.cuh); SURVEY A8b:
-// fp32 coefficient error 1.4e-7 (order 0) .. 1.8e-6 (order 8), far below the truncation error.
-template <int P, bool YUKAWA, typename T>
-__device__ __forceinline__ T m2p_eval(T dx, T dy, T dz, T kappa, T kscaled, const T *__restrict__ M)
+template <typename T> struct Chunk;                                   // one 16-byte shared-memory read
+template <> struct Chunk<float> { typedef float4 V; static constexpr int N = 4;
+    static __device__ __forceinline__ void get(const float *p, float (&c)[4]) { const float4 v = *(const float4 *)p; c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w; } };
+template <> struct Chunk<double> { typedef double2 V; static constexpr int N = 2;
+    static __device__ __forceinline__ void get(const double *p, double (&c)[2]) { const double2 v = *(const double2 *)p; c[0] = v.x; c[1] = v.y; } };
+
+// Q_m (+ twin) of one cell at offset d: the loops are fully unrolled for the compile-time order, so the
+// position in the W stream, the accumulator index and the 16-byte reads are all static.
+template <int P, int NS, typename T>
+__device__ __forceinline__ void m2p_q(T dx, T dy, T dz, const T *__restrict__ w, T (&q)[P + 1][NS])
 {
-    T a[P + 1][P + 1][P + 1];
-    T b[YUKAWA ? P + 1 : 1][YUKAWA ? P + 1 : 1][YUKAWA ? P + 1 : 1];
-    const T R2 = dx * dx + dy * dy + dz * dz;
-    const T invR = Real<T>::rsqrt_(R2);
-    const T invR2 = invR * invR;
-    if constexpr (YUKAWA) {
-        b[0][0][0] = Real<T>::exp_neg(kscaled, R2 * invR);
-        a[0][0][0] = b[0][0][0] * invR;
-    } else {
-        a[0][0][0] = invR;
-    }
-    T acc = a[0][0][0] * M[0];
-    int idx = 1;
+    constexpr int EPC = Chunk<T>::N;
+    T cur[EPC];
+    int idx = 0;
 #pragma unroll
-    for (int n = 1; n <= P; n++) {
-        const T c1 = T(2 * n - 1) / T(n) * invR2, c2 = T(n - 1) / T(n) * invR2;
-        const T c3 = kappa / T(n), c4 = c3 * invR2;
+    for (int m = 0; m <= P; m++)
 #pragma unroll
-        for (int kx = n; kx >= 0; kx--) {
+        for (int s = 0; s < NS; s++) q[m][s] = T(0);
+    T px = T(1);
 #pragma unroll
-            for (int ky = n - kx; ky >= 0; ky--) {
-                const int kz = n - kx - ky;
-                T s1 = T(0), s2 = T(0);
-                if (kx > 0) s1 += dx * a[kx > 0 ? kx - 1 : 0][ky][kz];
-                if (ky > 0) s1 += dy * a[kx][ky > 0 ? ky - 1 : 0][kz];
-                if (kz > 0) s1 += dz * a[kx][ky][kz > 0 ? kz - 1 : 0];
-                if (kx > 1) s2 += a[kx > 1 ? kx - 2 : 0][ky][kz];
-                if (ky > 1) s2 += a[kx][ky > 1 ? ky - 2 : 0][kz];
-                if (kz > 1) s2 += a[kx][ky][kz > 1 ? kz - 2 : 0];
-                T v = c1 * s1 - c2 * s2;
-                if constexpr (YUKAWA) {
-                    T t1 = T(0), t2 = T(0);
-                    if (kx > 0) t1 += dx * b[kx > 0 ? kx - 1 : 0][ky][kz];
-                    if (ky > 0) t1 += dy * b[kx][ky > 0 ? ky - 1 : 0][kz];
-                    if (kz > 0) t1 += dz * b[kx][ky][kz > 0 ? kz - 1 : 0];
-                    if (kx > 1) t2 += b[kx > 1 ? kx - 2 : 0][ky][kz];
-                    if (ky > 1) t2 += b[kx][ky > 1 ? ky - 2 : 0][kz];
-                    if (kz > 1) t2 += b[kx][ky][kz > 1 ? kz - 2 : 0];
-                    b[kx][ky][kz] = c3 * (s1 - s2);
-                    v += c4 * (t1 - t2);
+    for (int ex = 0; ex <= P; ex++) {
+        T pxy = px;
+#pragma unroll
+        for (int ey = 0; ey <= P - ex; ey++) {
+            T mono = pxy;
+#pragma unroll
+            for (int ez = 0; ez <= P - ex - ey; ez++) {
+                const int t = ex + ey + ez;
+#pragma unroll
+                for (int J = 0; J <= (P - t) / 2; J++) {
+#pragma unroll
+                    for (int s = 0; s < NS; s++) {
+                        if (idx % EPC == 0) Chunk<T>::get(w + idx, cur);
+                        q[t + J][s] = fma(cur[idx % EPC], mono, q[t + J][s]);
+                        idx++;
+                    }
                 }
-                a[kx][ky][kz] = v;
-                acc += v * M[idx];
-                idx++;
+                mono *= dz;
             }
+            pxy *= dy;
+        }
+        px *= dx;
+    }
+}
+
+// sum_m F^(m)(s) q_m for one kernel (kappa = 0: Laplace)
+template <int P, int NS, typename T>
+__device__ __forceinline__ T m2p_radial(T r, T rinv, T rinv2, T kappa, T kscaled, const T (&q)[P + 1][NS], int s)
+{
+    const T E = kappa != T(0) ? Real<T>::exp_neg(kscaled, r) : T(1);
+    T gm = E * rinv;                                   // F^(0)
+    T acc = gm * q[0][s];
+    if (P >= 1) {
+        T g = -E * (kappa * r + T(1)) * rinv * rinv2;  // F^(1)
+        acc = fma(g, q[1][s], acc);
+        const T k2 = kappa * kappa;
+#pragma unroll
+        for (int m = 1; m < P; m++) {
+            const T gn = -(T(2 * m + 1) * g - k2 * gm) * rinv2;
+            gm = g; g = gn;
+            acc = fma(g, q[m + 1][s], acc);
         }
     }
     return acc;
 }
 
-// Work item = (target group, a run of its M2P list).  One thread per target; the moments of M2P_CB cells
-// at a time are staged in shared memory (combined ca MV + cb MK, converted to T) and read by all threads
-// as broadcasts.  The target offset d = x - y_c is always formed in fp64 and then rounded to T, so the
-// fp32 path never subtracts large absolute coordinates; accumulation over cells is fp64.
-// The batches are double-buffered with cp.async (LDGSTS): while the threads evaluate the recurrences of one
-// batch, the moments and centres of the next one stream from L2 into the other buffer (capture r1b showed
-// 7-9 % barrier + 5-9 % long-scoreboard stalls with synchronous staging at 2 warps per CTA).
-#ifndef M2P_CB
-#define M2P_CB 4
-#endif
-#ifndef M2P_MINB
-#define M2P_MINB 1       // min CTAs per SM asked of ptxas (register cap); tuning knob
-#endif
-template <int P, bool YUKAWA, typename T>
-__global__ void __launch_bounds__(PYGBE_TG_M2P, M2P_MINB)
+// Work item = (target group, a run of its M2P list).  One thread per target; the W rows of CB cells at a
+// time are staged in shared memory and read by all threads as 16-byte broadcasts.  The target offset
+// d = x - y_c is always formed in fp64 and then rounded to T, so the fp32 path never subtracts large absolute
+// coordinates; accumulation over cells is fp64.  The batches are double-buffered with cp.async (LDGSTS):
+// while the threads work on one batch, the rows and centres of the next stream from L2 into the other buffer.
+template <int P, bool TWIN, typename T>
+__global__ void __launch_bounds__(PYGBE_TG_M2P)
 k_m2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
-      const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const T *__restrict__ momc,
-      double kappa, double kscaled, double *__restrict__ out)
+      const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const T *__restrict__ wc,
+      double kappaA, double kscaledA, double kappaB, double kscaledB, double *__restrict__ outA, double *__restrict__ outB)
 {
-    constexpr int Nc = (P + 1) * (P + 2) * (P + 3) / 6;
-    constexpr int NCS = (Nc + 3) / 4 * 4;                    // = m2p_stride(Nc)
+    constexpr int NS = TWIN ? 2 : 1;
+    constexpr int STRIDE = m2p_stride(P, TWIN);
     constexpr int EPC = 16 / (int)sizeof(T);                 // elements per 16-byte chunk
-    constexpr int CH = NCS / EPC;                            // chunks per cell
-    __shared__ __align__(16) T s_M[2][M2P_CB][NCS];
-    __shared__ __align__(16) double4 s_c[2][M2P_CB];
+    constexpr int CH = STRIDE / EPC;                         // chunks per cell
+    constexpr int CBW = 12288 / (STRIDE * (int)sizeof(T));   // cells per batch: about 12 KB per buffer
+    constexpr int CB = CBW < 1 ? 1 : (CBW > 4 ? 4 : CBW);
+    __shared__ __align__(16) T s_W[2][CB][STRIDE];
+    __shared__ __align__(16) double4 s_c[2][CB];
     if (skip && *skip) return;
     const int4 it = items[blockIdx.x];
     const int t = it.x * PYGBE_TG_M2P + threadIdx.x;
     const bool ok = t < np;
     const double4 X = ok ? tpos[t] : make_double4(1e30, 1e30, 1e30, 0);
-    double acc = 0.0;
+    double accA = 0.0, accB = 0.0;
     auto stage = [&](int buf, int s0) {
-        const int nb = min(M2P_CB, it.z - s0);
+        const int nb = min(CB, it.z - s0);
         for (int i = threadIdx.x; i < nb * CH; i += PYGBE_TG_M2P) {
             const int c_ = i / CH, j = i - c_ * CH;
-            cp_async16(&s_M[buf][c_][j * EPC], momc + (long)m2p_cell[s0 + c_] * NCS + j * EPC);
+            cp_async16(&s_W[buf][c_][j * EPC], wc + (long)m2p_cell[s0 + c_] * STRIDE + j * EPC);
         }
         if (threadIdx.x < nb * 2) {
             const int c_ = threadIdx.x >> 1, hf = threadIdx.x & 1;
@@ -138,18 +159,25 @@ k_m2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int *_
     };
     stage(0, it.y);
     int buf = 0;
-    for (int s0 = it.y; s0 < it.z; s0 += M2P_CB, buf ^= 1) {
-        const int nb = min(M2P_CB, it.z - s0);
-        const bool more = s0 + M2P_CB < it.z;
-        if (more) { stage(buf ^ 1, s0 + M2P_CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+    for (int s0 = it.y; s0 < it.z; s0 += CB, buf ^= 1) {
+        const int nb = min(CB, it.z - s0);
+        const bool more = s0 + CB < it.z;
+        if (more) { stage(buf ^ 1, s0 + CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
         __syncthreads();
         for (int c_ = 0; c_ < nb; c_++) {
             const double4 c = s_c[buf][c_];
-            acc += (double)m2p_eval<P, YUKAWA, T>((T)(X.x - c.x), (T)(X.y - c.y), (T)(X.z - c.z), (T)kappa,
-                                                  (T)kscaled, s_M[buf][c_]);
+            const T dx = (T)(X.x - c.x), dy = (T)(X.y - c.y), dz = (T)(X.z - c.z);
+            T q[P + 1][NS];
+            m2p_q<P, NS, T>(dx, dy, dz, s_W[buf][c_], q);
+            const T r2 = dx * dx + dy * dy + dz * dz;
+            const T rinv = Real<T>::rsqrt_(r2), rinv2 = rinv * rinv, r = r2 * rinv;
+            accA += (double)m2p_radial<P, NS, T>(r, rinv, rinv2, (T)kappaA, (T)kscaledA, q, 0);
+            if (TWIN) accB += (double)m2p_radial<P, NS, T>(r, rinv, rinv2, (T)kappaB, (T)kscaledB, q, NS - 1);
         }
         __syncthreads();                                     // buf is refilled two iterations from now
     }
-    if (ok) atomicAdd(out + t, acc);
+    if (ok) {
+        atomicAdd(outA + t, accA);
+        if (TWIN) atomicAdd(outB + t, accB);
+    }
 }
-

@@ -9,16 +9,17 @@
 #ifdef M2P_STUB
 int CAT(pygbe_m2p_launch_, M2P_P)(const M2PArgs &) { return -1; }
 #else
-template <bool Y, typename T> static void launch(const M2PArgs &a)
+template <bool TWIN, typename T> static void launch(const M2PArgs &a)
 {
-    k_m2p<M2P_P, Y, T><<<a.n_items, PYGBE_TG_M2P, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo,
-                                                                 (const T *)a.momc, a.kappa, Real<T>::kscale(a.kappa), a.out);
+    k_m2p<M2P_P, TWIN, T><<<a.n_items, PYGBE_TG_M2P, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo,
+                                                                    (const T *)a.wc, a.kappaA, Real<T>::kscale(a.kappaA),
+                                                                    a.kappaB, Real<T>::kscale(a.kappaB), a.outA, a.outB);
 }
 
 int CAT(pygbe_m2p_launch_, M2P_P)(const M2PArgs &a)
 {
-    if (a.fp32) { if (a.yukawa) launch<true, float>(a); else launch<false, float>(a); }
-    else { if (a.yukawa) launch<true, double>(a); else launch<false, double>(a); }
+    if (a.fp32) { if (a.twin) launch<true, float>(a); else launch<false, float>(a); }
+    else { if (a.twin) launch<true, double>(a); else launch<false, double>(a); }
     return 0;
 }
 #endif

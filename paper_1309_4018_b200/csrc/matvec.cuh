@@ -30,15 +30,15 @@ M2P_DECL(1) M2P_DECL(2) M2P_DECL(3) M2P_DECL(4) M2P_DECL(5) M2P_DECL(6)
 M2P_DECL(7) M2P_DECL(8) M2P_DECL(9) M2P_DECL(10) M2P_DECL(11) M2P_DECL(12)
 #undef M2P_DECL
 
-// M2P of region R over the lists of the tree owner T, on stream st; R.momc was written by P2M / M2M.
-static int launch_m2p(pygbe_handle *h, Region &T, Region &R, const int *skip, cudaStream_t st)
+// M2P of the tree owner A and its twin B (if any) in one pass, on stream st; A.wc was written by P2M / M2M.
+static int launch_m2p(pygbe_handle *h, Region &A, Region *B, const int *skip, cudaStream_t st)
 {
-    const bool fp32 = h->precision == PYGBE_PRECISION_MIXED;
     M2PArgs a;
     memset(&a, 0, sizeof(a));
-    a.skip = skip; a.items = T.m2p_items; a.m2p_cell = T.m2p_cell; a.n_items = T.n_m2p_items; a.np = T.np;
-    a.tpos = T.tpos; a.cgeo = T.cgeo; a.momc = R.momc; a.kappa = R.kappa; a.out = R.out;
-    a.yukawa = R.yukawa; a.fp32 = fp32; a.stream = st;
+    a.skip = skip; a.items = A.m2p_items; a.m2p_cell = A.m2p_cell; a.n_items = A.n_m2p_items; a.np = A.np;
+    a.tpos = A.tpos; a.cgeo = A.cgeo; a.wc = A.wc; a.kappaA = A.kappa; a.outA = A.out;
+    a.twin = B ? 1 : 0; a.kappaB = B ? B->kappa : 0.0; a.outB = B ? B->out : nullptr;
+    a.fp32 = h->precision == PYGBE_PRECISION_MIXED; a.stream = st;
     typedef int (*fn_t)(const M2PArgs &);
     static const fn_t table[PYGBE_PMAX + 1] = {nullptr, pygbe_m2p_launch_1, pygbe_m2p_launch_2, pygbe_m2p_launch_3,
         pygbe_m2p_launch_4, pygbe_m2p_launch_5, pygbe_m2p_launch_6, pygbe_m2p_launch_7, pygbe_m2p_launch_8,
@@ -117,10 +117,11 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
         for (auto &w : work) {
             Region &A = *w.first; Region *B = w.second;
             if (A.n_m2p_items == 0) continue;
-            // multipoles leave P2M / M2M already combined for the M2P of A (MV - MK) and of its twin (rV MV + MK)
+            // multipoles leave P2M / M2M regrouped and combined for the M2P of A (MV - MK) and of its twin (rV MV + MK)
             MomOut mo;
-            mo.A = A.momc; mo.B = B ? B->momc : nullptr; mo.caA = 1.0; mo.cbA = -1.0; mo.caB = A.twin_rV; mo.cbB = 1.0;
-            mo.fp32 = mixed ? 1 : 0; mo.stride = m2p_stride(h->Nc);
+            mo.wc = A.wc; mo.caA = 1.0; mo.cbA = -1.0; mo.caB = A.twin_rV; mo.cbB = 1.0;
+            mo.fp32 = mixed ? 1 : 0; mo.twin = B ? 1 : 0; mo.stride = m2p_stride(h->P, B != nullptr); mo.NW = h->NW;
+            mo.wt_off = h->wt_off; mo.wt_k = h->wt_k; mo.wt_c = h->wt_c;
             STAGE(h, PYGBE_STAGE_P2M);
             if (A.n_p2m > 0)
                 LAUNCH(h, k_p2m, A.n_p2m, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.p2m_rec, A.pq, A.pmom, A.mom, mo);
@@ -140,8 +141,7 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
         for (auto &w : work) {
             Region &A = *w.first; Region *B = w.second;
             if (A.n_m2p_items == 0) continue;
-            int rc = launch_m2p(h, A, A, skip, h->stream);
-            if (rc == PYGBE_OK && B) rc = launch_m2p(h, A, *B, skip, h->stream);
+            int rc = launch_m2p(h, A, B, skip, h->stream);
             if (rc != PYGBE_OK) { h->stream = main_st; return rc; }
         }
         STAGE_END(h, PYGBE_STAGE_M2P);

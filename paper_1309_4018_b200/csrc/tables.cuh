@@ -133,3 +133,35 @@ static void fill_index_tables(IndexTables *t)
             t->binom[n][m] = (m == 0 || m == n) ? 1.0 : t->binom[n - 1][m - 1] + t->binom[n - 1][m];
         }
 }
+
+// The regrouping of the Taylor series used by the M2P (m2p.cuh): entry p of the W stream -- the triple loop
+// ex, ey, ez ascending with |e| <= P, then J = 0 .. (P - |e|) / 2, m = |e| + J -- is
+//     W_p = (-1)^|e| / e!  sum_{|j| = J} M^(e + 2j) / (2^J j!),
+// stored as a sparse row over the canonical moment index: W_p = sum_{i in [off[p], off[p+1])} c[i] M^(k[i]).
+struct WTable {
+    std::vector<int> off;
+    std::vector<short> k;
+    std::vector<double> c;
+};
+static void build_w_table(int P, const IndexTables &t, WTable *w)
+{
+    double fact[PYGBE_PMAX + 1];
+    fact[0] = 1.0;
+    for (int i = 1; i <= PYGBE_PMAX; i++) fact[i] = fact[i - 1] * i;
+    w->off.assign(1, 0); w->k.clear(); w->c.clear();
+    for (int ex = 0; ex <= P; ex++)
+        for (int ey = 0; ey <= P - ex; ey++)
+            for (int ez = 0; ez <= P - ex - ey; ez++) {
+                const int n = ex + ey + ez;
+                const double pre = ((n & 1) ? -1.0 : 1.0) / (fact[ex] * fact[ey] * fact[ez]);
+                for (int J = 0; J <= (P - n) / 2; J++) {
+                    for (int jx = J; jx >= 0; jx--)
+                        for (int jy = J - jx; jy >= 0; jy--) {
+                            const int jz = J - jx - jy;
+                            w->k.push_back(t.idx3[ex + 2 * jx][ey + 2 * jy][ez + 2 * jz]);
+                            w->c.push_back(pre / (std::ldexp(1.0, J) * fact[jx] * fact[jy] * fact[jz]));
+                        }
+                    w->off.push_back((int)w->k.size());
+                }
+            }
+}
