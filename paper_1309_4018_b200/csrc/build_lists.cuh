@@ -96,9 +96,10 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     TRY(h->mem.alloc(&d_mcnt, R.ng)); TRY(h->mem.alloc(&d_pcnt, R.ng)); TRY(h->mem.alloc(&d_over, 1));
     CUDA_TRY(cudaMemsetAsync(d_over, 0, sizeof(int), h->stream));
     const double near_dist = h->thres > 0 ? h->thres * R.Lmax : 0.0;
-    // break-even between one Taylor evaluation and the direct sum over a leaf's points, from the SASS
-    // instruction counts (profiles/r1b_mixed_path.md): ~50 points in fp32, ~18 in fp64 at P = 6 (Nc = 84)
-    const int small_leaf = (int)((mixed ? 50.0 : 18.0) * h->Nc / 84.0 / K);
+    // break-even between one Taylor evaluation and the direct sum over a leaf's points: a regrouped M2P
+    // evaluation costs Nc - 1 + NW FMA-pipe instructions per region, a P2P pair ~14 per region, and the sweep of
+    // profiles/r2a_upward.md puts the optimum at ~16 points for P = 6 (344 instructions) in both precisions
+    const int small_leaf = (int)(16.0 * (h->Nc + 2.0 * h->NW) / 344.0 / K);
     LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.ggeo, R.cgeo, R.crange, R.cchild,
            h->theta, near_dist, small_leaf, 0, d_mcnt, d_pcnt, nullptr, nullptr, nullptr, nullptr, d_over);
     std::vector<int> mcnt, pcnt;
