@@ -47,21 +47,24 @@ def make_problem(name):
 
 
 # ------------------------------------------------------------------------------------------ flop model
+def m2p_nw(P):
+    """W_{m,e} per moment set of the regrouped Taylor series (m2p.cuh): 130 at P = 6, 295 at P = 8."""
+    return sum((t + 1) * (t + 2) // 2 * ((P - t) // 2 + 1) for t in range(P + 1))
+
+
 def m2p_flops(P, yukawa):
-    """Algorithmic flops of one (target, cell) Taylor evaluation: the recurrence of reading A13 term by
-    term (multiply-add = 2) plus the contraction with the moments.  DESIGN.md 'Flop model'."""
-    f = 3 + 5 + 2 + (3 if yukawa else 0) + 1          # d, R^2, 1/R^2 & 1/R, [exp, kR, *], a0*M0
-    for n in range(1, P + 1):
-        f += 4 if not yukawa else 6                    # c1..c4
-        for kx in range(n, -1, -1):
-            for ky in range(n - kx, -1, -1):
-                kz = n - kx - ky
-                n1 = sum(1 for k in (kx, ky, kz) if k > 0)
-                n2 = sum(1 for k in (kx, ky, kz) if k > 1)
-                s = (2 * n1 - 1) + max(n2 - 1, 0)      # s1 (mul+add chain), s2 (adds)
-                f += s + 3 + 2                         # v = c1 s1 - c2 s2 ; acc += v M
-                if yukawa:
-                    f += s + 2 + 3                     # t1, t2 ; b = c3 (s1 - s2) ; v += c4 (t1 - t2)
+    """Algorithmic flops of one (target, cell) Taylor evaluation as the kernel does it (m2p.cuh; multiply-add
+    = 2, rsqrt = exp = 1): offset and radius, the Nc - 1 monomials d^e, one FMA per W_{m,e} for every region
+    in `yukawa` (a tuple of booleans: one entry, or two for twin regions evaluated in one pass), and per
+    region the P + 1 radial derivatives F^(m) and their dot product with Q_m.  DESIGN.md 'Flop model'."""
+    if isinstance(yukawa, bool):
+        yukawa = (yukawa,)
+    nc = (P + 1) * (P + 2) * (P + 3) // 6
+    f = 3 + 5 + 3 + (nc - 1)                           # d ; r^2 ; 1/r, 1/r^2, r ; monomials
+    for yk in yukawa:
+        f += 2 * m2p_nw(P)                             # Q_m += W d^e
+        f += (2 if yk else 0) + 1 + 5                  # [kappa r, exp] ; F0 ; F1
+        f += 4 * (P - 1) + 2 * (P + 1)                 # F^(m+1) recurrence ; sum_m F^(m) Q_m
     return f
 
 
@@ -270,7 +273,8 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
         if dom == "p2p":
             flops = st["p2p_pairs"] / nreg * (P2P_FLOPS_FUSED if nreg == 2 else sum(P2P_FLOPS[yk] for yk in yuk))
         else:
-            flops = st["m2p_evals"] / nreg * sum(m2p_flops(kw["P"], yk) for yk in yuk)
+            # twin regions share one fused evaluation per (target, cell); otherwise one evaluation per region
+            flops = st["m2p_evals"] / nreg * (m2p_flops(kw["P"], tuple(yuk)) if nreg == 2 else sum(m2p_flops(kw["P"], yk) for yk in yuk))
         peaks = pg.alu_peaks(local)
         mp = {}
         try:
@@ -284,7 +288,7 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
         # dram__bytes_read.sum + dram__bytes_write.sum of the stage's launches from the ncu --set full capture of this
         # command (profiles/r1b_mixed_path.md, config kirkwood_l5): bytes per matvec, both regions; else null
         traffic = {("kirkwood_l5", "f32", "m2p"): 1.50e6 + 1.51e6, ("kirkwood_l5", "f32", "p2p"): 3.86e6}.get((args.config, dt, dom))
-        kname = {"m2p": "k_m2p<%d,*,%s> x %d regions (+ k_mom_combine)" % (kw["P"], "float" if dt == "f32" else "double", nreg),
+        kname = {"m2p": "k_m2p<%d,%s,%s>" % (kw["P"], "twin regions fused" if nreg == 2 else "per tree", "float" if dt == "f32" else "double"),
                  "p2p": "k_p2p<%s,%s>" % ("float" if dt == "f32" else "double", "twin regions fused" if nreg == 2 else "per region")}[dom]
         roofline = {"bound": "alu", "kernel": "%s, %d launches/matvec" % (kname, round(nreg_launch[dom])),
                     "achieved": achieved, "peak": nominal[dt], "unit": "TFLOP/s", "frac": achieved / nominal[dt],

@@ -182,6 +182,8 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     // M2P CTAs keep only 8-16 warps per SM resident (72-127 registers): finer items even out the tail
     int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[R.ng] / (3 * want_items)));
     m2p_item = (m2p_item + 3) / 4 * 4;
+    // P2P items are runs of source tiles: (first point, points <= P2P_TILE, anchor cell, 0), whole panels only
+    const int tile_panels = std::max(1, P2P_TILE / K);
     std::vector<int4> sub, pitems, mitems;
     for (int g = 0; g < R.ng; g++) {
         int first = (int)sub.size(), acc = 0;
@@ -189,7 +191,10 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
             int a = prng[r].x;
             while (a < prng[r].y) {
                 int take = std::min(prng[r].y - a, p2p_item - acc);
-                sub.push_back(make_int4(a, a + take, prng[r].z, 0));
+                for (int b = a; b < a + take; b += tile_panels) {
+                    const int nb = std::min(tile_panels, a + take - b);
+                    sub.push_back(make_int4(b * K, nb * K, prng[r].z, 0));
+                }
                 a += take; acc += take;
                 if (acc == p2p_item) { pitems.push_back(make_int4(g, first, (int)sub.size(), 0)); first = (int)sub.size(); acc = 0; }
             }

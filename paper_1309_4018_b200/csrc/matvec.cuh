@@ -59,7 +59,7 @@ static void launch_p2p(pygbe_handle *h, Region &A, Region *B, const int *skip)
     double *oA = A.out, *oB = B ? B->out : nullptr;
 #define P2P_GO(YA, TW, YB)                                                                                     \
     do { auto kern = k_p2p<T, YA, TW, YB>;                                                                     \
-    LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, h->K, A.np, A.tpos,              \
+    LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, A.np, A.tpos,              \
            A.cgeo, pos, chg, kA, kB, rV, oA, oB); } while (0)
     if (!B) { if (A.yukawa) P2P_GO(true, false, false); else P2P_GO(false, false, false); }
     else if (A.yukawa) { if (B->yukawa) P2P_GO(true, true, true); else P2P_GO(true, true, false); }

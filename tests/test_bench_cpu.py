@@ -20,13 +20,15 @@ def _free_port():
 
 def test_whole_job_value_and_flop_model():
     assert bench.whole_job_value(4, 1000, 10, 2.0) == 20000.0
-    # P = 0 limit of the recurrence count: geometry + one product; more terms with order; Yukawa > Laplace
+    # regrouped Taylor series (m2p.cuh): W_{m,e} counts, more terms with order, Yukawa = Laplace + exp
+    assert bench.m2p_nw(6) == 130 and bench.m2p_nw(8) == 295 and bench.m2p_nw(0) == 1
     f = [bench.m2p_flops(P, False) for P in (1, 2, 6, 8)]
     assert all(b > a for a, b in zip(f, f[1:]))
-    assert bench.m2p_flops(6, True) > 1.7 * bench.m2p_flops(6, False)
-    # cross-check against the SASS of k_m2p<6,*,float>: 336 FFMA + 76 FMUL + 64 FADD = 812 flops (Laplace),
-    # 614 FFMA + 142 FMUL + 254 FADD = 1624 flops (Yukawa); the model counts a little less (no re-association)
-    assert bench.m2p_flops(6, False) == 732 and bench.m2p_flops(6, True) == 1444
+    assert bench.m2p_flops(6, True) == bench.m2p_flops(6, False) + 2
+    # cross-check against the SASS of k_m2p<6, twin, float> per (target, cell): 276 FFMA + 116 FMUL + 10 FADD
+    # + 3 MUFU = 681 flops; the model counts the fp64 offset subtraction and the unfused radial terms on top
+    assert bench.m2p_flops(6, False) == 394 and bench.m2p_flops(6, (False, True)) == 696
+    assert bench.m2p_flops(6, (False, True)) < bench.m2p_flops(6, False) + bench.m2p_flops(6, True)
     assert bench.P2P_FLOPS_FUSED < bench.P2P_FLOPS[False] + bench.P2P_FLOPS[True]
 
 
