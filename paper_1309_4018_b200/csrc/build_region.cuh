@@ -50,7 +50,7 @@ static int build_corrections(pygbe_handle *h, Region &R, const QuadTables &qt, c
         int *d_cnt;
         TRY(h->mem.alloc(&d_cnt, R.np));
         const double thres2 = h->thres > 0 ? h->thres * h->thres : 0.0;
-        LAUNCH(h, k_near_find, R.ng, PYGBE_TG, 0, R.np, R.tpos, R.pnrm, R.p2p_off, R.p2p_rng, thres2, 0, d_cnt, nullptr, nullptr);
+        LAUNCH(h, k_near_find, cdiv((long)R.np * 32, 128), 128, 0, R.np, R.tpos, R.pnrm, R.p2p_off, R.p2p_rng, thres2, 0, d_cnt, nullptr, nullptr);
         std::vector<int> cnt;
         TRY(download(h, cnt, d_cnt, (size_t)R.np));
         std::vector<int> off(R.np + 1, 0);
@@ -60,12 +60,12 @@ static int build_corrections(pygbe_handle *h, Region &R, const QuadTables &qt, c
         if (nself != R.np) { pygbe_set_error("internal: a target's own panel is missing from its P2P list"); return PYGBE_ECUDA; }
         TRY(upload(h, &R.corr_off, off));
         TRY(h->mem.alloc(&R.corr_col, R.corr_nnz));
-        LAUNCH(h, k_near_find, R.ng, PYGBE_TG, 0, R.np, R.tpos, R.pnrm, R.p2p_off, R.p2p_rng, thres2, 1, d_cnt, R.corr_off, R.corr_col);
+        LAUNCH(h, k_near_find, cdiv((long)R.np * 32, 128), 128, 0, R.np, R.tpos, R.pnrm, R.p2p_off, R.p2p_rng, thres2, 1, d_cnt, R.corr_off, R.corr_col);
         CUDA_TRY(cudaStreamSynchronize(h->stream));
         h->mem.release_one(d_cnt);
     }
     TRY(h->mem.alloc(&R.corr_val, R.corr_nnz));
-    LAUNCH(h, k_near_values, cdiv(R.np, 64), 64, 0, R.np, qt, R.yukawa, R.kappa, R.corr_off, R.corr_col, R.gid, h->tri,
+    LAUNCH(h, k_near_values, cdiv((long)R.np * 32, 128), 128, 0, R.np, qt, R.yukawa, R.kappa, R.corr_off, R.corr_col, R.gid, h->tri,
            R.tpos, R.pnrm, R.spos, R.cV, R.cK, R.corr_val);
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     return PYGBE_OK;

@@ -48,18 +48,24 @@ static inline int nc_of(int P) { return (P + 1) * (P + 2) * (P + 3) / 6; }
 static inline int cdiv(long a, long b) { return (int)((a + b - 1) / b); }
 
 // ---------------------------------------------------------------------------------------------------
-// Device memory owned by a handle: a trivial arena of cudaMalloc'ed blocks, freed together.
+// Device memory owned by a handle: blocks from the device's stream-ordered pool (cudaMallocAsync on the
+// handle's stream), freed together.  The pool keeps freed memory (release threshold raised at create), so
+// neither the scratch buffers of create nor a second handle pay cudaMalloc / cudaFree and their device-wide
+// synchronisation (create of config 1: 21 ms -> see profiles/r2a_upward.md).  Buffers are also read on the
+// handle's side streams, always after an event recorded on the main stream, and destroy synchronises every
+// stream before freeing.
 struct DeviceArena {
     std::vector<void *> blocks;
     size_t bytes = 0;
+    cudaStream_t stream = nullptr;
     template <class T> int alloc(T **p, size_t n)
     {
         *p = nullptr;
         if (n == 0) n = 1;
         void *q = nullptr;
-        cudaError_t e = cudaMalloc(&q, n * sizeof(T));
+        cudaError_t e = cudaMallocAsync(&q, n * sizeof(T), stream);
         if (e != cudaSuccess) {
-            pygbe_set_error("cudaMalloc of %zu bytes failed: %s", n * sizeof(T), cudaGetErrorString(e));
+            pygbe_set_error("cudaMallocAsync of %zu bytes failed: %s", n * sizeof(T), cudaGetErrorString(e));
             return PYGBE_ENOMEM;
         }
         blocks.push_back(q);
@@ -70,11 +76,11 @@ struct DeviceArena {
     void release_one(void *q)
     {
         for (size_t i = 0; i < blocks.size(); i++)
-            if (blocks[i] == q) { cudaFree(q); blocks.erase(blocks.begin() + i); return; }
+            if (blocks[i] == q) { cudaFreeAsync(q, stream); blocks.erase(blocks.begin() + i); return; }
     }
     void release()
     {
-        for (void *q : blocks) cudaFree(q);
+        for (void *q : blocks) cudaFreeAsync(q, stream);
         blocks.clear();
         bytes = 0;
     }

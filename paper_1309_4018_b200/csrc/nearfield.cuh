@@ -61,31 +61,36 @@ __global__ void k_prep(const int *__restrict__ skip, int np, int K, const double
 // Step 1: for each target, find the source panels of its group's P2P ranges that are the target's own
 // panel or lie inside the near-singular region |x_i - c_j|^2 < thres^2 * 2 A_j  (
 // reading A7).  fill == 0 counts, fill == 1 writes column indices (ascending).
-__global__ void __launch_bounds__(PYGBE_TG)
+// One warp per target: the lanes test 32 consecutive source panels at a time (coalesced), ballots keep the
+// column order ascending.
+__global__ void __launch_bounds__(128)
 k_near_find(int np, const double4 *__restrict__ tpos, const double4 *__restrict__ pnrm,
             const int *__restrict__ p2p_off,
             const int4 *__restrict__ p2p_rng, double thres2, int fill, int *__restrict__ cnt,
             const int *__restrict__ off, int *__restrict__ col)
 {
-    int g = blockIdx.x;
-    int t = g * PYGBE_TG + threadIdx.x;
+    const int t = (int)((blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     if (t >= np) return;
-    double4 X = tpos[t];
+    const int g = t / PYGBE_TG;
+    const double4 X = tpos[t];
     int n = 0;
-    int base = fill ? off[t] : 0;
+    const int base = fill ? off[t] : 0;
     for (int r = p2p_off[g]; r < p2p_off[g + 1]; r++) {
-        int4 rg = p2p_rng[r];
-        for (int j = rg.x; j < rg.y; j++) {
-            double4 c = tpos[j];
-            double dx = X.x - c.x, dy = X.y - c.y, dz = X.z - c.z;
-            bool near = (j == t) || (thres2 > 0.0 && dx * dx + dy * dy + dz * dz < thres2 * 2.0 * pnrm[j].w);
-            if (near) {
-                if (fill) col[base + n] = j;
-                n++;
+        const int4 rg = p2p_rng[r];
+        for (int j0 = rg.x; j0 < rg.y; j0 += 32) {
+            const int j = j0 + lane;
+            bool near = false;
+            if (j < rg.y) {
+                const double4 c = tpos[j];
+                const double dx = X.x - c.x, dy = X.y - c.y, dz = X.z - c.z;
+                near = (j == t) || (thres2 > 0.0 && dx * dx + dy * dy + dz * dz < thres2 * 2.0 * pnrm[j].w);
             }
+            const unsigned m = __ballot_sync(0xffffffffu, near);
+            if (fill && near) col[base + n + __popc(m & ((1u << lane) - 1u))] = j;
+            n += __popc(m);
         }
     }
-    if (!fill) cnt[t] = n;
+    if (!fill && lane == 0) cnt[t] = n;
 }
 
 // Semi-analytic self integral of the single-layer kernel (PAPER.md:165 [22], :235 "N_k"; reading A6):
@@ -119,7 +124,7 @@ __device__ double self_integral(const double *t, double kappa, const QuadTables 
 
 // Step 2: value of each correction entry = (fine rule or semi-analytic) - (what P2P adds with the K-point
 // rule), for the single- and the double-layer kernel, with sigma_S c_S / sigma_S of the source panel
-// folded in.  One thread per entry.  Self panel: V = semi-analytic, K = 0 (flat panel).
+// folded in.  One warp per target row, lanes over its entries.  Self panel: V = semi-analytic, K = 0 (flat panel).
 __global__ void k_near_values(int np, QuadTables q, bool yukawa, double kappa, const int *__restrict__ off,
                               const int *__restrict__ col, const int *__restrict__ gid,
                               const double *__restrict__ tri, const double4 *__restrict__ tpos,
@@ -127,11 +132,11 @@ __global__ void k_near_values(int np, QuadTables q, bool yukawa, double kappa, c
                               const double *__restrict__ cV, const double *__restrict__ cK,
                               double2 *__restrict__ val)
 {
-    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int t = (int)((blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
     if (t >= np) return;
     double4 X = tpos[t];
     const double inv4pi = 0.07957747154594767;
-    for (int e = off[t]; e < off[t + 1]; e++) {
+    for (int e = off[t] + lane; e < off[t + 1]; e += 32) {
         int j = col[e];
         double4 nA = pnrm[j];
         // coarse part, exactly as k_p2p evaluates it (unit densities)

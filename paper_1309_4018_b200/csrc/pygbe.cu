@@ -1,6 +1,7 @@
 // pygbe.cu -- the C ABI of include/pygbe.h.  Orchestration only: the host code parses inputs, sizes buffers,
 // turns traversal output into work items and launches kernels (build_*.cuh, matvec.cuh, solve.cuh); every
 // arithmetic step of the path runs on the device.
+#include <mutex>
 #include "common.cuh"
 #include "host_util.cuh"
 #include "tables.cuh"
@@ -22,11 +23,29 @@ void pygbe_set_error(const char *fmt, ...)
 extern "C" const char *pygbe_last_error(void) { return g_err; }
 extern "C" const char *pygbe_version(void) { return "pygbe-b200 0.2 sm_100a"; }
 
+// Pinned host blocks (128 B: GMRES flags and scalars read back each poll) are kept for the life of the
+// process and handed from handle to handle: cudaMallocHost costs 2-3 ms, a third of create at config 1.
+static std::mutex g_pinned_mu;
+static std::vector<void *> g_pinned_free;
+static void *pinned_block_get()
+{
+    {
+        std::lock_guard<std::mutex> lk(g_pinned_mu);
+        if (!g_pinned_free.empty()) { void *p = g_pinned_free.back(); g_pinned_free.pop_back(); return p; }
+    }
+    void *p = nullptr;
+    return cudaMallocHost(&p, 128) == cudaSuccess ? p : nullptr;
+}
+static void pinned_block_put(void *p)
+{
+    std::lock_guard<std::mutex> lk(g_pinned_mu);
+    g_pinned_free.push_back(p);
+}
+
 static void free_handle(pygbe_handle *h)
 {
     h->mem.release();
-    if (h->pinned_flags) cudaFreeHost(h->pinned_flags);
-    if (h->pinned_scal) cudaFreeHost(h->pinned_scal);
+    if (h->pinned_scal) pinned_block_put(h->pinned_scal);
     for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->ev_join) cudaEventDestroy(h->ev_join);
