@@ -98,7 +98,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     const double near_dist = h->thres > 0 ? h->thres * R.Lmax : 0.0;
     // break-even between one Taylor evaluation and the direct sum over a leaf's points: a regrouped M2P
     // evaluation costs Nc - 1 + NW FMA-pipe instructions per region, a P2P pair ~14 per region, and the sweep of
-    // profiles/r2a_upward.md puts the optimum at ~16 points for P = 6 (344 instructions) in both precisions
+    // profiles/r2a_regrouped_path.md puts the optimum at ~16 points for P = 6 (344 instructions) in both precisions
     const int small_leaf = (int)(16.0 * (h->Nc + 2.0 * h->NW) / 344.0 / K);
     LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.ggeo, R.cgeo, R.crange, R.cchild,
            h->theta, near_dist, small_leaf, 0, d_mcnt, d_pcnt, nullptr, nullptr, nullptr, nullptr, d_over);

@@ -51,7 +51,7 @@ static inline int cdiv(long a, long b) { return (int)((a + b - 1) / b); }
 // Device memory owned by a handle: blocks from the device's stream-ordered pool (cudaMallocAsync on the
 // handle's stream), freed together.  The pool keeps freed memory (release threshold raised at create), so
 // neither the scratch buffers of create nor a second handle pay cudaMalloc / cudaFree and their device-wide
-// synchronisation (create of config 1: 21 ms -> see profiles/r2a_upward.md).  Buffers are also read on the
+// synchronisation (create of config 1: 21 ms -> see profiles/r2a_regrouped_path.md).  Buffers are also read on the
 // handle's side streams, always after an event recorded on the main stream, and destroy synchronises every
 // stream before freeing.
 struct DeviceArena {

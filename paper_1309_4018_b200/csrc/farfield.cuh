@@ -51,7 +51,7 @@ __device__ __forceinline__ void wc_store(const MomOut &o, long cell, const doubl
 // (cV, cK: the per-region constants folded into the densities; k_prep leaves the two products in pq).  Each matvec the P2M is
 // then a streaming product: 2 Nc doubles read per panel, coalesced, two FMAs per 16 bytes -- HBM / L2 bound
 // as SURVEY 8(d) puts it (27.5 MB at 20 480 panels and P = 6) instead of the ALU- and latency-bound
-// monomial loop over the Gauss points of the first versions (29 us -> see profiles/r2a_upward.md).
+// monomial loop over the Gauss points of the first versions (29 us -> see profiles/r2a_regrouped_path.md).
 // pmom[panel][set][Nc], panels in the region's Morton order.
 #define PMOM_THREADS 128
 __global__ void __launch_bounds__(PMOM_THREADS)
