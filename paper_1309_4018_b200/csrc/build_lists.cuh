@@ -85,7 +85,9 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
         }
         TRY(upload(h, &R.panel_anchor, panel_anchor));
         TRY(h->mem.alloc(&R.sposf, R.npts)); TRY(h->mem.alloc(&R.schgf, R.npts));
-        LAUNCH(h, k_make_sposf, cdiv(R.np, 128), 128, 0, R.np, K, R.panel_anchor, R.cgeo, R.spos, R.sposf);
+        R.quad = K % 4 == 0;                  // packed-fp32 P2P on quads of Gauss points (p2p.cuh)
+        if (R.quad) LAUNCH(h, k_make_sposq, cdiv(R.npts, 256), 256, 0, R.np, K, R.panel_anchor, R.cgeo, R.spos, (float *)R.sposf);
+        else LAUNCH(h, k_make_sposf, cdiv(R.np, 128), 128, 0, R.np, K, R.panel_anchor, R.cgeo, R.spos, R.sposf);
     }
 
     // ---- target groups + traversal (count, offsets, fill)

@@ -109,6 +109,7 @@ struct Region {
     double4 *spos = nullptr;        // (x, y, z, w_g A_j / 4pi)
     double4 *schg = nullptr;        // per matvec: (mV, mKx, mKy, mKz)
     float4 *sposf = nullptr;        // mixed precision: position relative to the anchor cell centre, weight
+    bool quad = false;              // sposf / schgf hold quads of four points, structure-of-arrays (packed P2P, p2p.cuh)
     float4 *schgf = nullptr;
     double *pphi = nullptr, *pdphi = nullptr;   // per matvec: gathered densities
     double2 *pq = nullptr;          // per matvec: (cV dphi, cK phi) per panel, the weights of the panel moments (P2M)

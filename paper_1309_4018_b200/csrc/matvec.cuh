@@ -55,12 +55,16 @@ static void launch_p2p(pygbe_handle *h, Region &A, Region *B, const int *skip)
     typedef typename Real<T>::vec4 V4;
     const V4 *pos = sizeof(T) == 4 ? (const V4 *)A.sposf : (const V4 *)A.spos;
     const V4 *chg = sizeof(T) == 4 ? (const V4 *)A.schgf : (const V4 *)A.schg;
-    const double kA = A.kappa, kB = B ? B->kappa : 0.0, rV = A.twin_rV;
+    const double kA = A.kappa, kB = B ? B->kappa : 0.0, rV = B ? A.twin_rV : 1.0;
     double *oA = A.out, *oB = B ? B->out : nullptr;
+    const bool quad = sizeof(T) == 4 && A.quad;
 #define P2P_GO(YA, TW, YB)                                                                                     \
-    do { auto kern = k_p2p<T, YA, TW, YB>;                                                                     \
-    LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, A.np, A.tpos,              \
-           A.cgeo, pos, chg, kA, kB, rV, oA, oB); } while (0)
+    do { if (quad) { auto kern = k_p2p_quad<YA, TW, YB>;                                                       \
+             LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, A.np, A.tpos, A.cgeo,   \
+                    (const float4 *)A.sposf, (const float4 *)A.schgf, kA, kB, rV, oA, oB); }                   \
+         else { auto kern = k_p2p<T, YA, TW, YB>;                                                              \
+             LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, A.np, A.tpos,           \
+                    A.cgeo, pos, chg, kA, kB, rV, oA, oB); } } while (0)
     if (!B) { if (A.yukawa) P2P_GO(true, false, false); else P2P_GO(false, false, false); }
     else if (A.yukawa) { if (B->yukawa) P2P_GO(true, true, true); else P2P_GO(true, true, false); }
     else { if (B->yukawa) P2P_GO(false, true, true); else P2P_GO(false, true, false); }
@@ -91,7 +95,8 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
     for (auto &w : work) {
         Region &A = *w.first; Region *B = w.second;
         LAUNCH(h, k_prep, cdiv((long)A.np * h->K, 256), 256, 0, skip, A.np, h->K, x, A.phi_idx, A.dphi_idx, A.cV, A.cK, A.pnrm,
-               A.spos, A.schg, mixed ? A.schgf : (float4 *)nullptr, A.pphi, A.pdphi, A.pq, A.out, B ? B->out : (double *)nullptr);
+               A.spos, mixed ? (double4 *)nullptr : A.schg, mixed ? A.schgf : (float4 *)nullptr, A.quad ? 1 : 0, A.pphi, A.pdphi,
+               A.pq, A.out, B ? B->out : (double *)nullptr);
     }
     STAGE_END(h, PYGBE_STAGE_PREP);
     if (fork) {

@@ -35,9 +35,10 @@ __global__ void k_prep(const int *__restrict__ skip, int np, int K, const double
                        const int *__restrict__ dphi_idx, const double *__restrict__ cV,
                        const double *__restrict__ cK, const double4 *__restrict__ pnrm,
                        const double4 *__restrict__ spos, double4 *__restrict__ schg,
-                       float4 *__restrict__ schgf, double *__restrict__ pphi, double *__restrict__ pdphi,
+                       float4 *__restrict__ schgf, int quad, double *__restrict__ pphi, double *__restrict__ pdphi,
                        double2 *__restrict__ pq, double *__restrict__ out, double *__restrict__ out_twin)
-{
+{   // schg: fp64 charges (null in the mixed-precision matvec, whose kernels read schgf only); schgf: fp32 copy,
+    // point by point or, with quad = 1, in the quad layout of the packed P2P (p2p.cuh)
     if (skip && *skip) return;
     const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;      // Gauss point
     if (i >= (long)np * K) return;
@@ -53,8 +54,15 @@ __global__ void k_prep(const int *__restrict__ skip, int np, int K, const double
     const double4 n = pnrm[p];
     const double w = spos[i].w;
     const double4 c = make_double4(w * qV, w * qK * n.x, w * qK * n.y, w * qK * n.z);
-    schg[i] = c;
-    if (schgf) schgf[i] = make_float4((float)c.x, (float)c.y, (float)c.z, (float)c.w);
+    if (schg) schg[i] = c;
+    if (schgf) {
+        if (quad) {
+            float *f = (float *)schgf + 16 * (i >> 2) + (i & 3);
+            f[0] = (float)c.x; f[4] = (float)c.y; f[8] = (float)c.z; f[12] = (float)c.w;
+        } else {
+            schgf[i] = make_float4((float)c.x, (float)c.y, (float)c.z, (float)c.w);
+        }
+    }
 }
 
 // ------------------------------------------------------------------- singular / near-singular panels

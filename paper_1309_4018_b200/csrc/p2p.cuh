@@ -138,3 +138,146 @@ k_p2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *
         if constexpr (TWIN) atomicAdd(outB + t, accB);
     }
 }
+
+// ------------------------------------------------------------------------------------------------------
+// Mixed precision, K a multiple of 4: the same sums with packed fp32 arithmetic (add / mul / fma .f32x2:
+// FADD2 / FMUL2 / FFMA2 on sm_100), two source points per instruction.  The first fp32 kernel was issue-bound
+// at 29 instructions per fused pair (profiles/r2a_regrouped_path.md); packing halves the FP32 issue slots (the
+// MUFU rsqrt / ex2 and the zero-distance guard stay scalar).  Sources are stored as quads of four consecutive
+// Gauss points, structure-of-arrays inside the quad, so that one LDS.128 yields two register pairs:
+//   posq[3 q + {0,1,2}] = (x0..x3), (y0..y3), (z0..z3)   relative to the anchor cell centre (create)
+//   chgq[4 q + {0,1,2,3}] = (mV0..3), (mKx0..3), (mKy0..3), (mKz0..3)   (k_prep, every matvec)
+// Region B's charges are rV mV and -mK: its sum is accumulated as sum (mV + t (1 + kappa r) / rV) w and
+// multiplied by rV once at the end.
+typedef unsigned long long f2_t;                                      // two packed floats
+__device__ __forceinline__ f2_t f2_pack(float lo, float hi) { f2_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void f2_unpack(f2_t v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f2_t f2_add(f2_t a, f2_t b) { f2_t r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2_t f2_sub(f2_t a, f2_t b) { f2_t r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2_t f2_mul(f2_t a, f2_t b) { f2_t r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f2_t f2_fma(f2_t a, f2_t b, f2_t c) { f2_t r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+
+struct P2PQuadConst {                                                 // loop invariants, already packed
+    f2_t nksA, nksB;            // -kappa log2(e) of regions A and B
+    f2_t kA;                    // kappa_A
+    f2_t sB, cB;                // 1 / rV and kappa_B / rV
+};
+
+// two source points (packed) against one target
+template <bool YA, bool TWIN, bool YB>
+__device__ __forceinline__ void p2p_pair2(f2_t X, f2_t Y, f2_t Z, f2_t px, f2_t py, f2_t pz, f2_t mV, f2_t mKx, f2_t mKy,
+                                          f2_t mKz, const P2PQuadConst &k, f2_t &accA, f2_t &accB)
+{
+    const f2_t dx = f2_sub(X, px), dy = f2_sub(Y, py), dz = f2_sub(Z, pz);
+    const f2_t r2 = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
+    const f2_t mKd = f2_fma(mKz, dz, f2_fma(mKy, dy, f2_mul(mKx, dx)));
+    float r2a, r2b;
+    f2_unpack(r2, r2a, r2b);
+    const float ia = r2a > 0.f ? Real<float>::rsqrt_(r2a) : 0.f, ib = r2b > 0.f ? Real<float>::rsqrt_(r2b) : 0.f;
+    const f2_t rinv = f2_pack(ia, ib);
+    const f2_t t = f2_mul(mKd, f2_mul(rinv, rinv));
+    const f2_t r = f2_mul(r2, rinv);
+    if constexpr (YA) {
+        float ea, eb;
+        f2_unpack(f2_mul(r, k.nksA), ea, eb);
+        asm("ex2.approx.ftz.f32 %0, %0;" : "+f"(ea));
+        asm("ex2.approx.ftz.f32 %0, %0;" : "+f"(eb));
+        const f2_t u = f2_fma(f2_mul(t, k.kA), r, t);                 // t (1 + kappa r)
+        accA = f2_fma(f2_sub(mV, u), f2_mul(rinv, f2_pack(ea, eb)), accA);
+    } else {
+        accA = f2_fma(f2_sub(mV, t), rinv, accA);
+    }
+    if constexpr (TWIN) {
+        if constexpr (YB) {
+            float ea, eb;
+            f2_unpack(f2_mul(r, k.nksB), ea, eb);
+            asm("ex2.approx.ftz.f32 %0, %0;" : "+f"(ea));
+            asm("ex2.approx.ftz.f32 %0, %0;" : "+f"(eb));
+            const f2_t u = f2_mul(t, f2_fma(k.cB, r, k.sB));          // t (1 + kappa r) / rV
+            accB = f2_fma(f2_add(mV, u), f2_mul(rinv, f2_pack(ea, eb)), accB);
+        } else {
+            accB = f2_fma(f2_fma(t, k.sB, mV), rinv, accB);           // (mV + t / rV) / r
+        }
+    }
+}
+
+#define P2P_QTILE (P2P_TILE / 4)                                       // quads per tile
+template <bool YA, bool TWIN, bool YB>
+__global__ void __launch_bounds__(PYGBE_TG)
+k_p2p_quad(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *__restrict__ tiles, int np,
+           const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const float4 *__restrict__ posq,
+           const float4 *__restrict__ chgq, double kappaA, double kappaB, double rV, double *__restrict__ outA,
+           double *__restrict__ outB)
+{
+    __shared__ __align__(16) float4 s_pos[2][3 * P2P_QTILE];
+    __shared__ __align__(16) float4 s_chg[2][4 * P2P_QTILE];
+    __shared__ __align__(16) double4 s_an[2];
+    if (skip && *skip) return;
+    const int4 it = items[blockIdx.x];
+    const int t = it.x * PYGBE_TG + threadIdx.x;
+    const bool ok = t < np;
+    const double4 X = ok ? tpos[t] : make_double4(0, 0, 0, 0);
+    P2PQuadConst kc;
+    {
+        const float a = -(float)Real<float>::kscale(kappaA), b = -(float)Real<float>::kscale(kappaB);
+        const float s = (float)(1.0 / rV), c = (float)(kappaB / rV), ka = (float)kappaA;
+        kc.nksA = f2_pack(a, a); kc.nksB = f2_pack(b, b); kc.kA = f2_pack(ka, ka); kc.sB = f2_pack(s, s); kc.cB = f2_pack(c, c);
+    }
+    double accA = 0.0, accB = 0.0;
+    auto stage = [&](int buf, const int4 &tl) {                      // tl = (first point, points, anchor, -), both multiples of 4
+        const int q0 = tl.x >> 2, nq = tl.y >> 2;
+        for (int i = threadIdx.x; i < 3 * nq; i += PYGBE_TG) cp_async16(&s_pos[buf][i], posq + 3 * (long)q0 + i);
+        for (int i = threadIdx.x; i < 4 * nq; i += PYGBE_TG) cp_async16(&s_chg[buf][i], chgq + 4 * (long)q0 + i);
+        if (threadIdx.x < 2)
+            cp_async16((char *)&s_an[buf] + 16 * threadIdx.x, (const char *)(cgeo + tl.z) + 16 * threadIdx.x);
+        cp_async_commit();
+    };
+    int4 cur = tiles[it.y];
+    int4 nxt = it.y + 1 < it.z ? tiles[it.y + 1] : cur;
+    stage(0, cur);
+    int buf = 0;
+    for (int k = it.y; k < it.z; k++, buf ^= 1) {
+        const bool more = k + 1 < it.z;
+        if (more) { stage(buf ^ 1, nxt); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+        const int nq = cur.y >> 2;
+        cur = nxt;
+        if (k + 2 < it.z) nxt = tiles[k + 2];
+        __syncthreads();
+        const double4 an = s_an[buf];
+        const float x = (float)(X.x - an.x), y = (float)(X.y - an.y), z = (float)(X.z - an.z);
+        const f2_t X2 = f2_pack(x, x), Y2 = f2_pack(y, y), Z2 = f2_pack(z, z);
+        const float4 *sp = s_pos[buf], *sc = s_chg[buf];
+        f2_t a0 = 0, a1 = 0, b0 = 0, b1 = 0;                          // (+0.f, +0.f)
+#pragma unroll 2
+        for (int q = 0; q < nq; q++) {
+            const float4 px = sp[3 * q], py = sp[3 * q + 1], pz = sp[3 * q + 2];
+            const float4 mV = sc[4 * q], mKx = sc[4 * q + 1], mKy = sc[4 * q + 2], mKz = sc[4 * q + 3];
+            p2p_pair2<YA, TWIN, YB>(X2, Y2, Z2, f2_pack(px.x, px.y), f2_pack(py.x, py.y), f2_pack(pz.x, pz.y), f2_pack(mV.x, mV.y),
+                                    f2_pack(mKx.x, mKx.y), f2_pack(mKy.x, mKy.y), f2_pack(mKz.x, mKz.y), kc, a0, b0);
+            p2p_pair2<YA, TWIN, YB>(X2, Y2, Z2, f2_pack(px.z, px.w), f2_pack(py.z, py.w), f2_pack(pz.z, pz.w), f2_pack(mV.z, mV.w),
+                                    f2_pack(mKx.z, mKx.w), f2_pack(mKy.z, mKy.w), f2_pack(mKz.z, mKz.w), kc, a1, b1);
+        }
+        float lo, hi;
+        f2_unpack(f2_add(a0, a1), lo, hi);
+        accA += (double)(lo + hi);
+        if constexpr (TWIN) { f2_unpack(f2_add(b0, b1), lo, hi); accB += (double)(lo + hi); }
+        __syncthreads();                                             // buf is refilled two iterations from now
+    }
+    if (ok) {
+        atomicAdd(outA + t, accA);
+        if constexpr (TWIN) atomicAdd(outB + t, rV * accB);
+    }
+}
+
+// quad layout of the fp32 source coordinates (create time): see k_make_sposf for the rounding
+__global__ void k_make_sposq(int np, int K, const int *__restrict__ panel_anchor, const double4 *__restrict__ cgeo,
+                             const double4 *__restrict__ spos, float *__restrict__ posq)
+{
+    const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;      // Gauss point
+    if (i >= (long)np * K) return;
+    const double4 an = cgeo[panel_anchor[i / K]];
+    const double4 s = spos[i];
+    const long q = i >> 2;
+    const int l = (int)(i & 3);
+    posq[12 * q + l] = (float)(s.x - an.x); posq[12 * q + 4 + l] = (float)(s.y - an.y); posq[12 * q + 8 + l] = (float)(s.z - an.z);
+}

@@ -139,7 +139,7 @@ extern "C" int pygbe_reaction_potential(pygbe_handle *h, const double *x_dev, do
     for (Region &R : h->regions) {
         if (R.nq == 0) continue;
         LAUNCH(h, k_prep, cdiv((long)R.np * h->K, 256), 256, 0, nullptr, R.np, h->K, x_dev, R.phi_idx, R.dphi_idx, R.cV, R.cK, R.pnrm,
-               R.spos, R.schg, (float4 *)nullptr, R.pphi, R.pdphi, R.pq, R.out, (double *)nullptr);
+               R.spos, R.schg, (float4 *)nullptr, 0, R.pphi, R.pdphi, R.pq, R.out, (double *)nullptr);
         dim3 grid(cdiv(R.npts, EN_CHUNK), R.nq);
         if (R.yukawa) LAUNCH(h, k_reaction<true>, grid, EN_THREADS, 0, R.npts, R.spos, R.schg, R.nq, R.qpos, R.qid, R.kappa, phi_dev);
         else LAUNCH(h, k_reaction<false>, grid, EN_THREADS, 0, R.npts, R.spos, R.schg, R.nq, R.qpos, R.qid, R.kappa, phi_dev);

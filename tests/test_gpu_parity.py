@@ -221,6 +221,25 @@ def test_treecode_error_decreases_with_order(env):
     assert all(b < a for a, b in zip(errs, errs[1:]))
 
 
+@pytest.mark.parametrize("maker,level", [(W.kirkwood_problem, 3), (W.stern_sphere_problem, 3)])
+def test_mixed_precision_other_orders(env, maker, level):
+    """fp32 evaluation of the regrouped Taylor series (csrc/m2p.cuh) at orders other than the benchmark's, with
+    twin regions (one fused pass) and without: against the oracle, and against the fp64 kernels of the same order."""
+    pg, torch, orc = env
+    prob = maker(level)
+    o = orc.Oracle(prob)
+    x = np.random.default_rng(12).normal(size=o.n)
+    yo = o.matvec(x)
+    for P in (2, 4, 8, 10, 12):
+        h64, y64 = gpu_matvec(pg, torch, prob, x, K=4, P=P, theta=0.5, ncrit=16)
+        h32, y32 = gpu_matvec(pg, torch, prob, x, K=4, P=P, theta=0.5, ncrit=16, precision=pg.PRECISION_MIXED)
+        assert h32.stats()["m2p_evals"] > 0
+        assert rel(y32, y64) < 5e-6, (P, rel(y32, y64))
+        if P >= 6:
+            assert rel(y32, yo) <= TOL_TREE
+        h64.close(); h32.close()
+
+
 @pytest.mark.parametrize("ncrit", [8, 40, 500])
 def test_treecode_leaf_sizes(env, ncrit):
     pg, torch, orc = env
