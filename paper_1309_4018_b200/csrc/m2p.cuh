@@ -120,6 +120,62 @@ __device__ __forceinline__ T m2p_radial(T r, T rinv, T rinv2, T kappa, T kscaled
     return acc;
 }
 
+// fp32 twin regions: the W of A and B are interleaved in the row, so the pair (Q_m^A, Q_m^B) is one packed
+// accumulator and each W pair costs one FFMA2 with the monomial as broadcast operand; the radial part runs on
+// the pairs (F_A^(m), F_B^(m)) likewise.  Returns (sum_m F_A^(m) Q_m^A, sum_m F_B^(m) Q_m^B).
+template <int P>
+__device__ __forceinline__ f2_t m2p_twin_packed(float dx, float dy, float dz, const float *__restrict__ w, float kappaA,
+                                                float ksA, float kappaB, float ksB)
+{
+    f2_t q[P + 1];
+#pragma unroll
+    for (int m = 0; m <= P; m++) q[m] = 0;
+    int idx = 0;
+    float4 cur = make_float4(0.f, 0.f, 0.f, 0.f);
+    float px = 1.f;
+#pragma unroll
+    for (int ex = 0; ex <= P; ex++) {
+        float pxy = px;
+#pragma unroll
+        for (int ey = 0; ey <= P - ex; ey++) {
+            float mono = pxy;
+#pragma unroll
+            for (int ez = 0; ez <= P - ex - ey; ez++) {
+                const int t = ex + ey + ez;
+                const f2_t m2 = f2_pack(mono, mono);
+#pragma unroll
+                for (int J = 0; J <= (P - t) / 2; J++) {
+                    if (idx % 2 == 0) cur = *(const float4 *)(w + 2 * idx);
+                    q[t + J] = f2_fma(idx % 2 == 0 ? f2_pack(cur.x, cur.y) : f2_pack(cur.z, cur.w), m2, q[t + J]);
+                    idx++;
+                }
+                mono *= dz;
+            }
+            pxy *= dy;
+        }
+        px *= dx;
+    }
+    const float r2 = dx * dx + dy * dy + dz * dz;
+    const float rinv = Real<float>::rsqrt_(r2), rinv2 = rinv * rinv, r = r2 * rinv;
+    const float EA = kappaA != 0.f ? Real<float>::exp_neg(ksA, r) : 1.f, EB = kappaB != 0.f ? Real<float>::exp_neg(ksB, r) : 1.f;
+    const f2_t ri2 = f2_pack(rinv2, rinv2), kap = f2_pack(kappaA, kappaB), k2 = f2_mul(kap, kap);
+    f2_t gm = f2_mul(f2_pack(EA, EB), f2_pack(rinv, rinv));                                    // F^(0)
+    f2_t acc = f2_mul(gm, q[0]);
+    if (P >= 1) {
+        const float nr3 = -rinv * rinv2;
+        f2_t g = f2_mul(f2_mul(f2_pack(EA, EB), f2_fma(kap, f2_pack(r, r), f2_pack(1.f, 1.f))), f2_pack(nr3, nr3));   // F^(1)
+        acc = f2_fma(g, q[1], acc);
+#pragma unroll
+        for (int m = 1; m < P; m++) {
+            const float c = -(float)(2 * m + 1);
+            const f2_t gn = f2_mul(f2_fma(g, f2_pack(c, c), f2_mul(k2, gm)), ri2);             // -[(2m+1) g - k^2 gm] / r^2
+            gm = g; g = gn;
+            acc = f2_fma(g, q[m + 1], acc);
+        }
+    }
+    return acc;
+}
+
 // Work item = (target group, a run of its M2P list).  One thread per target; the W rows of CB cells at a
 // time are staged in shared memory and read by all threads as 16-byte broadcasts.  The target offset
 // d = x - y_c is always formed in fp64 and then rounded to T, so the fp32 path never subtracts large absolute
@@ -167,12 +223,19 @@ k_m2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int *_
         for (int c_ = 0; c_ < nb; c_++) {
             const double4 c = s_c[buf][c_];
             const T dx = (T)(X.x - c.x), dy = (T)(X.y - c.y), dz = (T)(X.z - c.z);
-            T q[P + 1][NS];
-            m2p_q<P, NS, T>(dx, dy, dz, s_W[buf][c_], q);
-            const T r2 = dx * dx + dy * dy + dz * dz;
-            const T rinv = Real<T>::rsqrt_(r2), rinv2 = rinv * rinv, r = r2 * rinv;
-            accA += (double)m2p_radial<P, NS, T>(r, rinv, rinv2, (T)kappaA, (T)kscaledA, q, 0);
-            if (TWIN) accB += (double)m2p_radial<P, NS, T>(r, rinv, rinv2, (T)kappaB, (T)kscaledB, q, NS - 1);
+            if constexpr (TWIN && sizeof(T) == 4) {
+                float va, vb;
+                f2_unpack(m2p_twin_packed<P>(dx, dy, dz, (const float *)s_W[buf][c_], (float)kappaA, (float)kscaledA,
+                                             (float)kappaB, (float)kscaledB), va, vb);
+                accA += (double)va; accB += (double)vb;
+            } else {
+                T q[P + 1][NS];
+                m2p_q<P, NS, T>(dx, dy, dz, s_W[buf][c_], q);
+                const T r2 = dx * dx + dy * dy + dz * dz;
+                const T rinv = Real<T>::rsqrt_(r2), rinv2 = rinv * rinv, r = r2 * rinv;
+                accA += (double)m2p_radial<P, NS, T>(r, rinv, rinv2, (T)kappaA, (T)kscaledA, q, 0);
+                if (TWIN) accB += (double)m2p_radial<P, NS, T>(r, rinv, rinv2, (T)kappaB, (T)kscaledB, q, NS - 1);
+            }
         }
         __syncthreads();                                     // buf is refilled two iterations from now
     }
@@ -180,4 +243,232 @@ k_m2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int *_
         atomicAdd(outA + t, accA);
         if (TWIN) atomicAdd(outB + t, accB);
     }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// fp32 twin regions, two targets per thread.  The kernel above is bound by the shared-memory data pipe, not by
+// issue or the FMA pipe (ncu: l1tex__data_pipe_lsu_wavefronts 79 % of peak while active; every broadcast
+// LDS.128 is two wavefronts for four W): with two targets in a thread each W read feeds twice the FMAs.  One
+// warp per 64-target group; the monomials of the two targets travel as one packed pair.
+template <int P>
+__device__ __forceinline__ void m2p_twin_packed2(f2_t dx, f2_t dy, f2_t dz, const float *__restrict__ w, f2_t (&qa)[P + 1],
+                                                 f2_t (&qb)[P + 1])
+{
+#pragma unroll
+    for (int m = 0; m <= P; m++) { qa[m] = 0; qb[m] = 0; }
+    int idx = 0;
+    float4 cur = make_float4(0.f, 0.f, 0.f, 0.f);
+    f2_t px = f2_pack(1.f, 1.f);
+#pragma unroll
+    for (int ex = 0; ex <= P; ex++) {
+        f2_t pxy = px;
+#pragma unroll
+        for (int ey = 0; ey <= P - ex; ey++) {
+            f2_t mono = pxy;
+#pragma unroll
+            for (int ez = 0; ez <= P - ex - ey; ez++) {
+                const int t = ex + ey + ez;
+                float ma, mb;
+                f2_unpack(mono, ma, mb);
+                const f2_t m2a = f2_pack(ma, ma), m2b = f2_pack(mb, mb);
+#pragma unroll
+                for (int J = 0; J <= (P - t) / 2; J++) {
+                    if (idx % 2 == 0) cur = *(const float4 *)(w + 2 * idx);
+                    const f2_t w2 = idx % 2 == 0 ? f2_pack(cur.x, cur.y) : f2_pack(cur.z, cur.w);
+                    qa[t + J] = f2_fma(w2, m2a, qa[t + J]);
+                    qb[t + J] = f2_fma(w2, m2b, qb[t + J]);
+                    idx++;
+                }
+                mono = f2_mul(mono, dz);
+            }
+            pxy = f2_mul(pxy, dy);
+        }
+        px = f2_mul(px, dx);
+    }
+}
+
+// (sum_m F_A^(m) Q_m^A, sum_m F_B^(m) Q_m^B) of one target from its packed accumulators
+template <int P>
+__device__ __forceinline__ f2_t m2p_radial_packed(float dx, float dy, float dz, const f2_t (&q)[P + 1], float kappaA, float ksA,
+                                                  float kappaB, float ksB)
+{
+    const float r2 = dx * dx + dy * dy + dz * dz;
+    const float rinv = Real<float>::rsqrt_(r2), rinv2 = rinv * rinv, r = r2 * rinv;
+    const float EA = kappaA != 0.f ? Real<float>::exp_neg(ksA, r) : 1.f, EB = kappaB != 0.f ? Real<float>::exp_neg(ksB, r) : 1.f;
+    const f2_t ri2 = f2_pack(rinv2, rinv2), kap = f2_pack(kappaA, kappaB), k2 = f2_mul(kap, kap);
+    f2_t gm = f2_mul(f2_pack(EA, EB), f2_pack(rinv, rinv));                                    // F^(0)
+    f2_t acc = f2_mul(gm, q[0]);
+    if (P >= 1) {
+        const float nr3 = -rinv * rinv2;
+        f2_t g = f2_mul(f2_mul(f2_pack(EA, EB), f2_fma(kap, f2_pack(r, r), f2_pack(1.f, 1.f))), f2_pack(nr3, nr3));   // F^(1)
+        acc = f2_fma(g, q[1], acc);
+#pragma unroll
+        for (int m = 1; m < P; m++) {
+            const float c = -(float)(2 * m + 1);
+            const f2_t gn = f2_mul(f2_fma(g, f2_pack(c, c), f2_mul(k2, gm)), ri2);             // -[(2m+1) g - k^2 gm] / r^2
+            gm = g; g = gn;
+            acc = f2_fma(g, q[m + 1], acc);
+        }
+    }
+    return acc;
+}
+
+#define M2P2_THREADS (PYGBE_TG_M2P / 2)
+template <int P>
+__global__ void __launch_bounds__(M2P2_THREADS)
+k_m2p_twin2(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
+            const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const float *__restrict__ wc,
+            double kappaA, double kscaledA, double kappaB, double kscaledB, double *__restrict__ outA, double *__restrict__ outB)
+{
+    constexpr int STRIDE = m2p_stride(P, true);
+    constexpr int CH = STRIDE / 4;                           // 16-byte chunks per cell
+    constexpr int CBW = 12288 / (STRIDE * 4);
+    constexpr int CB = CBW < 1 ? 1 : (CBW > 4 ? 4 : CBW);
+    __shared__ __align__(16) float s_W[2][CB][STRIDE];
+    __shared__ __align__(16) double4 s_c[2][CB];
+    if (skip && *skip) return;
+    const int4 it = items[blockIdx.x];
+    const int t0 = it.x * PYGBE_TG_M2P + threadIdx.x, t1 = t0 + M2P2_THREADS;
+    const bool ok0 = t0 < np, ok1 = t1 < np;
+    const double4 X0 = ok0 ? tpos[t0] : make_double4(1e30, 1e30, 1e30, 0), X1 = ok1 ? tpos[t1] : make_double4(1e30, 1e30, 1e30, 0);
+    const float kA = (float)kappaA, ksA = (float)kscaledA, kB = (float)kappaB, ksB = (float)kscaledB;
+    double aA0 = 0.0, aB0 = 0.0, aA1 = 0.0, aB1 = 0.0;
+    auto stage = [&](int buf, int s0) {
+        const int nb = min(CB, it.z - s0);
+        for (int i = threadIdx.x; i < nb * CH; i += M2P2_THREADS) {
+            const int c_ = i / CH, j = i - c_ * CH;
+            cp_async16(&s_W[buf][c_][j * 4], wc + (long)m2p_cell[s0 + c_] * STRIDE + j * 4);
+        }
+        if (threadIdx.x < nb * 2) {
+            const int c_ = threadIdx.x >> 1, hf = threadIdx.x & 1;
+            cp_async16((char *)&s_c[buf][c_] + 16 * hf, (const char *)(cgeo + m2p_cell[s0 + c_]) + 16 * hf);
+        }
+        cp_async_commit();
+    };
+    stage(0, it.y);
+    int buf = 0;
+    for (int s0 = it.y; s0 < it.z; s0 += CB, buf ^= 1) {
+        const int nb = min(CB, it.z - s0);
+        const bool more = s0 + CB < it.z;
+        if (more) { stage(buf ^ 1, s0 + CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+        __syncthreads();
+        for (int c_ = 0; c_ < nb; c_++) {
+            const double4 c = s_c[buf][c_];
+            const float dx0 = (float)(X0.x - c.x), dy0 = (float)(X0.y - c.y), dz0 = (float)(X0.z - c.z);
+            const float dx1 = (float)(X1.x - c.x), dy1 = (float)(X1.y - c.y), dz1 = (float)(X1.z - c.z);
+            f2_t qa[P + 1], qb[P + 1];
+            m2p_twin_packed2<P>(f2_pack(dx0, dx1), f2_pack(dy0, dy1), f2_pack(dz0, dz1), s_W[buf][c_], qa, qb);
+            float va, vb;
+            f2_unpack(m2p_radial_packed<P>(dx0, dy0, dz0, qa, kA, ksA, kB, ksB), va, vb);
+            aA0 += (double)va; aB0 += (double)vb;
+            f2_unpack(m2p_radial_packed<P>(dx1, dy1, dz1, qb, kA, ksA, kB, ksB), va, vb);
+            aA1 += (double)va; aB1 += (double)vb;
+        }
+        __syncthreads();                                     // buf is refilled two iterations from now
+    }
+    if (ok0) { atomicAdd(outA + t0, aA0); atomicAdd(outB + t0, aB0); }
+    if (ok1) { atomicAdd(outA + t1, aA1); atomicAdd(outB + t1, aB1); }
+}
+
+// fp32, a tree without twin, two targets per thread: the pair is (target 0, target 1) -- packed monomials,
+// packed accumulators Q_m, W as the broadcast operand -- including the radial part.
+template <int P>
+__global__ void __launch_bounds__(M2P2_THREADS)
+k_m2p_single2(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
+              const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const float *__restrict__ wc,
+              double kappa, double kscaled, double *__restrict__ out)
+{
+    constexpr int STRIDE = m2p_stride(P, false);
+    constexpr int CH = STRIDE / 4;                           // 16-byte chunks per cell
+    constexpr int CBW = 12288 / (STRIDE * 4);
+    constexpr int CB = CBW < 1 ? 1 : (CBW > 4 ? 4 : CBW);
+    __shared__ __align__(16) float s_W[2][CB][STRIDE];
+    __shared__ __align__(16) double4 s_c[2][CB];
+    if (skip && *skip) return;
+    const int4 it = items[blockIdx.x];
+    const int t0 = it.x * PYGBE_TG_M2P + threadIdx.x, t1 = t0 + M2P2_THREADS;
+    const bool ok0 = t0 < np, ok1 = t1 < np;
+    const double4 X0 = ok0 ? tpos[t0] : make_double4(1e30, 1e30, 1e30, 0), X1 = ok1 ? tpos[t1] : make_double4(1e30, 1e30, 1e30, 0);
+    const float kap = (float)kappa, ks = (float)kscaled;
+    const f2_t kap2 = f2_pack(kap, kap), k2 = f2_pack(kap * kap, kap * kap), one2 = f2_pack(1.f, 1.f);
+    double a0 = 0.0, a1 = 0.0;
+    auto stage = [&](int buf, int s0) {
+        const int nb = min(CB, it.z - s0);
+        for (int i = threadIdx.x; i < nb * CH; i += M2P2_THREADS) {
+            const int c_ = i / CH, j = i - c_ * CH;
+            cp_async16(&s_W[buf][c_][j * 4], wc + (long)m2p_cell[s0 + c_] * STRIDE + j * 4);
+        }
+        if (threadIdx.x < nb * 2) {
+            const int c_ = threadIdx.x >> 1, hf = threadIdx.x & 1;
+            cp_async16((char *)&s_c[buf][c_] + 16 * hf, (const char *)(cgeo + m2p_cell[s0 + c_]) + 16 * hf);
+        }
+        cp_async_commit();
+    };
+    stage(0, it.y);
+    int buf = 0;
+    for (int s0 = it.y; s0 < it.z; s0 += CB, buf ^= 1) {
+        const int nb = min(CB, it.z - s0);
+        const bool more = s0 + CB < it.z;
+        if (more) { stage(buf ^ 1, s0 + CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+        __syncthreads();
+        for (int c_ = 0; c_ < nb; c_++) {
+            const double4 c = s_c[buf][c_];
+            const f2_t dx = f2_pack((float)(X0.x - c.x), (float)(X1.x - c.x)), dy = f2_pack((float)(X0.y - c.y), (float)(X1.y - c.y)),
+                       dz = f2_pack((float)(X0.z - c.z), (float)(X1.z - c.z));
+            const float *w = s_W[buf][c_];
+            f2_t q[P + 1];
+#pragma unroll
+            for (int m = 0; m <= P; m++) q[m] = 0;
+            int idx = 0;
+            float cur[4] = {0.f, 0.f, 0.f, 0.f};
+            f2_t px = one2;
+#pragma unroll
+            for (int ex = 0; ex <= P; ex++) {
+                f2_t pxy = px;
+#pragma unroll
+                for (int ey = 0; ey <= P - ex; ey++) {
+                    f2_t mono = pxy;
+#pragma unroll
+                    for (int ez = 0; ez <= P - ex - ey; ez++) {
+                        const int t = ex + ey + ez;
+#pragma unroll
+                        for (int J = 0; J <= (P - t) / 2; J++) {
+                            if (idx % 4 == 0) Chunk<float>::get(w + idx, cur);
+                            q[t + J] = f2_fma(f2_pack(cur[idx % 4], cur[idx % 4]), mono, q[t + J]);
+                            idx++;
+                        }
+                        mono = f2_mul(mono, dz);
+                    }
+                    pxy = f2_mul(pxy, dy);
+                }
+                px = f2_mul(px, dx);
+            }
+            // radial part, both targets at once
+            const f2_t r2 = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
+            float ra, rb;
+            f2_unpack(r2, ra, rb);
+            const f2_t rinv = f2_pack(Real<float>::rsqrt_(ra), Real<float>::rsqrt_(rb)), rinv2 = f2_mul(rinv, rinv), r = f2_mul(r2, rinv);
+            f2_t E = one2;
+            if (kap != 0.f) { f2_unpack(r, ra, rb); E = f2_pack(Real<float>::exp_neg(ks, ra), Real<float>::exp_neg(ks, rb)); }
+            f2_t gm = f2_mul(E, rinv);                                                        // F^(0)
+            f2_t acc = f2_mul(gm, q[0]);
+            if (P >= 1) {
+                f2_t g = f2_mul(f2_mul(E, f2_fma(kap2, r, one2)), f2_mul(f2_sub(0, rinv), rinv2));   // F^(1)
+                acc = f2_fma(g, q[1], acc);
+#pragma unroll
+                for (int m = 1; m < P; m++) {
+                    const float cc = -(float)(2 * m + 1);
+                    const f2_t gn = f2_mul(f2_fma(g, f2_pack(cc, cc), f2_mul(k2, gm)), rinv2);
+                    gm = g; g = gn;
+                    acc = f2_fma(g, q[m + 1], acc);
+                }
+            }
+            float va, vb;
+            f2_unpack(acc, va, vb);
+            a0 += (double)va; a1 += (double)vb;
+        }
+        __syncthreads();                                     // buf is refilled two iterations from now
+    }
+    if (ok0) atomicAdd(out + t0, a0);
+    if (ok1) atomicAdd(out + t1, a1);
 }

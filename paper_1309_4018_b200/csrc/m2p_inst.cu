@@ -18,7 +18,14 @@ template <bool TWIN, typename T> static void launch(const M2PArgs &a)
 
 int CAT(pygbe_m2p_launch_, M2P_P)(const M2PArgs &a)
 {
-    if (a.fp32) { if (a.twin) launch<true, float>(a); else launch<false, float>(a); }
+    if (a.fp32 && a.twin) {               // two targets per thread, packed fp32
+        k_m2p_twin2<M2P_P><<<a.n_items, M2P2_THREADS, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo, (const float *)a.wc,
+                                                                  a.kappaA, Real<float>::kscale(a.kappaA), a.kappaB,
+                                                                  Real<float>::kscale(a.kappaB), a.outA, a.outB);
+    } else if (a.fp32) {
+        k_m2p_single2<M2P_P><<<a.n_items, M2P2_THREADS, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo, (const float *)a.wc,
+                                                                    a.kappaA, Real<float>::kscale(a.kappaA), a.outA);
+    }
     else { if (a.twin) launch<true, double>(a); else launch<false, double>(a); }
     return 0;
 }

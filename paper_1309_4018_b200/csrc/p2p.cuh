@@ -149,14 +149,6 @@ k_p2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *
 //   chgq[4 q + {0,1,2,3}] = (mV0..3), (mKx0..3), (mKy0..3), (mKz0..3)   (k_prep, every matvec)
 // Region B's charges are rV mV and -mK: its sum is accumulated as sum (mV + t (1 + kappa r) / rV) w and
 // multiplied by rV once at the end.
-typedef unsigned long long f2_t;                                      // two packed floats
-__device__ __forceinline__ f2_t f2_pack(float lo, float hi) { f2_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ void f2_unpack(f2_t v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
-__device__ __forceinline__ f2_t f2_add(f2_t a, f2_t b) { f2_t r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f2_t f2_sub(f2_t a, f2_t b) { f2_t r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f2_t f2_mul(f2_t a, f2_t b) { f2_t r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f2_t f2_fma(f2_t a, f2_t b, f2_t c) { f2_t r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-
 struct P2PQuadConst {                                                 // loop invariants, already packed
     f2_t nksA, nksB;            // -kappa log2(e) of regions A and B
     f2_t kA;                    // kappa_A
