@@ -189,3 +189,97 @@ k_precond_apply(const int *__restrict__ flags, int respect_done, long npan, cons
     const double z0 = m.x * u0 + m.y * u1, z1 = m.z * u0 + m.w * u1;
     if (add) { z[ix.x] += z0; z[ix.y] += z1; } else { z[ix.x] = z0; z[ix.y] = z1; }
 }
+
+// ---------------------------------------------------------------------------------- fused Arnoldi step
+// One cooperative launch per GMRES iteration instead of nine small ones (zero, dots, axpys, dots, axpys, norm,
+// scale, Givens: ~35 us of launch gaps next to a 0.17 ms matvec at config 1).  Each CTA owns a slice of rows;
+// the phases are separated by grid-wide barriers:
+//   1  h1[i] += V_i . w (slice partials, atomics)                          [h1 is zero on entry]
+//   2  w -= sum_i h1[i] V_i on the slice, then h2[i] += V_i . w            (second Gram-Schmidt pass, CGS2)
+//   3  w -= sum_i h2[i] V_i, nrm2 += |w|^2
+//   4  V_(j+1) = w / sqrt(nrm2) on the slice; one thread: Hessenberg column, Givens, convergence test
+// Same arithmetic as k_gm_dots / k_gm_axpys / k_gm_scale / k_gm_givens; only the summation order of the
+// partials differs (atomics either way, reading A19).
+#include <cooperative_groups.h>
+__global__ void __launch_bounds__(GM_THREADS)
+k_gm_arnoldi(int *flags, double *V, long n, int j, int m, double *w, double *h1, double *h2, double *nrm2, double *H,
+             double *cs, double *sn, double *g, double *scal, double tol)
+{
+    namespace cgx = cooperative_groups;
+    if (flags[0]) return;                                    // uniform: set before this launch or not at all
+    cgx::grid_group grid = cgx::this_grid();
+    typedef cub::BlockReduce<double, GM_THREADS> Red;
+    __shared__ typename Red::TempStorage tmp;
+    const int nvec = j + 1;
+    const long per = (n + gridDim.x - 1) / gridDim.x;
+    const long lo = (long)blockIdx.x * per, hi = min(n, lo + per);
+    double *vn = V + (long)(j + 1) * n;
+    if (blockIdx.x == 0) {
+        for (int i = threadIdx.x; i < nvec; i += GM_THREADS) h2[i] = 0.0;
+        if (threadIdx.x == 0) *nrm2 = 0.0;
+    }
+    // phase 1
+    for (int i = 0; i < nvec; i++) {
+        const double *v = V + (long)i * n;
+        double acc = 0.0;
+        for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) acc += v[r] * w[r];
+        const double s = Red(tmp).Sum(acc);
+        if (threadIdx.x == 0) atomicAdd(h1 + i, s);
+        __syncthreads();
+    }
+    grid.sync();
+    // phase 2
+    for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) {
+        double acc = w[r];
+        for (int i = 0; i < nvec; i++) acc -= __ldcg(h1 + i) * V[(long)i * n + r];
+        w[r] = acc;
+    }
+    __syncthreads();
+    for (int i = 0; i < nvec; i++) {
+        const double *v = V + (long)i * n;
+        double acc = 0.0;
+        for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) acc += v[r] * w[r];
+        const double s = Red(tmp).Sum(acc);
+        if (threadIdx.x == 0) atomicAdd(h2 + i, s);
+        __syncthreads();
+    }
+    grid.sync();
+    // phase 3
+    {
+        double part = 0.0;
+        for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) {
+            double acc = w[r];
+            for (int i = 0; i < nvec; i++) acc -= __ldcg(h2 + i) * V[(long)i * n + r];
+            w[r] = acc;
+            part += acc * acc;
+        }
+        const double s = Red(tmp).Sum(part);
+        if (threadIdx.x == 0) atomicAdd(nrm2, s);
+    }
+    grid.sync();
+    // phase 4
+    const double nn = sqrt(__ldcg(nrm2));
+    for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) vn[r] = nn > 0.0 ? w[r] / nn : 0.0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        double *col = H + (long)j * (m + 1);
+        for (int i = 0; i <= j; i++) col[i] = __ldcg(h1 + i) + __ldcg(h2 + i);
+        col[j + 1] = nn;
+        for (int i = 0; i < j; i++) {
+            double t = cs[i] * col[i] + sn[i] * col[i + 1];
+            col[i + 1] = -sn[i] * col[i] + cs[i] * col[i + 1];
+            col[i] = t;
+        }
+        double d = hypot(col[j], col[j + 1]);
+        double c = d > 0.0 ? col[j] / d : 1.0, s = d > 0.0 ? col[j + 1] / d : 0.0;
+        cs[j] = c; sn[j] = s;
+        col[j] = d; col[j + 1] = 0.0;
+        g[j + 1] = -s * g[j];
+        g[j] = c * g[j];
+        double rel = fabs(g[j + 1]) / scal[0];
+        scal[2] = rel;
+        flags[1] = j + 1;
+        flags[2] += 1;                       // total iterations
+        if (rel <= tol) flags[0] = 1;
+        for (int i = 0; i <= j + 1; i++) h1[i] = 0.0;        // invariant: h1 is zero when the next step starts
+    }
+}

@@ -69,6 +69,13 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
     CUDA_TRY(cudaMemsetAsync(G.flags, 0, 4 * sizeof(int), st));
     CUDA_TRY(cudaMemsetAsync(G.scal, 0, 8 * sizeof(double), st));
     const int poll = n < 200000 ? 4 : 1;
+    int arn_grid = 1;
+    {
+        int occ = 1;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_gm_arnoldi, GM_THREADS, 0));
+        arn_grid = (int)std::max(1L, std::min((long)occ * h->n_sm, (long)cdiv(n, 512)));
+    }
+    CUDA_TRY(cudaMemsetAsync(G.h1, 0, (size_t)(G.m + 2) * sizeof(double), st));   // k_gm_arnoldi keeps h1 zero between steps
     const bool pc = h->precond == 1 && h->pinv != nullptr;
     int total = 0, done = 0;
     bool first = true;
@@ -88,14 +95,13 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
             } else {
                 TRY(matvec_impl(h, vj, G.w, G.flags));
             }
-            LAUNCH(h, k_gm_zero, cdiv(j + 2, 128), 128, 0, G.flags, G.h1, j + 1, G.h2, j + 1, G.scal + 3, 1);
-            LAUNCH(h, k_gm_dots, gridd, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.w, G.h1);
-            LAUNCH(h, k_gm_axpys, gridn, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.h1, G.w);
-            LAUNCH(h, k_gm_dots, gridd, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.w, G.h2);
-            LAUNCH(h, k_gm_axpys, gridn, GM_THREADS, 0, G.flags, G.V, n, j + 1, G.h2, G.w);
-            LAUNCH(h, k_gm_dots, gridd, GM_THREADS, 0, G.flags, G.w, n, 1, G.w, G.scal + 3);
-            LAUNCH(h, k_gm_scale, gridn, GM_THREADS, 0, G.flags, n, G.w, G.scal + 3, 1, vn);
-            LAUNCH(h, k_gm_givens, 1, 1, 0, G.flags, j, G.m, G.h1, G.h2, G.scal + 3, G.H, G.cs, G.sn, G.g, G.scal, tol);
+            {   // one cooperative launch: CGS2, normalisation, Givens, convergence test (gmres.cuh)
+                long nn = n; int jj = j, mm = G.m; double tl = tol;
+                double *nrm2 = G.scal + 3;
+                void *args[] = {&G.flags, &G.V, &nn, &jj, &mm, &G.w, &G.h1, &G.h2, &nrm2, &G.H, &G.cs, &G.sn, &G.g, &G.scal, &tl};
+                CUDA_TRY(cudaLaunchCooperativeKernel((const void *)k_gm_arnoldi, dim3(arn_grid), dim3(GM_THREADS), args, 0, st));
+                h->launches++;
+            }
             if ((j + 1) % poll == 0 || j + 1 == mc) {
                 CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
                 CUDA_TRY(cudaStreamSynchronize(st));
