@@ -66,3 +66,60 @@ def cavity_sphere(q, r_c, R, r_k, eps_in, eps_out, kappa, eps_cav, nmax=60):
         f, b, g, A = np.linalg.solve(M, rhs)
         phi += b * (r_k / R) ** n + g * (r_c / r_k) ** (n + 1)
     return 0.5 * C0 * q * phi
+
+
+def layered_sphere(q, r_k, radii, eps, kappa, charge_layer, nmax=60):
+    """Charge q on the axis at radius r_k inside layer `charge_layer` (kappa = 0 there) of a concentric system:
+    layer 0 is the ball r < radii[0], layer l lies between radii[l-1] and radii[l], the last layer is the
+    exterior.  Layer l has (eps[l], kappa[l]).  Separation of variables of eq. (1): per Legendre order n the
+    potential in layer l is A_l f_l(r) + B_l g_l(r) (+ the Coulomb harmonic in the charge's layer) with
+    (f, g) = (r^n, r^-(n+1)) for kappa = 0 and (i_n(kappa r), k_n(kappa r)) otherwise; B_0 = 0, A_last = 0; phi and
+    eps dphi/dr are continuous at every radius.  Returns the solvation energy 1/2 C0 q phi_reac(r_k)."""
+    from scipy.special import spherical_in
+    radii = [float(a) for a in radii]
+    L = len(radii) + 1
+    assert len(eps) == L and len(kappa) == L and kappa[charge_layer] == 0.0
+    Q = q / (4 * np.pi * eps[charge_layer])
+
+    def basis(l, n, r):
+        """(f, f', g, g') of layer l at r, each pair scaled to O(1) at the layer's reference radius."""
+        ref = radii[min(l, L - 2)]
+        if kappa[l] == 0.0:
+            f, df = (r / ref) ** n, n * (r / ref) ** n / r
+            g, dg = (ref / r) ** (n + 1), -(n + 1) * (ref / r) ** (n + 1) / r
+        else:
+            k = kappa[l]
+            fs, gs = spherical_in(n, k * ref), spherical_kn(n, k * ref)
+            f, df = spherical_in(n, k * r) / fs, k * spherical_in(n, k * r, derivative=True) / fs
+            g, dg = spherical_kn(n, k * r) / gs, k * spherical_kn(n, k * r, derivative=True) / gs
+        return f, df, g, dg
+
+    phi = 0.0
+    for n in range((nmax if r_k > 0 else 0) + 1):
+        # unknown index: A_l -> 2l, B_l -> 2l + 1
+        M = np.zeros((2 * L, 2 * L)); rhs = np.zeros(2 * L)
+        M[0, 1] = 1.0                      # B_0 = 0 (regular at the origin)
+        M[1, 2 * (L - 1)] = 1.0            # A_last = 0 (decays at infinity)
+        row = 2
+        for i, a in enumerate(radii):      # interface between layers i and i + 1
+            fi, dfi, gi, dgi = basis(i, n, a)
+            fo, dfo, go, dgo = basis(i + 1, n, a)
+            M[row, 2 * i], M[row, 2 * i + 1], M[row, 2 * i + 2], M[row, 2 * i + 3] = fi, gi, -fo, -go
+            M[row + 1, 2 * i], M[row + 1, 2 * i + 1] = eps[i] * dfi, eps[i] * dgi
+            M[row + 1, 2 * i + 2], M[row + 1, 2 * i + 3] = -eps[i + 1] * dfo, -eps[i + 1] * dgo
+            if i == charge_layer:          # outer boundary of the charge's layer: Coulomb harmonic Q r_k^n / r^(n+1)
+                c = Q * r_k ** n / a ** (n + 1) if r_k > 0 else (Q / a if n == 0 else 0.0)
+                rhs[row] -= c
+                rhs[row + 1] -= eps[i] * (-(n + 1) * c / a)
+            if i + 1 == charge_layer:      # inner boundary: Q r^n / r_k^(n+1)
+                c = Q * a ** n / r_k ** (n + 1)
+                rhs[row] += c
+                rhs[row + 1] += eps[i + 1] * (n * c / a)
+            row += 2
+        sol = np.linalg.solve(M, rhs)
+        if r_k > 0:
+            f, _, g, _ = basis(charge_layer, n, r_k)
+            phi += sol[2 * charge_layer] * f + sol[2 * charge_layer + 1] * g
+        else:
+            phi += sol[2 * charge_layer]   # f = 1 at the origin for n = 0, g term absent (B_0 = 0)
+    return 0.5 * C0 * q * phi

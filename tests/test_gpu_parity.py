@@ -240,6 +240,33 @@ def test_mixed_precision_other_orders(env, maker, level):
         h64.close(); h32.close()
 
 
+def test_nested_cavity_with_salt(env):
+    """Five regions, four nested surfaces, a Yukawa region at the centre (workloads.nested_sphere_problem; closed
+    form pinned on the oracle in test_oracle_pins.py): direct parity, treecode parity in both precisions, energy."""
+    pg, torch, orc = env
+    prob = W.nested_sphere_problem(2)
+    o = orc.Oracle(prob)
+    x = np.random.default_rng(31).normal(size=o.n)
+    yo = o.matvec(x)
+    h, y = gpu_matvec(pg, torch, prob, x, K=4, theta=0.0)
+    assert rel(y, yo) <= TOL_DIRECT
+    assert rel(h.rhs().cpu().numpy(), o.rhs()) <= 1e-13
+    xs, it, rr, rc = h.solve(tol=1e-9, max_iter=2000)
+    xo, _, _ = o.solve(tol=1e-9)
+    es, _ = h.energy(xs)
+    assert abs(es - o.solvation_energy(xo)) / abs(o.solvation_energy(xo)) < 1e-6
+    h.close()
+    prob3 = W.nested_sphere_problem(3)
+    o3 = orc.Oracle(prob3)
+    x3 = np.random.default_rng(32).normal(size=o3.n)
+    yo3 = o3.matvec(x3)
+    for prec in (pg.PRECISION_FP64, pg.PRECISION_MIXED):
+        h, y = gpu_matvec(pg, torch, prob3, x3, K=4, P=6, theta=0.5, ncrit=16, precision=prec)
+        assert h.stats()["m2p_evals"] > 0
+        assert rel(y, yo3) <= TOL_TREE
+        h.close()
+
+
 @pytest.mark.parametrize("ncrit", [8, 40, 500])
 def test_treecode_leaf_sizes(env, ncrit):
     pg, torch, orc = env

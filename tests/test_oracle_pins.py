@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 import workloads as W
-from closed_forms import C0, born, kirkwood, stern_sphere, cavity_sphere
+from closed_forms import C0, born, kirkwood, stern_sphere, cavity_sphere, layered_sphere
 
 
 @pytest.fixture(scope="module")
@@ -279,6 +279,34 @@ def test_cavity_analytic(orc):
         x, it, rel = o.solve(tol=1e-10)
         E[lvl] = o.solvation_energy(x)
     assert abs(E[2] - exact) / abs(exact) < 0.04
+    assert abs(_richardson(E[2], E[1]) - exact) / abs(exact) < 5e-3
+
+
+def test_layered_closed_form_reduces_to_the_special_cases():
+    """The general concentric-layer solution (any number of layers, Laplace or Yukawa each) against the four
+    special cases derived separately above."""
+    assert abs(layered_sphere(1, 0.0, [4], [4, 80], [0, 0.125], 0) - born(1, 4, 4, 80, 0.125)) < 1e-10
+    assert abs(layered_sphere(1, 0.0, [4, 6], [4, 80, 80], [0, 0, 0.125], 0) - stern_sphere(1, 4, 6, 4, 80, 0.125)) < 1e-10
+    assert abs(layered_sphere(1, 5.0, [2, 8], [80, 4, 80], [0, 0, 0.125], 1) - cavity_sphere(1, 2, 8, 5, 4, 80, 0.125, 80)) < 1e-9
+    assert abs(layered_sphere(1, 3.0, [10], [4, 80], [0, 0.125], 0) - kirkwood([[0, 0, 3.0]], [1.0], 10, 4, 80, 0.125)) < 1e-9
+
+
+def test_nested_ion_bearing_cavity_analytic(orc):
+    """PAPER.md:131 "cavities ... large enough to contain ions ... an interior Stern layer": a cavity with salt
+    (Yukawa, regular at the origin) inside its own Stern layer inside the protein shell inside an outer Stern
+    layer inside the salt solvent; five regions, four surfaces, charge in the shell: -39.694277 kJ/mol.  Pins the
+    per-region rule of reading A4 for a Yukawa region that is the *inside* of its only surface and for a Laplace
+    region bounded on both sides by solvent-like media."""
+    exact = layered_sphere(1, 5.0, [1.5, 2.5, 8, 10], [80, 80, 4, 80, 80], [0.5, 0, 0, 0, 0.125], 2)
+    assert abs(exact - (-39.694277)) < 1e-6
+    # the salt in the cavity matters: the same geometry with pure water inside differs by 6 %
+    assert abs(layered_sphere(1, 5.0, [1.5, 2.5, 8, 10], [80, 80, 4, 80, 80], [0.0, 0, 0, 0, 0.125], 2) - exact) / abs(exact) > 0.05
+    E = {}
+    for lvl in (1, 2):
+        o = orc.Oracle(W.nested_sphere_problem(lvl))
+        x, it, rel = o.solve(tol=1e-10)
+        E[lvl] = o.solvation_energy(x)
+    assert abs(E[2] - exact) / abs(exact) < 0.02
     assert abs(_richardson(E[2], E[1]) - exact) / abs(exact) < 5e-3
 
 

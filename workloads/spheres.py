@@ -115,3 +115,23 @@ def cavity_sphere_problem(level=2, r_cav=2.0, r_out=8.0, r_charge=5.0, eps_in=4.
                    [eps_in, eps_out, eps_cav], [0.0, kappa, 0.0],
                    [[0.0, 0.0, r_charge]], [q], [0], name=f"cavity_l{level}",
                    meta=dict(r_cav=r_cav, r_out=r_out, r_charge=r_charge, level=level))
+
+
+def nested_sphere_problem(level=2, radii=(1.5, 2.5, 8.0, 10.0), r_charge=5.0, eps_in=4.0, eps_out=80.0,
+                          kappa_cav=0.5, kappa=0.125, q=1.0):
+    """An ion-bearing cavity with its own Stern layer inside a protein shell with an outer Stern layer
+    ("cavities ... large enough to contain ions ... an interior Stern layer"), all concentric:
+        r < radii[0]            region 4: cavity solvent with salt (eps_out, kappa_cav)
+        radii[0] < r < radii[1] region 3: cavity Stern layer (eps_out, 0)
+        radii[1] < r < radii[2] region 0: protein (eps_in, 0), charge on the z axis at r_charge
+        radii[2] < r < radii[3] region 1: outer Stern layer (eps_out, 0)
+        r > radii[3]            region 2: solvent with salt (eps_out, kappa)
+    Four surfaces, every normal pointing away from the centre (region_in = the inner side)."""
+    a0, a1, a2, a3 = radii
+    s0 = Surface(*icosphere(level, a0), 4, 3)
+    s1 = Surface(*icosphere(level, a1), 3, 0)
+    s2 = Surface(*icosphere(level, a2), 0, 1)
+    s3 = Surface(*icosphere(level, a3), 1, 2)
+    return Problem([s0, s1, s2, s3], [eps_in, eps_out, eps_out, eps_out, eps_out], [0.0, 0.0, kappa, 0.0, kappa_cav],
+                   [[0.0, 0.0, r_charge]], [q], [0], name=f"nested_l{level}",
+                   meta=dict(radii=tuple(radii), r_charge=r_charge, level=level))
