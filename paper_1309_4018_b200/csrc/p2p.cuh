@@ -195,7 +195,10 @@ __device__ __forceinline__ void p2p_pair2(f2_t X, f2_t Y, f2_t Z, f2_t px, f2_t 
 
 #define P2P_QTILE (P2P_TILE / 4)                                       // quads per tile
 template <bool YA, bool TWIN, bool YB>
-__global__ void __launch_bounds__(PYGBE_TG)
+#ifndef P2PQ_MINB
+#define P2PQ_MINB 1
+#endif
+__global__ void __launch_bounds__(PYGBE_TG, P2PQ_MINB)
 k_p2p_quad(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *__restrict__ tiles, int np,
            const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const float4 *__restrict__ posq,
            const float4 *__restrict__ chgq, double kappaA, double kappaB, double rV, double *__restrict__ outA,
