@@ -260,6 +260,31 @@ def test_mixed_precision_other_gauss_rules(env, K):
     h.close()
 
 
+@pytest.mark.parametrize("maker,level", [(W.kirkwood_problem, 4), (W.nested_sphere_problem, 3)])
+def test_repeated_matvecs_agree(env, maker, level):
+    """The single-launch upward pass hands cells between CTAs through tickets and ready flags (csrc/farfield.cuh)
+    and three streams meet at the block combination: 40 back-to-back matvecs of the same vector, queued without
+    host synchronisation, must agree to summation-order noise, and a different vector in between must not leak."""
+    pg, torch, orc = env
+    prob = maker(level)
+    for prec in (pg.PRECISION_FP64, pg.PRECISION_MIXED):
+        h = pg.Handle.from_problem(prob, K=4, P=6, theta=0.5, ncrit=16, precision=prec)
+        rng = np.random.default_rng(77)
+        x = torch.tensor(rng.normal(size=h.n), device="cuda")
+        z = torch.tensor(rng.normal(size=h.n), device="cuda")
+        ys = [torch.empty_like(x) for _ in range(40)]
+        scratch = torch.empty_like(x)
+        for i, y in enumerate(ys):
+            h.matvec(x, y)
+            if i % 7 == 3:
+                h.matvec(z, scratch)
+        torch.cuda.synchronize()
+        y0 = ys[0].cpu().numpy()
+        for y in ys[1:]:                                         # only the order of the fp64 atomic adds varies
+            assert rel(y.cpu().numpy(), y0) < 1e-12
+        h.close()
+
+
 def test_nested_cavity_with_salt(env):
     """Five regions, four nested surfaces, a Yukawa region at the centre (workloads.nested_sphere_problem; closed
     form pinned on the oracle in test_oracle_pins.py): direct parity, treecode parity in both precisions, energy."""
