@@ -180,33 +180,74 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
 
     // ---- work items of bounded size, enough of them to fill 148 SMs several times over
     const long want_items = 148L * 16;
-    int p2p_item = (int)std::min(512L, std::max(32L, total_src_panels / want_items));
     // M2P CTAs keep only 8-16 warps per SM resident (72-127 registers): finer items even out the tail
     int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[R.ng] / (3 * want_items)));
     m2p_item = (m2p_item + 3) / 4 * 4;
-    // P2P items are runs of source tiles: (first point, points <= P2P_TILE, anchor cell, 0), whole panels only
+    // P2P tiles gather up to P2P_TILE source points from several panel ranges of one anchor cell: a group's near
+    // field is ~30 short runs of Morton-consecutive panels (one or two leaves each), and tiles cut range by range
+    // were 62 % full with a third of them under a quarter (config 1).  tile = (first segment, last segment + 1,
+    // anchor cell, 2 * points + self flag), segment = (first point, points), whole panels only; self flag = the
+    // tile holds panels of the group's own targets, the only place where a pair at zero distance can occur
+    // (reading A5).
     const int tile_panels = std::max(1, P2P_TILE / K);
     std::vector<int4> sub, pitems, mitems;
+    std::vector<int> gtile(R.ng + 1, 0);                           // first tile of each group
+    std::vector<int2> segs;
+    std::vector<int4> grng;
     for (int g = 0; g < R.ng; g++) {
-        int first = (int)sub.size(), acc = 0;
-        for (int r = poff2[g]; r < poff2[g + 1]; r++) {
-            int a = prng[r].x;
-            while (a < prng[r].y) {
-                int take = std::min(prng[r].y - a, p2p_item - acc);
-                for (int b = a; b < a + take; b += tile_panels) {
-                    const int nb = std::min(tile_panels, a + take - b);
-                    sub.push_back(make_int4(b * K, nb * K, prng[r].z, 0));
+        grng.assign(prng.begin() + poff2[g], prng.begin() + poff2[g + 1]);
+        std::stable_sort(grng.begin(), grng.end(), [](const int4 &a, const int4 &b) { return a.z < b.z; });
+        const int own_lo = g * PYGBE_TG, own_hi = std::min(R.np, own_lo + PYGBE_TG);
+        const size_t tile0 = sub.size();
+        long src = 0;
+        int fill = 0;                                              // panels in the open tile (sub.back())
+        for (size_t r = 0; r < grng.size(); r++) {
+            if (r > 0 && grng[r].z != grng[r - 1].z) fill = 0;     // another anchor: close the tile
+            int a = grng[r].x;
+            while (a < grng[r].y) {
+                if (fill == 0 || fill == tile_panels) {
+                    sub.push_back(make_int4((int)segs.size(), (int)segs.size(), grng[r].z, 0));
+                    fill = 0;
                 }
-                a += take; acc += take;
-                if (acc == p2p_item) { pitems.push_back(make_int4(g, first, (int)sub.size(), 0)); first = (int)sub.size(); acc = 0; }
+                const int take = std::min(grng[r].y - a, tile_panels - fill);
+                segs.push_back(make_int2(a * K, take * K));
+                int4 &t = sub.back();
+                t.y = (int)segs.size();
+                t.w += 2 * take * K;
+                if (a < own_hi && a + take > own_lo) t.w |= 1;
+                a += take; fill += take; src += take;
             }
         }
-        if (acc > 0) pitems.push_back(make_int4(g, first, (int)sub.size(), 0));
+        gtile[g + 1] = (int)sub.size();
         for (int s = moff[g]; s < moff[g + 1]; s += m2p_item)
             mitems.push_back(make_int4(g, s, std::min(s + m2p_item, moff[g + 1]), 0));
     }
+    // items = short runs of a group's tiles.  An SM holds ~12 of these CTAs, which share its pipes, so an item of n
+    // tiles lasts about n / 1100 of the whole launch at config 1 (13 k tiles): equal items of 5 tiles left a tail
+    // of a fifth of the kernel, single tiles none (the double buffer then only hides the first tile's latency
+    // behind other CTAs).  Large problems take longer runs to save the per-item target loads and atomics.
+    {
+        const long slots = 148L * 12;
+        int per_item = (int)std::min(8L, std::max(1L, (long)sub.size() / (slots * 24)));
+        if (const char *e = getenv("PYGBE_P2P_ITEM_TILES")) per_item = std::max(1, atoi(e));      // tuning
+        for (int g = 0; g < R.ng; g++)
+            for (int t = gtile[g]; t < gtile[g + 1]; t += per_item) {
+                const int n = std::min(per_item, gtile[g + 1] - t);
+                int acc = 0;
+                for (int u = 0; u < n; u++) acc += (sub[t + u].w >> 1) / K;
+                pitems.push_back(make_int4(g, t, t + n, acc));
+            }
+    }
+    if (getenv("PYGBE_DEBUG")) {
+        long pts = 0, selft = 0; int hist[9] = {0};
+        for (auto &t : sub) { pts += t.w >> 1; selft += t.w & 1; hist[std::min(8, (t.w >> 1) * 8 / P2P_TILE)]++; }
+        fprintf(stderr, "[pygbe] region: groups %d ranges %zu items %zu tiles %zu fill %.3f self tiles %ld; tile fill hist:",
+                R.ng, prng.size(), pitems.size(), sub.size(), (double)pts / (sub.size() * (double)P2P_TILE), selft);
+        for (int i = 0; i < 9; i++) fprintf(stderr, " %d", hist[i]);
+        fprintf(stderr, "\n");
+    }
     R.n_p2p_items = (int)pitems.size(); R.n_m2p_items = (int)mitems.size();
-    TRY(upload(h, &R.p2p_sub, sub)); TRY(upload(h, &R.p2p_items, pitems)); TRY(upload(h, &R.m2p_items, mitems));
+    TRY(upload(h, &R.p2p_sub, sub)); TRY(upload(h, &R.p2p_seg, segs)); TRY(upload(h, &R.p2p_items, pitems)); TRY(upload(h, &R.m2p_items, mitems));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     return PYGBE_OK;
 }

@@ -141,8 +141,9 @@ struct Region {
     int *p2p_off = nullptr;
     int4 *p2p_rng = nullptr;        // merged source panel ranges (lo, hi, anchor cell, -)
     int n_p2p_items = 0, n_m2p_items = 0;
-    int4 *p2p_items = nullptr;      // (group, first range, last range+1, unused) over p2p_sub
-    int4 *p2p_sub = nullptr;        // chunked panel ranges (lo, hi, anchor cell, -)
+    int4 *p2p_items = nullptr;      // (group, first tile, last tile + 1, source panels) over p2p_sub
+    int4 *p2p_sub = nullptr;        // tiles: (first segment, last segment + 1, anchor cell, 2 * points + self flag)
+    int2 *p2p_seg = nullptr;        // segments of the tiles: (first point, points), whole panels
     int4 *m2p_items = nullptr;      // (group, first list slot, last slot+1, unused)
     long p2p_pairs = 0, m2p_evals = 0;
     // multipoles ------------------------------------------------------------------------------------

@@ -60,10 +60,10 @@ static void launch_p2p(pygbe_handle *h, Region &A, Region *B, const int *skip)
     const bool quad = sizeof(T) == 4 && A.quad;
 #define P2P_GO(YA, TW, YB)                                                                                     \
     do { if (quad) { auto kern = k_p2p_quad<YA, TW, YB>;                                                       \
-             LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, A.np, A.tpos, A.cgeo,   \
+             LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, A.p2p_seg, A.np, A.tpos, A.cgeo, \
                     (const float4 *)A.sposf, (const float4 *)A.schgf, kA, kB, rV, oA, oB); }                   \
          else { auto kern = k_p2p<T, YA, TW, YB>;                                                              \
-             LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, A.np, A.tpos,           \
+             LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, A.p2p_seg, A.np, A.tpos, \
                     A.cgeo, pos, chg, kA, kB, rV, oA, oB); } } while (0)
     if (!B) { if (A.yukawa) P2P_GO(true, false, false); else P2P_GO(false, false, false); }
     else if (A.yukawa) { if (B->yukawa) P2P_GO(true, true, true); else P2P_GO(true, true, false); }

@@ -19,7 +19,9 @@
 #include "mathx.cuh"
 #include "m2p.cuh"       // cp_async helpers
 
+#ifndef P2P_TILE
 #define P2P_TILE 128
+#endif
 
 // fp32 source coordinates relative to the centre of the panel's anchor cell (create time, mixed precision).
 // The subtraction is done in fp64 and rounded once, exactly as the kernel re-bases the targets, so the
@@ -62,8 +64,9 @@ __device__ __forceinline__ void p2p_pair(T dx, T dy, T dz, T mV, T mKx, T mKy, T
     }
 }
 
-// Work item = (target group, a run of source tiles).  tile = (first point, number of points <= P2P_TILE,
-// anchor cell, -): for T = float the stored source coordinates are relative to the anchor cell's centre and
+// Work item = (target group, a run of source tiles).  tile = (first segment, last segment + 1, anchor cell,
+// 2 * points + self flag), segment = (first point, points): the <= P2P_TILE points of a tile are gathered from
+// several runs of Morton-consecutive panels of one anchor cell (build_lists.cuh).  For T = float the stored source coordinates are relative to the anchor cell's centre and
 // the target is re-based per tile in fp64 (3 subtractions per thread per tile), so every fp32 difference is
 // between numbers of the size of a cell, not of the molecule.  Tiles are double-buffered with cp.async
 // (LDGSTS): while the threads sum one tile, the points, weights and anchor centre of the next stream into
@@ -71,7 +74,8 @@ __device__ __forceinline__ void p2p_pair(T dx, T dy, T dz, T mV, T mKx, T mKy, T
 // each tile synchronously: 16 % wait + 9 % scoreboard stalls, profiles/r1b_mixed_path.md).
 template <typename T, bool YA, bool TWIN, bool YB>
 __global__ void __launch_bounds__(PYGBE_TG)
-k_p2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *__restrict__ tiles, int np,
+k_p2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *__restrict__ tiles,
+      const int2 *__restrict__ segs, int np,
       const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo,
       const typename Real<T>::vec4 *__restrict__ pos, const typename Real<T>::vec4 *__restrict__ chg,
       double kappaA, double kappaB, double rV, double *__restrict__ outA, double *__restrict__ outB)
@@ -89,10 +93,20 @@ k_p2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *
     const T kA = (T)kappaA, kB = (T)kappaB, ksA = (T)Real<T>::kscale(kappaA), ksB = (T)Real<T>::kscale(kappaB);
     const T rv = (T)rV;
     double accA = 0.0, accB = 0.0;
-    auto stage = [&](int buf, const int4 &tl) {
-        for (int i = threadIdx.x; i < tl.y * V4C; i += PYGBE_TG) {
-            cp_async16((char *)s_pos[buf] + 16 * i, (const char *)(pos + tl.x) + 16 * i);
-            cp_async16((char *)s_chg[buf] + 16 * i, (const char *)(chg + tl.x) + 16 * i);
+    auto stage = [&](int buf, const int4 &tl) {                      // gather the tile's segments into consecutive slots
+        const int lane = threadIdx.x & 31;
+        int off = 0;                                                 // points staged so far
+        for (int s0 = tl.x; s0 < tl.y; s0 += 32) {
+            const int ns = min(32, tl.y - s0);
+            const int2 mine = lane < ns ? segs[s0 + lane] : make_int2(0, 0);
+            for (int s = 0; s < ns; s++) {
+                const int p0 = __shfl_sync(0xffffffffu, mine.x, s), c = __shfl_sync(0xffffffffu, mine.y, s) * V4C;
+                for (int i = threadIdx.x; i < 2 * c; i += PYGBE_TG) {
+                    if (i < c) cp_async16((char *)(s_pos[buf] + off) + 16 * i, (const char *)(pos + p0) + 16 * i);
+                    else cp_async16((char *)(s_chg[buf] + off) + 16 * (i - c), (const char *)(chg + p0) + 16 * (i - c));
+                }
+                off += c / V4C;
+            }
         }
         if (sizeof(T) == 4 && threadIdx.x < 2)
             cp_async16((char *)&s_an[buf] + 16 * threadIdx.x, (const char *)(cgeo + tl.z) + 16 * threadIdx.x);
@@ -105,7 +119,7 @@ k_p2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *
     for (int k = it.y; k < it.z; k++, buf ^= 1) {
         const bool more = k + 1 < it.z;
         if (more) { stage(buf ^ 1, nxt); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
-        const int n = cur.y;
+        const int n = cur.w >> 1;
         cur = nxt;
         if (k + 2 < it.z) nxt = tiles[k + 2];
         __syncthreads();
@@ -153,19 +167,25 @@ struct P2PQuadConst {                                                 // loop in
     f2_t nksA, nksB;            // -kappa log2(e) of regions A and B
     f2_t kA;                    // kappa_A
     f2_t sB, cB;                // 1 / rV and kappa_B / rV
+    f2_t tiny;                  // floor of r^2 in the unguarded tiles
 };
 
-// two source points (packed) against one target
-template <bool YA, bool TWIN, bool YB>
+// two source points (packed) against one target.  GUARD: the tile holds panels of the group's own targets, a
+// pair can be at zero distance (reading A5) and must contribute nothing -> select on r^2 > 0 (two scalar ALU
+// instructions per pair).  Every other tile takes the unguarded form: r^2 carries a 1e-30 floor inside its
+// first FMA (free, far below one ulp of any real r^2), so that points of a degenerate mesh that coincide after
+// rounding give a finite value instead of a NaN.
+template <bool YA, bool TWIN, bool YB, bool GUARD>
 __device__ __forceinline__ void p2p_pair2(f2_t X, f2_t Y, f2_t Z, f2_t px, f2_t py, f2_t pz, f2_t mV, f2_t mKx, f2_t mKy,
                                           f2_t mKz, const P2PQuadConst &k, f2_t &accA, f2_t &accB)
 {
     const f2_t dx = f2_sub(X, px), dy = f2_sub(Y, py), dz = f2_sub(Z, pz);
-    const f2_t r2 = f2_fma(dz, dz, f2_fma(dy, dy, f2_mul(dx, dx)));
+    const f2_t r2 = f2_fma(dz, dz, f2_fma(dy, dy, GUARD ? f2_mul(dx, dx) : f2_fma(dx, dx, k.tiny)));
     const f2_t mKd = f2_fma(mKz, dz, f2_fma(mKy, dy, f2_mul(mKx, dx)));
-    float r2a, r2b;
+    float r2a, r2b, ia, ib;
     f2_unpack(r2, r2a, r2b);
-    const float ia = r2a > 0.f ? Real<float>::rsqrt_(r2a) : 0.f, ib = r2b > 0.f ? Real<float>::rsqrt_(r2b) : 0.f;
+    if constexpr (GUARD) { ia = r2a > 0.f ? Real<float>::rsqrt_(r2a) : 0.f; ib = r2b > 0.f ? Real<float>::rsqrt_(r2b) : 0.f; }
+    else { ia = Real<float>::rsqrt_(r2a); ib = Real<float>::rsqrt_(r2b); }
     const f2_t rinv = f2_pack(ia, ib);
     const f2_t t = f2_mul(mKd, f2_mul(rinv, rinv));
     const f2_t r = f2_mul(r2, rinv);
@@ -193,13 +213,30 @@ __device__ __forceinline__ void p2p_pair2(f2_t X, f2_t Y, f2_t Z, f2_t px, f2_t 
     }
 }
 
+// one staged tile of nq quads against one target
+template <bool YA, bool TWIN, bool YB, bool GUARD>
+__device__ __forceinline__ void p2p_quad_tile(const float4 *__restrict__ sp, const float4 *__restrict__ sc, int nq, f2_t X2,
+                                              f2_t Y2, f2_t Z2, const P2PQuadConst &kc, f2_t &a0, f2_t &a1, f2_t &b0, f2_t &b1)
+{
+#pragma unroll 2
+    for (int q = 0; q < nq; q++) {
+        const float4 px = sp[3 * q], py = sp[3 * q + 1], pz = sp[3 * q + 2];
+        const float4 mV = sc[4 * q], mKx = sc[4 * q + 1], mKy = sc[4 * q + 2], mKz = sc[4 * q + 3];
+        p2p_pair2<YA, TWIN, YB, GUARD>(X2, Y2, Z2, f2_pack(px.x, px.y), f2_pack(py.x, py.y), f2_pack(pz.x, pz.y), f2_pack(mV.x, mV.y),
+                                       f2_pack(mKx.x, mKx.y), f2_pack(mKy.x, mKy.y), f2_pack(mKz.x, mKz.y), kc, a0, b0);
+        p2p_pair2<YA, TWIN, YB, GUARD>(X2, Y2, Z2, f2_pack(px.z, px.w), f2_pack(py.z, py.w), f2_pack(pz.z, pz.w), f2_pack(mV.z, mV.w),
+                                       f2_pack(mKx.z, mKx.w), f2_pack(mKy.z, mKy.w), f2_pack(mKz.z, mKz.w), kc, a1, b1);
+    }
+}
+
 #define P2P_QTILE (P2P_TILE / 4)                                       // quads per tile
 template <bool YA, bool TWIN, bool YB>
 #ifndef P2PQ_MINB
-#define P2PQ_MINB 1
+#define P2PQ_MINB 12                                                  // 80 registers: 12 CTAs per SM (uncapped: 114 / 8)
 #endif
 __global__ void __launch_bounds__(PYGBE_TG, P2PQ_MINB)
-k_p2p_quad(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *__restrict__ tiles, int np,
+k_p2p_quad(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *__restrict__ tiles,
+           const int2 *__restrict__ segs, int np,
            const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const float4 *__restrict__ posq,
            const float4 *__restrict__ chgq, double kappaA, double kappaB, double rV, double *__restrict__ outA,
            double *__restrict__ outB)
@@ -217,12 +254,24 @@ k_p2p_quad(const int *__restrict__ skip, const int4 *__restrict__ items, const i
         const float a = -(float)Real<float>::kscale(kappaA), b = -(float)Real<float>::kscale(kappaB);
         const float s = (float)(1.0 / rV), c = (float)(kappaB / rV), ka = (float)kappaA;
         kc.nksA = f2_pack(a, a); kc.nksB = f2_pack(b, b); kc.kA = f2_pack(ka, ka); kc.sB = f2_pack(s, s); kc.cB = f2_pack(c, c);
+        kc.tiny = f2_pack(1e-30f, 1e-30f);
     }
     double accA = 0.0, accB = 0.0;
-    auto stage = [&](int buf, const int4 &tl) {                      // tl = (first point, points, anchor, -), both multiples of 4
-        const int q0 = tl.x >> 2, nq = tl.y >> 2;
-        for (int i = threadIdx.x; i < 3 * nq; i += PYGBE_TG) cp_async16(&s_pos[buf][i], posq + 3 * (long)q0 + i);
-        for (int i = threadIdx.x; i < 4 * nq; i += PYGBE_TG) cp_async16(&s_chg[buf][i], chgq + 4 * (long)q0 + i);
+    auto stage = [&](int buf, const int4 &tl) {                      // segments = (first point, points), multiples of 4
+        const int lane = threadIdx.x & 31;
+        int qoff = 0;                                                // quads staged so far
+        for (int s0 = tl.x; s0 < tl.y; s0 += 32) {
+            const int ns = min(32, tl.y - s0);
+            const int2 mine = lane < ns ? segs[s0 + lane] : make_int2(0, 0);
+            for (int s = 0; s < ns; s++) {
+                const int q0 = __shfl_sync(0xffffffffu, mine.x, s) >> 2, nq = __shfl_sync(0xffffffffu, mine.y, s) >> 2;
+                for (int i = threadIdx.x; i < 7 * nq; i += PYGBE_TG) {
+                    if (i < 3 * nq) cp_async16(&s_pos[buf][3 * qoff + i], posq + 3 * (long)q0 + i);
+                    else cp_async16(&s_chg[buf][4 * qoff + i - 3 * nq], chgq + 4 * (long)q0 + i - 3 * nq);
+                }
+                qoff += nq;
+            }
+        }
         if (threadIdx.x < 2)
             cp_async16((char *)&s_an[buf] + 16 * threadIdx.x, (const char *)(cgeo + tl.z) + 16 * threadIdx.x);
         cp_async_commit();
@@ -234,7 +283,8 @@ k_p2p_quad(const int *__restrict__ skip, const int4 *__restrict__ items, const i
     for (int k = it.y; k < it.z; k++, buf ^= 1) {
         const bool more = k + 1 < it.z;
         if (more) { stage(buf ^ 1, nxt); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
-        const int nq = cur.y >> 2;
+        const int nq = cur.w >> 3;
+        const bool self = (cur.w & 1) != 0;
         cur = nxt;
         if (k + 2 < it.z) nxt = tiles[k + 2];
         __syncthreads();
@@ -243,15 +293,8 @@ k_p2p_quad(const int *__restrict__ skip, const int4 *__restrict__ items, const i
         const f2_t X2 = f2_pack(x, x), Y2 = f2_pack(y, y), Z2 = f2_pack(z, z);
         const float4 *sp = s_pos[buf], *sc = s_chg[buf];
         f2_t a0 = 0, a1 = 0, b0 = 0, b1 = 0;                          // (+0.f, +0.f)
-#pragma unroll 2
-        for (int q = 0; q < nq; q++) {
-            const float4 px = sp[3 * q], py = sp[3 * q + 1], pz = sp[3 * q + 2];
-            const float4 mV = sc[4 * q], mKx = sc[4 * q + 1], mKy = sc[4 * q + 2], mKz = sc[4 * q + 3];
-            p2p_pair2<YA, TWIN, YB>(X2, Y2, Z2, f2_pack(px.x, px.y), f2_pack(py.x, py.y), f2_pack(pz.x, pz.y), f2_pack(mV.x, mV.y),
-                                    f2_pack(mKx.x, mKx.y), f2_pack(mKy.x, mKy.y), f2_pack(mKz.x, mKz.y), kc, a0, b0);
-            p2p_pair2<YA, TWIN, YB>(X2, Y2, Z2, f2_pack(px.z, px.w), f2_pack(py.z, py.w), f2_pack(pz.z, pz.w), f2_pack(mV.z, mV.w),
-                                    f2_pack(mKx.z, mKx.w), f2_pack(mKy.z, mKy.w), f2_pack(mKz.z, mKz.w), kc, a1, b1);
-        }
+        if (self) p2p_quad_tile<YA, TWIN, YB, true>(sp, sc, nq, X2, Y2, Z2, kc, a0, a1, b0, b1);     // uniform over the CTA
+        else p2p_quad_tile<YA, TWIN, YB, false>(sp, sc, nq, X2, Y2, Z2, kc, a0, a1, b0, b1);
         float lo, hi;
         f2_unpack(f2_add(a0, a1), lo, hi);
         accA += (double)(lo + hi);
