@@ -180,9 +180,11 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
 
     // ---- work items of bounded size, enough of them to fill 148 SMs several times over
     const long want_items = 148L * 16;
-    // M2P CTAs keep only 8-16 warps per SM resident (72-127 registers): finer items even out the tail
-    int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[R.ng] / (3 * want_items)));
+    // M2P CTAs keep only 8-20 warps per SM resident (72-127 registers): finer items even out the tail (config 1:
+    // 4 cells per item 0.057 ms, 8 cells 0.060, 16 cells 0.068)
+    int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[R.ng] / (6 * want_items)));
     m2p_item = (m2p_item + 3) / 4 * 4;
+    if (const char *e = getenv("PYGBE_M2P_ITEM")) m2p_item = std::max(1, atoi(e));                 // tuning
     // P2P tiles gather up to P2P_TILE source points from several panel ranges of one anchor cell: a group's near
     // field is ~30 short runs of Morton-consecutive panels (one or two leaves each), and tiles cut range by range
     // were 62 % full with a third of them under a quarter (config 1).  tile = (first segment, last segment + 1,

@@ -11,6 +11,7 @@
 
 #define GM_THREADS 256
 #define GM_ROWS_PER_CTA 2048
+#define GM_MAXVEC 256              // Gram-Schmidt coefficients staged in shared memory per pass of k_gm_arnoldi
 
 // out[i] += V_i . w for i < nvec (out pre-zeroed); V row-major [nvec][n].
 __global__ void __launch_bounds__(GM_THREADS)
@@ -218,41 +219,60 @@ k_gm_arnoldi(int *flags, double *V, long n, int j, int m, double *w, double *h1,
         for (int i = threadIdx.x; i < nvec; i += GM_THREADS) h2[i] = 0.0;
         if (threadIdx.x == 0) *nrm2 = 0.0;
     }
+    // The dots of a slice are spread over the warps (warp k takes V_k, V_(k+8), ...; lanes stride over the rows,
+    // one shuffle reduction and one atomic per vector) instead of one block reduction with two CTA barriers per
+    // vector, which made the step grow by 2.7 us per basis vector (profiles/r2b_launches.csv: 14 ... 50 us).
+    __shared__ double s_h[GM_MAXVEC];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    auto slice_dots = [&](double *hout) {
+        for (int i = warp; i < nvec; i += GM_THREADS / 32) {
+            const double *v = V + (long)i * n;
+            double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+            long r = lo + lane;
+            for (; r + 96 < hi; r += 128) {
+                a0 += v[r] * w[r]; a1 += v[r + 32] * w[r + 32]; a2 += v[r + 64] * w[r + 64]; a3 += v[r + 96] * w[r + 96];
+            }
+            for (; r < hi; r += 32) a0 += v[r] * w[r];
+            double acc = (a0 + a1) + (a2 + a3);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            if (lane == 0) atomicAdd(hout + i, acc);
+        }
+    };
+    auto slice_update = [&](const double *hin, bool want_norm) {   // w -= sum_i hin[i] V_i on the slice
+        double part = 0.0;
+        for (int i0 = 0; i0 < nvec; i0 += GM_MAXVEC) {             // coefficients through shared memory, GM_MAXVEC at a time
+            const int nv = min(GM_MAXVEC, nvec - i0);
+            for (int i = threadIdx.x; i < nv; i += GM_THREADS) s_h[i] = __ldcg(hin + i0 + i);
+            __syncthreads();
+            const double *Vb = V + (long)i0 * n;
+            const bool last = i0 + nv == nvec;
+            for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) {
+                double a0 = w[r], a1 = 0.0, a2 = 0.0, a3 = 0.0;
+                int i = 0;
+                for (; i + 3 < nv; i += 4) {
+                    a0 -= s_h[i] * Vb[(long)i * n + r]; a1 -= s_h[i + 1] * Vb[(long)(i + 1) * n + r];
+                    a2 -= s_h[i + 2] * Vb[(long)(i + 2) * n + r]; a3 -= s_h[i + 3] * Vb[(long)(i + 3) * n + r];
+                }
+                for (; i < nv; i++) a0 -= s_h[i] * Vb[(long)i * n + r];
+                const double acc = (a0 + a1) + (a2 + a3);
+                w[r] = acc;
+                if (last) part += acc * acc;
+            }
+            __syncthreads();                                 // the slice of w is complete, s_h may be rewritten
+        }
+        return want_norm ? part : 0.0;
+    };
     // phase 1
-    for (int i = 0; i < nvec; i++) {
-        const double *v = V + (long)i * n;
-        double acc = 0.0;
-        for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) acc += v[r] * w[r];
-        const double s = Red(tmp).Sum(acc);
-        if (threadIdx.x == 0) atomicAdd(h1 + i, s);
-        __syncthreads();
-    }
+    slice_dots(h1);
     grid.sync();
     // phase 2
-    for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) {
-        double acc = w[r];
-        for (int i = 0; i < nvec; i++) acc -= __ldcg(h1 + i) * V[(long)i * n + r];
-        w[r] = acc;
-    }
-    __syncthreads();
-    for (int i = 0; i < nvec; i++) {
-        const double *v = V + (long)i * n;
-        double acc = 0.0;
-        for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) acc += v[r] * w[r];
-        const double s = Red(tmp).Sum(acc);
-        if (threadIdx.x == 0) atomicAdd(h2 + i, s);
-        __syncthreads();
-    }
+    slice_update(h1, false);
+    slice_dots(h2);
     grid.sync();
     // phase 3
     {
-        double part = 0.0;
-        for (long r = lo + threadIdx.x; r < hi; r += GM_THREADS) {
-            double acc = w[r];
-            for (int i = 0; i < nvec; i++) acc -= __ldcg(h2 + i) * V[(long)i * n + r];
-            w[r] = acc;
-            part += acc * acc;
-        }
+        const double part = slice_update(h2, true);
         const double s = Red(tmp).Sum(part);
         if (threadIdx.x == 0) atomicAdd(nrm2, s);
     }
