@@ -220,6 +220,7 @@ k_m2p(const int *__restrict__ skip, const int4 *__restrict__ items, const int *_
         const bool more = s0 + CB < it.z;
         if (more) { stage(buf ^ 1, s0 + CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
         __syncthreads();
+#pragma unroll 1                                             // one copy of the straight-line body: four copies (65 KB of code at P = 8) thrash the instruction cache
         for (int c_ = 0; c_ < nb; c_++) {
             const double4 c = s_c[buf][c_];
             const T dx = (T)(X.x - c.x), dy = (T)(X.y - c.y), dz = (T)(X.z - c.z);
@@ -352,6 +353,7 @@ k_m2p_twin2(const int *__restrict__ skip, const int4 *__restrict__ items, const 
         const bool more = s0 + CB < it.z;
         if (more) { stage(buf ^ 1, s0 + CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
         __syncthreads();
+#pragma unroll 1                                             // one copy of the straight-line body: four copies (65 KB of code at P = 8) thrash the instruction cache
         for (int c_ = 0; c_ < nb; c_++) {
             const double4 c = s_c[buf][c_];
             const float dx0 = (float)(X0.x - c.x), dy0 = (float)(X0.y - c.y), dz0 = (float)(X0.z - c.z);
@@ -411,6 +413,7 @@ k_m2p_single2(const int *__restrict__ skip, const int4 *__restrict__ items, cons
         const bool more = s0 + CB < it.z;
         if (more) { stage(buf ^ 1, s0 + CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
         __syncthreads();
+#pragma unroll 1                                             // one copy of the straight-line body: four copies (65 KB of code at P = 8) thrash the instruction cache
         for (int c_ = 0; c_ < nb; c_++) {
             const double4 c = s_c[buf][c_];
             const f2_t dx = f2_pack((float)(X0.x - c.x), (float)(X1.x - c.x)), dy = f2_pack((float)(X0.y - c.y), (float)(X1.y - c.y)),
