@@ -130,6 +130,24 @@ def test_restarted_gmres_and_noconv(env):
     h.close()
 
 
+def test_gmres_basis_longer_than_one_coefficient_pass(env):
+    """k_gm_arnoldi stages the Gram-Schmidt coefficients GM_MAXVEC = 256 at a time: a run whose Krylov basis
+    grows past 256 vectors (irregular molecular mesh, no restart) must reach the same solution as a restarted
+    one, and its residual must hold when recomputed from b - A x with one more matvec."""
+    pg, torch, orc = env
+    prob = W.protein_problem(250, spacing=1.1, seed=31)
+    h = pg.Handle.from_problem(prob, K=4, P=6, theta=0.5)
+    xa, ita, rra, _ = h.solve(tol=1e-11, restart=600, max_iter=600)
+    assert ita > 256 and rra <= 1e-11
+    b = h.rhs()
+    res = float(torch.linalg.norm(b - h.matvec(xa)) / torch.linalg.norm(b))
+    assert res <= 1e-10
+    xb, itb, rrb, _ = h.solve(tol=1e-11, restart=100, max_iter=5000)
+    assert float(torch.linalg.norm(xa - xb) / torch.linalg.norm(xb)) <= 1e-8
+    assert abs(h.energy(xa)[0] - h.energy(xb)[0]) <= 1e-8 * abs(h.energy(xb)[0])
+    h.close()
+
+
 # ----------------------------------------------------------------------------------------- treecode
 @pytest.mark.parametrize("maker,level", [(W.kirkwood_problem, 4), (W.stern_sphere_problem, 3),
                                          (W.cavity_sphere_problem, 3)])
