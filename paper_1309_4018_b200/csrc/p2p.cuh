@@ -218,7 +218,11 @@ template <bool YA, bool TWIN, bool YB, bool GUARD>
 __device__ __forceinline__ void p2p_quad_tile(const float4 *__restrict__ sp, const float4 *__restrict__ sc, int nq, f2_t X2,
                                               f2_t Y2, f2_t Z2, const P2PQuadConst &kc, f2_t &a0, f2_t &a1, f2_t &b0, f2_t &b1)
 {
-#pragma unroll 2
+#ifndef P2PQ_UNROLL
+#define P2PQ_UNROLL 2
+#endif
+    constexpr int UNR = P2PQ_UNROLL;
+#pragma unroll UNR
     for (int q = 0; q < nq; q++) {
         const float4 px = sp[3 * q], py = sp[3 * q + 1], pz = sp[3 * q + 2];
         const float4 mV = sc[4 * q], mKx = sc[4 * q + 1], mKy = sc[4 * q + 2], mKz = sc[4 * q + 3];
@@ -232,7 +236,7 @@ __device__ __forceinline__ void p2p_quad_tile(const float4 *__restrict__ sp, con
 #define P2P_QTILE (P2P_TILE / 4)                                       // quads per tile
 template <bool YA, bool TWIN, bool YB>
 #ifndef P2PQ_MINB
-#define P2PQ_MINB 12                                                  // 80 registers: 12 CTAs per SM (uncapped: 114 / 8)
+#define P2PQ_MINB 16                                                  // 64 registers: 16 CTAs per SM (uncapped: 114 / 8; 12: 0.0859, 16: 0.0842, 20: 0.0848 ms)
 #endif
 __global__ void __launch_bounds__(PYGBE_TG, P2PQ_MINB)
 k_p2p_quad(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *__restrict__ tiles,
