@@ -475,3 +475,109 @@ k_m2p_single2(const int *__restrict__ skip, const int4 *__restrict__ items, cons
     if (ok0) atomicAdd(out + t0, a0);
     if (ok1) atomicAdd(out + t1, a1);
 }
+
+// ------------------------------------------------------------------------------------------------------
+// fp64, two targets per thread (one warp per 64-target group).  The one-target kernel above reads one W per
+// DFMA through 16-byte broadcasts and sits on the shared-memory data pipe like its fp32 predecessor did (52 %
+// of the fp64 pipe at config 1); with two targets every W read feeds two DFMAs.
+template <int P, int NS>
+__device__ __forceinline__ void m2p_q2(double dx0, double dy0, double dz0, double dx1, double dy1, double dz1,
+                                       const double *__restrict__ w, double (&q0)[P + 1][NS], double (&q1)[P + 1][NS])
+{
+    double cur[2];
+    int idx = 0;
+#pragma unroll
+    for (int m = 0; m <= P; m++)
+#pragma unroll
+        for (int s = 0; s < NS; s++) { q0[m][s] = 0.0; q1[m][s] = 0.0; }
+    double px0 = 1.0, px1 = 1.0;
+#pragma unroll
+    for (int ex = 0; ex <= P; ex++) {
+        double pxy0 = px0, pxy1 = px1;
+#pragma unroll
+        for (int ey = 0; ey <= P - ex; ey++) {
+            double m0 = pxy0, m1 = pxy1;
+#pragma unroll
+            for (int ez = 0; ez <= P - ex - ey; ez++) {
+                const int t = ex + ey + ez;
+#pragma unroll
+                for (int J = 0; J <= (P - t) / 2; J++) {
+#pragma unroll
+                    for (int s = 0; s < NS; s++) {
+                        if (idx % 2 == 0) Chunk<double>::get(w + idx, cur);
+                        q0[t + J][s] = fma(cur[idx % 2], m0, q0[t + J][s]);
+                        q1[t + J][s] = fma(cur[idx % 2], m1, q1[t + J][s]);
+                        idx++;
+                    }
+                }
+                m0 *= dz0; m1 *= dz1;
+            }
+            pxy0 *= dy0; pxy1 *= dy1;
+        }
+        px0 *= dx0; px1 *= dx1;
+    }
+}
+
+template <int P, bool TWIN>
+__global__ void __launch_bounds__(M2P2_THREADS)
+k_m2p_dbl2(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
+           const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const double *__restrict__ wc,
+           double kappaA, double kappaB, double *__restrict__ outA, double *__restrict__ outB)
+{
+    constexpr int NS = TWIN ? 2 : 1;
+    constexpr int STRIDE = m2p_stride(P, TWIN);
+    constexpr int CH = STRIDE / 2;                           // 16-byte chunks per cell
+    constexpr int CBW = 12288 / (STRIDE * 8);
+    constexpr int CB = CBW < 1 ? 1 : (CBW > 4 ? 4 : CBW);
+    __shared__ __align__(16) double s_W[2][CB][STRIDE];
+    __shared__ __align__(16) double4 s_c[2][CB];
+    if (skip && *skip) return;
+    const int4 it = items[blockIdx.x];
+    const int t0 = it.x * PYGBE_TG_M2P + threadIdx.x, t1 = t0 + M2P2_THREADS;
+    const bool ok0 = t0 < np, ok1 = t1 < np;
+    const double4 X0 = ok0 ? tpos[t0] : make_double4(1e30, 1e30, 1e30, 0), X1 = ok1 ? tpos[t1] : make_double4(1e30, 1e30, 1e30, 0);
+    double aA0 = 0.0, aB0 = 0.0, aA1 = 0.0, aB1 = 0.0;
+    auto stage = [&](int buf, int s0) {
+        const int nb = min(CB, it.z - s0);
+        for (int i = threadIdx.x; i < nb * CH; i += M2P2_THREADS) {
+            const int c_ = i / CH, j = i - c_ * CH;
+            cp_async16(&s_W[buf][c_][j * 2], wc + (long)m2p_cell[s0 + c_] * STRIDE + j * 2);
+        }
+        if (threadIdx.x < nb * 2) {
+            const int c_ = threadIdx.x >> 1, hf = threadIdx.x & 1;
+            cp_async16((char *)&s_c[buf][c_] + 16 * hf, (const char *)(cgeo + m2p_cell[s0 + c_]) + 16 * hf);
+        }
+        cp_async_commit();
+    };
+    stage(0, it.y);
+    int buf = 0;
+    for (int s0 = it.y; s0 < it.z; s0 += CB, buf ^= 1) {
+        const int nb = min(CB, it.z - s0);
+        const bool more = s0 + CB < it.z;
+        if (more) { stage(buf ^ 1, s0 + CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+        __syncthreads();
+#pragma unroll 1                                             // one copy of the straight-line body (instruction cache)
+        for (int c_ = 0; c_ < nb; c_++) {
+            const double4 c = s_c[buf][c_];
+            const double dx0 = X0.x - c.x, dy0 = X0.y - c.y, dz0 = X0.z - c.z;
+            const double dx1 = X1.x - c.x, dy1 = X1.y - c.y, dz1 = X1.z - c.z;
+            double q0[P + 1][NS], q1[P + 1][NS];
+            m2p_q2<P, NS>(dx0, dy0, dz0, dx1, dy1, dz1, s_W[buf][c_], q0, q1);
+            {
+                const double r2 = dx0 * dx0 + dy0 * dy0 + dz0 * dz0;
+                const double rinv = Real<double>::rsqrt_(r2), rinv2 = rinv * rinv, r = r2 * rinv;
+                aA0 += m2p_radial<P, NS, double>(r, rinv, rinv2, kappaA, kappaA, q0, 0);
+                if (TWIN) aB0 += m2p_radial<P, NS, double>(r, rinv, rinv2, kappaB, kappaB, q0, NS - 1);
+            }
+            {
+                const double r2 = dx1 * dx1 + dy1 * dy1 + dz1 * dz1;
+                const double rinv = Real<double>::rsqrt_(r2), rinv2 = rinv * rinv, r = r2 * rinv;
+                aA1 += m2p_radial<P, NS, double>(r, rinv, rinv2, kappaA, kappaA, q1, 0);
+                if (TWIN) aB1 += m2p_radial<P, NS, double>(r, rinv, rinv2, kappaB, kappaB, q1, NS - 1);
+            }
+        }
+        __syncthreads();                                     // buf is refilled two iterations from now
+    }
+    if (ok0) { atomicAdd(outA + t0, aA0); if (TWIN) atomicAdd(outB + t0, aB0); }
+    if (ok1) { atomicAdd(outA + t1, aA1); if (TWIN) atomicAdd(outB + t1, aB1); }
+}

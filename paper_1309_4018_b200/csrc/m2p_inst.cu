@@ -26,7 +26,17 @@ int CAT(pygbe_m2p_launch_, M2P_P)(const M2PArgs &a)
         k_m2p_single2<M2P_P><<<a.n_items, M2P2_THREADS, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo, (const float *)a.wc,
                                                                     a.kappaA, Real<float>::kscale(a.kappaA), a.outA);
     }
+#if M2P_P <= 7
+    else if (a.twin) {                    // fp64, two targets per thread: 0.156 -> 0.145 ms at P = 6 (config 1)
+        k_m2p_dbl2<M2P_P, true><<<a.n_items, M2P2_THREADS, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo,
+                                                                       (const double *)a.wc, a.kappaA, a.kappaB, a.outA, a.outB);
+    } else {
+        k_m2p_dbl2<M2P_P, false><<<a.n_items, M2P2_THREADS, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo,
+                                                                        (const double *)a.wc, a.kappaA, a.kappaB, a.outA, a.outB);
+    }
+#else                                     // P >= 8: 158+ registers with two targets, no gain (1.344 against 1.331 ms at P = 8)
     else { if (a.twin) launch<true, double>(a); else launch<false, double>(a); }
+#endif
     return 0;
 }
 #endif
