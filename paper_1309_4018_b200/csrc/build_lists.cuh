@@ -70,6 +70,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     R.nleaves = (int)leaves.size();
     TRY(upload(h, &R.leaf_cell, leaves));
 
+    dbg_t("  octree split + download");
     // ---- anchors (mixed precision): the ancestor of each leaf at the level where cells are <= 16 A wide
     const bool mixed = h->precision == PYGBE_PRECISION_MIXED;
     std::vector<int> anchor_of(ncells, 0);
@@ -150,6 +151,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     for (void *q : {(void *)d_mcnt, (void *)d_pcnt, (void *)d_over, (void *)d_poff_raw, (void *)d_pleaf_raw})
         h->mem.release_one(q);
 
+    dbg_t("  anchors, groups, traversal");
     // ---- P2P lists: leaves -> panel ranges sorted by position; adjacent ranges with the same anchor merge
     std::vector<int4> prng;               // merged ranges, CSR by group
     std::vector<int> poff2(R.ng + 1, 0);
@@ -178,6 +180,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     for (int g = 0; g < R.ng; g++) R.m2p_evals += (long)std::min(PYGBE_TG, R.np - g * PYGBE_TG) * mcnt[g];
     TRY(upload(h, &R.p2p_off, poff2)); TRY(upload(h, &R.p2p_rng, prng));
 
+    dbg_t("  P2P ranges (host)");
     // ---- work items of bounded size, enough of them to fill 148 SMs several times over
     const long want_items = 148L * 16;
     // M2P CTAs keep only 8-20 warps per SM resident (72-127 registers): finer items even out the tail (config 1:
@@ -248,6 +251,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
         for (int i = 0; i < 9; i++) fprintf(stderr, " %d", hist[i]);
         fprintf(stderr, "\n");
     }
+    dbg_t("  tiles + items (host)");
     R.n_p2p_items = (int)pitems.size(); R.n_m2p_items = (int)mitems.size();
     TRY(upload(h, &R.p2p_sub, sub)); TRY(upload(h, &R.p2p_seg, segs)); TRY(upload(h, &R.p2p_items, pitems)); TRY(upload(h, &R.m2p_items, mitems));
     CUDA_TRY(cudaStreamSynchronize(h->stream));

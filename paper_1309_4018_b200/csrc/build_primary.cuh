@@ -30,6 +30,7 @@ static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<do
     for (int a = 0; a < 3; a++) R.root_c[a] = 0.5 * (lo[a] + hi[a]);
     R.root_edge = edge;
 
+    dbg_t("boundary + bbox (host)");
     // ---- Morton keys, sort, gather into sorted order, Gauss points
     int *d_gid_u, *d_phi_u, *d_dphi_u, *d_row_u, *d_iota;
     double *d_cV_u, *d_cK_u;
@@ -62,8 +63,11 @@ static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<do
     for (void *q : {(void *)d_gid_u, (void *)d_phi_u, (void *)d_dphi_u, (void *)d_row_u, (void *)d_iota,
                     (void *)d_cV_u, (void *)d_cK_u, (void *)d_keys_u})
         h->mem.release_one(q);
+    dbg_t("keys, sort, gather");
     TRY(build_tree_and_lists(h, R));
+    dbg_t("tree + lists total");
     TRY(build_corrections(h, R, qt, nullptr));
+    dbg_t("corrections");
     if (R.n_m2p_items > 0) {
         TRY(h->mem.alloc(&R.mom, (size_t)R.ncells * 2 * h->Nc));
         TRY(h->mem.alloc(&R.pmom, (size_t)R.np * 2 * h->Nc));

@@ -8,6 +8,17 @@ static inline double now_ms()
     return duration<double, std::milli>(steady_clock::now().time_since_epoch()).count();
 }
 
+// PYGBE_DEBUG=1: host milliseconds since the previous checkpoint (create-time diagnostics on stderr)
+static inline void dbg_t(const char *what)
+{
+    static const bool on = getenv("PYGBE_DEBUG") != nullptr;
+    static double last = 0.0;
+    if (!on) return;
+    const double t = now_ms();
+    if (what) fprintf(stderr, "[pygbe] %-28s %8.3f ms\n", what, t - last);
+    last = t;
+}
+
 template <class T> static int upload(pygbe_handle *h, T **dst, const std::vector<T> &src)
 {
     TRY(h->mem.alloc(dst, src.size()));

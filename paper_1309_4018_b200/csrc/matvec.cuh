@@ -58,8 +58,13 @@ static void launch_p2p(pygbe_handle *h, Region &A, Region *B, const int *skip)
     const double kA = A.kappa, kB = B ? B->kappa : 0.0, rV = B ? A.twin_rV : 1.0;
     double *oA = A.out, *oB = B ? B->out : nullptr;
     const bool quad = sizeof(T) == 4 && A.quad;
+    static const int two = getenv("PYGBE_P2P_TWO") ? atoi(getenv("PYGBE_P2P_TWO")) : 1;    // tuning: 0 never, 1 single regions, 2 always
+    const bool quad2 = quad && (two == 2 || (two == 1 && !B));
 #define P2P_GO(YA, TW, YB)                                                                                     \
-    do { if (quad) { auto kern = k_p2p_quad<YA, TW, YB>;                                                       \
+    do { if (quad2) { auto kern = k_p2p_quad2<YA, TW, YB>;                                                     \
+             LAUNCH(h, kern, A.n_p2p_items, P2PQ2_THREADS, 0, skip, A.p2p_items, A.p2p_sub, A.p2p_seg, A.np, A.tpos, A.cgeo, \
+                    (const float4 *)A.sposf, (const float4 *)A.schgf, kA, kB, rV, oA, oB); }                   \
+         else if (quad) { auto kern = k_p2p_quad<YA, TW, YB>;                                                  \
              LAUNCH(h, kern, A.n_p2p_items, PYGBE_TG, 0, skip, A.p2p_items, A.p2p_sub, A.p2p_seg, A.np, A.tpos, A.cgeo, \
                     (const float4 *)A.sposf, (const float4 *)A.schgf, kA, kB, rV, oA, oB); }                   \
          else { auto kern = k_p2p<T, YA, TW, YB>;                                                              \

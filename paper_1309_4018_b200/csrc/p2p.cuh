@@ -311,6 +311,107 @@ k_p2p_quad(const int *__restrict__ skip, const int4 *__restrict__ items, const i
     }
 }
 
+// ------------------------------------------------------------------------------------------------------
+// Two targets per thread (one warp per 64-target group): every LDS.128 of a source quad serves two targets.
+// The single-region kernels (Laplace only: 6.5 packed instructions per pair) sit on the shared-memory data pipe
+// with one target per thread (l1tex__data_pipe_lsu_wavefronts 75-82 % of peak, profiles/r3a); the fused twin
+// kernel does not (54 %) and keeps one target per thread.
+template <bool YA, bool TWIN, bool YB, bool GUARD>
+__device__ __forceinline__ void p2p_quad_tile2(const float4 *__restrict__ sp, const float4 *__restrict__ sc, int nq, f2_t X0,
+                                               f2_t Y0, f2_t Z0, f2_t X1, f2_t Y1, f2_t Z1, const P2PQuadConst &kc,
+                                               f2_t (&a)[4], f2_t (&b)[4])
+{
+#pragma unroll 1
+    for (int q = 0; q < nq; q++) {
+        const float4 px = sp[3 * q], py = sp[3 * q + 1], pz = sp[3 * q + 2];
+        const float4 mV = sc[4 * q], mKx = sc[4 * q + 1], mKy = sc[4 * q + 2], mKz = sc[4 * q + 3];
+        const f2_t pxl = f2_pack(px.x, px.y), pyl = f2_pack(py.x, py.y), pzl = f2_pack(pz.x, pz.y), mVl = f2_pack(mV.x, mV.y),
+                   kxl = f2_pack(mKx.x, mKx.y), kyl = f2_pack(mKy.x, mKy.y), kzl = f2_pack(mKz.x, mKz.y);
+        const f2_t pxh = f2_pack(px.z, px.w), pyh = f2_pack(py.z, py.w), pzh = f2_pack(pz.z, pz.w), mVh = f2_pack(mV.z, mV.w),
+                   kxh = f2_pack(mKx.z, mKx.w), kyh = f2_pack(mKy.z, mKy.w), kzh = f2_pack(mKz.z, mKz.w);
+        p2p_pair2<YA, TWIN, YB, GUARD>(X0, Y0, Z0, pxl, pyl, pzl, mVl, kxl, kyl, kzl, kc, a[0], b[0]);
+        p2p_pair2<YA, TWIN, YB, GUARD>(X1, Y1, Z1, pxl, pyl, pzl, mVl, kxl, kyl, kzl, kc, a[1], b[1]);
+        p2p_pair2<YA, TWIN, YB, GUARD>(X0, Y0, Z0, pxh, pyh, pzh, mVh, kxh, kyh, kzh, kc, a[2], b[2]);
+        p2p_pair2<YA, TWIN, YB, GUARD>(X1, Y1, Z1, pxh, pyh, pzh, mVh, kxh, kyh, kzh, kc, a[3], b[3]);
+    }
+}
+
+#define P2PQ2_THREADS (PYGBE_TG / 2)
+template <bool YA, bool TWIN, bool YB>
+__global__ void __launch_bounds__(P2PQ2_THREADS)
+k_p2p_quad2(const int *__restrict__ skip, const int4 *__restrict__ items, const int4 *__restrict__ tiles,
+            const int2 *__restrict__ segs, int np, const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo,
+            const float4 *__restrict__ posq, const float4 *__restrict__ chgq, double kappaA, double kappaB, double rV,
+            double *__restrict__ outA, double *__restrict__ outB)
+{
+    __shared__ __align__(16) float4 s_pos[2][3 * P2P_QTILE];
+    __shared__ __align__(16) float4 s_chg[2][4 * P2P_QTILE];
+    __shared__ __align__(16) double4 s_an[2];
+    if (skip && *skip) return;
+    const int4 it = items[blockIdx.x];
+    const int lane = threadIdx.x;
+    const int t0 = it.x * PYGBE_TG + lane, t1 = t0 + P2PQ2_THREADS;
+    const bool ok0 = t0 < np, ok1 = t1 < np;
+    const double4 XA = ok0 ? tpos[t0] : make_double4(0, 0, 0, 0), XB = ok1 ? tpos[t1] : make_double4(0, 0, 0, 0);
+    P2PQuadConst kc;
+    {
+        const float a = -(float)Real<float>::kscale(kappaA), b = -(float)Real<float>::kscale(kappaB);
+        const float s = (float)(1.0 / rV), c = (float)(kappaB / rV), ka = (float)kappaA;
+        kc.nksA = f2_pack(a, a); kc.nksB = f2_pack(b, b); kc.kA = f2_pack(ka, ka); kc.sB = f2_pack(s, s); kc.cB = f2_pack(c, c);
+        kc.tiny = f2_pack(1e-30f, 1e-30f);
+    }
+    double accA0 = 0.0, accB0 = 0.0, accA1 = 0.0, accB1 = 0.0;
+    auto stage = [&](int buf, const int4 &tl) {                      // segments = (first point, points), multiples of 4
+        int qoff = 0;                                                // quads staged so far
+        for (int s0 = tl.x; s0 < tl.y; s0 += 32) {
+            const int ns = min(32, tl.y - s0);
+            const int2 mine = lane < ns ? segs[s0 + lane] : make_int2(0, 0);
+            for (int s = 0; s < ns; s++) {
+                const int q0 = __shfl_sync(0xffffffffu, mine.x, s) >> 2, nq = __shfl_sync(0xffffffffu, mine.y, s) >> 2;
+                for (int i = lane; i < 7 * nq; i += P2PQ2_THREADS) {
+                    if (i < 3 * nq) cp_async16(&s_pos[buf][3 * qoff + i], posq + 3 * (long)q0 + i);
+                    else cp_async16(&s_chg[buf][4 * qoff + i - 3 * nq], chgq + 4 * (long)q0 + i - 3 * nq);
+                }
+                qoff += nq;
+            }
+        }
+        if (lane < 2) cp_async16((char *)&s_an[buf] + 16 * lane, (const char *)(cgeo + tl.z) + 16 * lane);
+        cp_async_commit();
+    };
+    int4 cur = tiles[it.y];
+    int4 nxt = it.y + 1 < it.z ? tiles[it.y + 1] : cur;
+    stage(0, cur);
+    int buf = 0;
+    for (int k = it.y; k < it.z; k++, buf ^= 1) {
+        const bool more = k + 1 < it.z;
+        if (more) { stage(buf ^ 1, nxt); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+        const int nq = cur.w >> 3;
+        const bool self = (cur.w & 1) != 0;
+        cur = nxt;
+        if (k + 2 < it.z) nxt = tiles[k + 2];
+        __syncwarp();                                                // one warp: every lane's copies have landed
+        const double4 an = s_an[buf];
+        const float x0 = (float)(XA.x - an.x), y0 = (float)(XA.y - an.y), z0 = (float)(XA.z - an.z);
+        const float x1 = (float)(XB.x - an.x), y1 = (float)(XB.y - an.y), z1 = (float)(XB.z - an.z);
+        const float4 *sp = s_pos[buf], *sc = s_chg[buf];
+        f2_t a[4] = {0, 0, 0, 0}, b[4] = {0, 0, 0, 0};
+        if (self) p2p_quad_tile2<YA, TWIN, YB, true>(sp, sc, nq, f2_pack(x0, x0), f2_pack(y0, y0), f2_pack(z0, z0), f2_pack(x1, x1),
+                                                      f2_pack(y1, y1), f2_pack(z1, z1), kc, a, b);
+        else p2p_quad_tile2<YA, TWIN, YB, false>(sp, sc, nq, f2_pack(x0, x0), f2_pack(y0, y0), f2_pack(z0, z0), f2_pack(x1, x1),
+                                                  f2_pack(y1, y1), f2_pack(z1, z1), kc, a, b);
+        float lo, hi;
+        f2_unpack(f2_add(a[0], a[2]), lo, hi); accA0 += (double)(lo + hi);
+        f2_unpack(f2_add(a[1], a[3]), lo, hi); accA1 += (double)(lo + hi);
+        if constexpr (TWIN) {
+            f2_unpack(f2_add(b[0], b[2]), lo, hi); accB0 += (double)(lo + hi);
+            f2_unpack(f2_add(b[1], b[3]), lo, hi); accB1 += (double)(lo + hi);
+        }
+        __syncwarp();                                                // buf is refilled two iterations from now
+    }
+    if (ok0) { atomicAdd(outA + t0, accA0); if constexpr (TWIN) atomicAdd(outB + t0, rV * accB0); }
+    if (ok1) { atomicAdd(outA + t1, accA1); if constexpr (TWIN) atomicAdd(outB + t1, rV * accB1); }
+}
+
 // quad layout of the fp32 source coordinates (create time): see k_make_sposf for the rounding
 __global__ void k_make_sposq(int np, int K, const int *__restrict__ panel_anchor, const double4 *__restrict__ cgeo,
                              const double4 *__restrict__ spos, float *__restrict__ posq)
