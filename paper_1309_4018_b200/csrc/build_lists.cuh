@@ -103,7 +103,8 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     // evaluation costs Nc - 1 + NW FMA-pipe instructions per region, a P2P pair ~14 per region, and the sweep of
     // profiles/r2a_regrouped_path.md puts the optimum at ~16 points for P = 6 (344 instructions) in both precisions
     const int small_leaf = (int)(16.0 * (h->Nc + 2.0 * h->NW) / 344.0 / K);
-    LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.ggeo, R.cgeo, R.crange, R.cchild,
+    const int exact_mac = getenv("PYGBE_BOUND_MAC") ? 0 : 1;     // tuning: 1 = group MAC on the group's own points
+    LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.tpos, R.np, exact_mac, R.ggeo, R.cgeo, R.crange, R.cchild,
            h->theta, near_dist, small_leaf, 0, d_mcnt, d_pcnt, nullptr, nullptr, nullptr, nullptr, d_over);
     std::vector<int> mcnt, pcnt;
     TRY(download(h, mcnt, d_mcnt, (size_t)R.ng));
@@ -113,7 +114,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     int *d_poff_raw, *d_pleaf_raw;
     TRY(upload(h, &R.m2p_off, moff)); TRY(upload(h, &d_poff_raw, poff));
     TRY(h->mem.alloc(&R.m2p_cell, moff[R.ng])); TRY(h->mem.alloc(&d_pleaf_raw, poff[R.ng]));
-    LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.ggeo, R.cgeo, R.crange, R.cchild,
+    LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.tpos, R.np, exact_mac, R.ggeo, R.cgeo, R.crange, R.cchild,
            h->theta, near_dist, small_leaf, 1, d_mcnt, d_pcnt, R.m2p_off, d_poff_raw, R.m2p_cell, d_pleaf_raw, d_over);
     std::vector<int> pleaf;
     TRY(download(h, pleaf, d_pleaf_raw, (size_t)poff[R.ng]));

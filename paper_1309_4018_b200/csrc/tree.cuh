@@ -207,7 +207,8 @@ k_group_geometry(const double4 *__restrict__ tpos, int np, double4 *__restrict__
 #define TRAV_WARPS 4
 #define TRAV_STACK 256
 __global__ void __launch_bounds__(TRAV_WARPS * 32)
-k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__ cgeo,
+k_traverse(int ng, const double4 *__restrict__ tpos, int np, int exact, const double4 *__restrict__ ggeo,
+           const double4 *__restrict__ cgeo,
            const int2 *__restrict__ crange, const int2 *__restrict__ cchild, double theta,
            double near_dist, int small_leaf, int fill, int *__restrict__ m2p_cnt, int *__restrict__ p2p_cnt,
            const int *__restrict__ m2p_off, const int *__restrict__ p2p_off, int *__restrict__ m2p_cell,
@@ -219,21 +220,59 @@ k_traverse(int ng, const double4 *__restrict__ ggeo, const double4 *__restrict__
     if (g >= ng) return;
     int *stack = s_stack[warp];
     const double4 G = ggeo[2 * g], H = ggeo[2 * g + 1];
+    // the group's own targets, PYGBE_TG / 32 per lane (exact minimum distance of the undecided cells)
+    double tx[PYGBE_TG / 32], ty[PYGBE_TG / 32], tz[PYGBE_TG / 32];
+#pragma unroll
+    for (int k = 0; k < PYGBE_TG / 32; k++) {
+        const int t = g * PYGBE_TG + k * 32 + lane;
+        const double4 x = tpos[min(t, np - 1)];                      // a ragged last group repeats its last target
+        tx[k] = x.x; ty[k] = x.y; tz[k] = x.z;
+    }
     int nm = 0, npp = 0, sp = 0;
     const int mbase = fill ? m2p_off[g] : 0, pbase = fill ? p2p_off[g] : 0;
     // the root is tested like a child of a virtual parent
     int first = 0, count = 1;
     while (true) {
         int c = (lane < count) ? first + lane : -1;
-        bool acc = false, leaf = false, open = false;
+        bool acc = false, leaf = false, open = false, maybe = false;
+        double dist = 0.0, rb = 0.0;
         if (c >= 0) {
             double4 cg = cgeo[c];
             double dx = G.x - cg.x, dy = G.y - cg.y, dz = G.z - cg.z;
             // lower bound of the distance from the cell centre to any target of the group: the better of
             // the bounding sphere and the bounding box
             double bx = fmax(fabs(dx) - H.x, 0.0), by = fmax(fabs(dy) - H.y, 0.0), bz = fmax(fabs(dz) - H.z, 0.0);
-            double dist = fmax(sqrt(dx * dx + dy * dy + dz * dz) - G.w, sqrt(bx * bx + by * by + bz * bz));
-            acc = (theta * dist > cg.w) && (dist - 0.8660254037844387 * cg.w > near_dist);
+            const double dc = sqrt(dx * dx + dy * dy + dz * dz);
+            dist = fmax(dc - G.w, sqrt(bx * bx + by * by + bz * bz));
+            rb = cg.w;
+            acc = (theta * dist > rb) && (dist - 0.8660254037844387 * rb > near_dist);
+            // undecided: the bound fails, but the farthest any target can be (dc + radius) would pass
+            const double far = dc + G.w;
+            maybe = !acc && (theta * far > rb) && (far - 0.8660254037844387 * rb > near_dist);
+        }
+        if (exact) {
+            // eq. (15) for every target of the group against the undecided cells: the minimum over the group's
+            // own points instead of its bounding volume (accepts 5-10 % closer cells; still reading A9)
+            unsigned mm = __ballot_sync(0xffffffffu, maybe);
+            while (mm) {
+                const int k = __ffs(mm) - 1;
+                mm &= mm - 1;
+                const double4 cg = cgeo[first + k];
+                double d2 = 1e300;
+#pragma unroll
+                for (int j = 0; j < PYGBE_TG / 32; j++) {
+                    const double ex = tx[j] - cg.x, ey = ty[j] - cg.y, ez = tz[j] - cg.z;
+                    d2 = fmin(d2, ex * ex + ey * ey + ez * ez);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) d2 = fmin(d2, __shfl_xor_sync(0xffffffffu, d2, o));
+                if (lane == k) {
+                    dist = sqrt(d2);
+                    acc = (theta * dist > rb) && (dist - 0.8660254037844387 * rb > near_dist);
+                }
+            }
+        }
+        if (c >= 0) {
             if (acc && cchild[c].y == 0) {
                 // an accepted leaf with so few panels that summing its points directly (exact) costs fewer
                 // instructions than one Taylor evaluation goes to the direct list instead
