@@ -292,9 +292,9 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
         dt = "f32" if precision == pg.PRECISION_MIXED else "f64"
         achieved = flops / (stage_ms[dom] * 1e-3) / 1e12
         # dram__bytes_read.sum + dram__bytes_write.sum of the stage's launches from the ncu --set full capture of this
-        # command (profiles/r2b_packed_path.md, config kirkwood_l5): bytes per matvec, both regions; else null
-        traffic = {("kirkwood_l5", "f32", "m2p"): 2.60e6, ("kirkwood_l5", "f32", "p2p"): 3.66e6}.get((args.config, dt, dom))
-        kname = {"m2p": "%s<%d,%s>" % ("k_m2p_twin2 / k_m2p_single2 (two targets per thread, packed f32x2)" if dt == "f32" else "k_m2p<double>", kw["P"],
+        # command (profiles/r3c_group_mac_path.md, config kirkwood_l5): bytes per matvec, both regions; else null
+        traffic = {("kirkwood_l5", "f32", "m2p"): 2.65e6, ("kirkwood_l5", "f32", "p2p"): 3.78e6}.get((args.config, dt, dom))
+        kname = {"m2p": "%s<%d,%s>" % ("k_m2p_twin2 / k_m2p_single2 (two targets per thread, packed f32x2)" if dt == "f32" else "k_m2p_dbl2 / k_m2p<double>", kw["P"],
                                        "twin regions fused" if nreg == 2 else "per tree"),
                  "p2p": "%s<%s>" % ("k_p2p_quad (packed f32x2)" if dt == "f32" and kw["K"] % 4 == 0 else "k_p2p<%s>" % ("float" if dt == "f32" else "double"),
                                     "twin regions fused" if nreg == 2 else "per region")}[dom]
