@@ -155,6 +155,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     dbg_t("  anchors, groups, traversal");
     // ---- P2P lists: leaves -> panel ranges sorted by position; adjacent ranges with the same anchor merge
     std::vector<int4> prng;               // merged ranges, CSR by group
+    prng.reserve(pleaf.size());
     std::vector<int> poff2(R.ng + 1, 0);
     long total_src_panels = 0;
     R.p2p_pairs = 0;
@@ -165,7 +166,9 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
             int c = pleaf[r];
             tmp.push_back(make_int4(crange_h[c].x, crange_h[c].y, anchor_of[c], 0));
         }
-        std::sort(tmp.begin(), tmp.end(), [](const int4 &a, const int4 &b) { return a.x < b.x; });
+        // the traversal emits a group's leaves in Morton order, i.e. by ascending panel range: sort only if not
+        auto by_pos = [](const int4 &a, const int4 &b) { return a.x < b.x; };
+        if (!std::is_sorted(tmp.begin(), tmp.end(), by_pos)) std::sort(tmp.begin(), tmp.end(), by_pos);
         size_t start = prng.size();
         for (const int4 &e : tmp) {
             if (prng.size() > start && prng.back().y == e.x && prng.back().z == e.z) prng.back().y = e.y;
@@ -199,6 +202,8 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     std::vector<int4> sub, pitems, mitems;
     std::vector<int> gtile(R.ng + 1, 0);                           // first tile of each group
     std::vector<int2> segs;
+    sub.reserve(total_src_panels / tile_panels + prng.size()); segs.reserve(total_src_panels / tile_panels + 2 * prng.size());
+    mitems.reserve((size_t)moff[R.ng] / m2p_item + R.ng);
     std::vector<int4> grng;
     for (int g = 0; g < R.ng; g++) {
         grng.assign(prng.begin() + poff2[g], prng.begin() + poff2[g + 1]);

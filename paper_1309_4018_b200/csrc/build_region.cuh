@@ -21,6 +21,10 @@ struct Boundary {
 //   sigma = +1, c = 1 if the region is region_in(S); sigma = -1, c = eps_in(S)/eps_out(S) if region_out(S).
 static void collect_boundary(const pygbe_handle *h, int id, Boundary &b)
 {
+    size_t total = 0;
+    for (int s = 0; s < h->nsurf; s++)
+        if (h->rin[s] == id || h->rout[s] == id) total += (size_t)h->surf_count[s];
+    b.gid.reserve(total); b.phi.reserve(total); b.dphi.reserve(total); b.row.reserve(total); b.cV.reserve(total); b.cK.reserve(total);
     for (int s = 0; s < h->nsurf; s++) {
         double sigma, c;
         int half;
