@@ -98,14 +98,17 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     int *d_mcnt, *d_pcnt, *d_over;
     TRY(h->mem.alloc(&d_mcnt, R.ng)); TRY(h->mem.alloc(&d_pcnt, R.ng)); TRY(h->mem.alloc(&d_over, 1));
     CUDA_TRY(cudaMemsetAsync(d_over, 0, sizeof(int), h->stream));
-    const double near_dist = h->thres > 0 ? h->thres * R.Lmax : 0.0;
+    double *d_clmax;
+    TRY(h->mem.alloc(&d_clmax, (size_t)ncells));
+    LAUNCH(h, k_cell_lmax, cdiv((long)ncells * 32, 128), 128, 0, ncells, R.crange, R.tpos, d_clmax);
+    const double thres_guard = h->thres > 0 ? h->thres : 0.0;
     // break-even between one Taylor evaluation and the direct sum over a leaf's points: a regrouped M2P
     // evaluation costs Nc - 1 + NW FMA-pipe instructions per region, a P2P pair ~14 per region, and the sweep of
     // profiles/r2a_regrouped_path.md puts the optimum at ~16 points for P = 6 (344 instructions) in both precisions
     const int small_leaf = (int)(16.0 * (h->Nc + 2.0 * h->NW) / 344.0 / K);
     const int exact_mac = getenv("PYGBE_BOUND_MAC") ? 0 : 1;     // tuning: 1 = group MAC on the group's own points
     LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.tpos, R.np, exact_mac, R.ggeo, R.cgeo, R.crange, R.cchild,
-           h->theta, near_dist, small_leaf, 0, d_mcnt, d_pcnt, nullptr, nullptr, nullptr, nullptr, d_over);
+           h->theta, thres_guard, d_clmax, small_leaf, 0, d_mcnt, d_pcnt, nullptr, nullptr, nullptr, nullptr, d_over);
     std::vector<int> mcnt, pcnt;
     TRY(download(h, mcnt, d_mcnt, (size_t)R.ng));
     TRY(download(h, pcnt, d_pcnt, (size_t)R.ng));
@@ -115,7 +118,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     TRY(upload(h, &R.m2p_off, moff)); TRY(upload(h, &d_poff_raw, poff));
     TRY(h->mem.alloc(&R.m2p_cell, moff[R.ng])); TRY(h->mem.alloc(&d_pleaf_raw, poff[R.ng]));
     LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.tpos, R.np, exact_mac, R.ggeo, R.cgeo, R.crange, R.cchild,
-           h->theta, near_dist, small_leaf, 1, d_mcnt, d_pcnt, R.m2p_off, d_poff_raw, R.m2p_cell, d_pleaf_raw, d_over);
+           h->theta, thres_guard, d_clmax, small_leaf, 1, d_mcnt, d_pcnt, R.m2p_off, d_poff_raw, R.m2p_cell, d_pleaf_raw, d_over);
     std::vector<int> pleaf;
     TRY(download(h, pleaf, d_pleaf_raw, (size_t)poff[R.ng]));
     {   // multipoles are needed for the listed cells and, to build those by M2M, for all their descendants
@@ -149,7 +152,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     int over = 0;
     CUDA_TRY(cudaMemcpy(&over, d_over, sizeof(int), cudaMemcpyDeviceToHost));
     if (over) { pygbe_set_error("traversal stack overflow"); return PYGBE_ECUDA; }
-    for (void *q : {(void *)d_mcnt, (void *)d_pcnt, (void *)d_over, (void *)d_poff_raw, (void *)d_pleaf_raw})
+    for (void *q : {(void *)d_mcnt, (void *)d_pcnt, (void *)d_over, (void *)d_poff_raw, (void *)d_pleaf_raw, (void *)d_clmax})
         h->mem.release_one(q);
 
     dbg_t("  anchors, groups, traversal");

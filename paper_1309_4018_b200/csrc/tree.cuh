@@ -192,6 +192,20 @@ k_group_geometry(const double4 *__restrict__ tpos, int np, double4 *__restrict__
     }
 }
 
+// longest panel L = sqrt(2A) of every cell (tpos.w), one warp per cell: the near-field guard of the traversal
+__global__ void __launch_bounds__(128)
+k_cell_lmax(int ncells, const int2 *__restrict__ crange, const double4 *__restrict__ tpos, double *__restrict__ clmax)
+{
+    const int c = (int)((blockIdx.x * (long)blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    if (c >= ncells) return;
+    const int2 r = crange[c];
+    double m = 0.0;
+    for (int p = r.x + lane; p < r.y; p += 32) m = fmax(m, tpos[p].w);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (lane == 0) clmax[c] = m;
+}
+
 // ---------------------------------------------------------------------------------------- traversal
 // One warp per target group walks the tree from the root.  A cell is accepted for the
 // Taylor expansion when the MAC of eq. (15) holds for every target of the group (reading A9):
@@ -201,8 +215,10 @@ k_group_geometry(const double4 *__restrict__ tpos, int np, double4 *__restrict__
 // group's own points (exact = 1; with the bound alone the direct lists were 27 % longer at config 1)
 // and, so that the near-singular region is always inside the direct list ("in practice,
 // the near-singular region is always contained in an area where the MAC criterion is not met"), when
-// additionally every panel centroid of the cell is farther than thres * Lmax from every target:
-//      dist - (sqrt(3)/2) r_b > thres * Lmax.
+// additionally every panel centroid of the cell is farther than thres * Lmax(cell) from every target, Lmax(cell)
+// the longest panel of that cell (the longest panel of the whole region made the direct lists of the irregular
+// molecular meshes 10 % longer):
+//      dist - (sqrt(3)/2) r_b > thres * Lmax(cell).
 // Accepted cells go to the M2P list; leaves that fail go to the P2P list (as cell ids); other cells
 // are opened.  Pass 1 (fill == 0) counts, pass 2 writes.  The lane that owns child d of the popped
 // cell tests it; ballots keep the output order deterministic (Morton order).
@@ -212,7 +228,7 @@ __global__ void __launch_bounds__(TRAV_WARPS * 32)
 k_traverse(int ng, const double4 *__restrict__ tpos, int np, int exact, const double4 *__restrict__ ggeo,
            const double4 *__restrict__ cgeo,
            const int2 *__restrict__ crange, const int2 *__restrict__ cchild, double theta,
-           double near_dist, int small_leaf, int fill, int *__restrict__ m2p_cnt, int *__restrict__ p2p_cnt,
+           double thres, const double *__restrict__ clmax, int small_leaf, int fill, int *__restrict__ m2p_cnt, int *__restrict__ p2p_cnt,
            const int *__restrict__ m2p_off, const int *__restrict__ p2p_off, int *__restrict__ m2p_cell,
            int *__restrict__ p2p_leaf, int *overflow)
 {
@@ -237,7 +253,7 @@ k_traverse(int ng, const double4 *__restrict__ tpos, int np, int exact, const do
     while (true) {
         int c = (lane < count) ? first + lane : -1;
         bool acc = false, leaf = false, open = false, maybe = false;
-        double dist = 0.0, rb = 0.0;
+        double dist = 0.0, rb = 0.0, near_dist = 0.0;
         if (c >= 0) {
             double4 cg = cgeo[c];
             double dx = G.x - cg.x, dy = G.y - cg.y, dz = G.z - cg.z;
@@ -247,6 +263,7 @@ k_traverse(int ng, const double4 *__restrict__ tpos, int np, int exact, const do
             const double dc = sqrt(dx * dx + dy * dy + dz * dz);
             dist = fmax(dc - G.w, sqrt(bx * bx + by * by + bz * bz));
             rb = cg.w;
+            near_dist = thres * clmax[c];
             acc = (theta * dist > rb) && (dist - 0.8660254037844387 * rb > near_dist);
             // undecided: the bound fails, but the farthest any target can be (dc + radius) would pass
             const double far = dc + G.w;
