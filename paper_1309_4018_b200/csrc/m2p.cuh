@@ -315,11 +315,15 @@ __device__ __forceinline__ f2_t m2p_radial_packed(float dx, float dy, float dz, 
 }
 
 #define M2P2_THREADS (PYGBE_TG_M2P / 2)
-#ifndef M2P2_MINB
-#define M2P2_MINB 1                  // register caps lose: 96 regs 0.0533 ms, 80 regs 0.0554, 72 regs 0.0571, 64 regs 0.0584 (P = 6, config 1)
+// register-cap experiment (-DM2P2_MINB=<CTAs per SM>): caps lose -- 96 regs 0.0533 ms, 80 regs 0.0554, 72 regs 0.0571,
+// 64 regs 0.0584 (P = 6, config 1) -- and even a minimum of 1 changes ptxas's allocation (138 regs, 0.0575 ms)
+#ifdef M2P2_MINB
+#define M2P2_BOUNDS __launch_bounds__(M2P2_THREADS, M2P2_MINB)
+#else
+#define M2P2_BOUNDS __launch_bounds__(M2P2_THREADS)
 #endif
 template <int P>
-__global__ void __launch_bounds__(M2P2_THREADS, M2P2_MINB)
+__global__ void M2P2_BOUNDS
 k_m2p_twin2(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
             const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const float *__restrict__ wc,
             double kappaA, double kscaledA, double kappaB, double kscaledB, double *__restrict__ outA, double *__restrict__ outB)
@@ -378,7 +382,7 @@ k_m2p_twin2(const int *__restrict__ skip, const int4 *__restrict__ items, const 
 // fp32, a tree without twin, two targets per thread: the pair is (target 0, target 1) -- packed monomials,
 // packed accumulators Q_m, W as the broadcast operand -- including the radial part.
 template <int P>
-__global__ void __launch_bounds__(M2P2_THREADS, M2P2_MINB)
+__global__ void M2P2_BOUNDS
 k_m2p_single2(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
               const double4 *__restrict__ tpos, const double4 *__restrict__ cgeo, const float *__restrict__ wc,
               double kappa, double kscaled, double *__restrict__ out)
