@@ -259,6 +259,13 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
                 R.ng, prng.size(), pitems.size(), sub.size(), (double)pts / (sub.size() * (double)P2P_TILE), selft);
         for (int i = 0; i < 9; i++) fprintf(stderr, " %d", hist[i]);
         fprintf(stderr, "\n");
+        int tmin = 1 << 30, tmax = 0, over15 = 0;
+        const double tavg = (double)sub.size() / std::max(1, R.ng);
+        for (int g = 0; g < R.ng; g++) {
+            const int nt = gtile[g + 1] - gtile[g];
+            tmin = std::min(tmin, nt); tmax = std::max(tmax, nt); over15 += nt > 1.5 * tavg;
+        }
+        fprintf(stderr, "[pygbe] tiles per group: min %d avg %.1f max %d, %d of %d groups above 1.5 x avg\n", tmin, tavg, tmax, over15, R.ng);
     }
     dbg_t("  tiles + items (host)");
     R.n_p2p_items = (int)pitems.size(); R.n_m2p_items = (int)mitems.size();
