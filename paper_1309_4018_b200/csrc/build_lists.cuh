@@ -76,7 +76,8 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     std::vector<int> anchor_of(ncells, 0);
     if (mixed) {
         int alevel = 0;
-        while (edge / (double)(1 << alevel) > 16.0 && alevel < PYGBE_MAXLEVEL) alevel++;
+        const double anchor_edge = getenv("PYGBE_ANCHOR_EDGE") ? atof(getenv("PYGBE_ANCHOR_EDGE")) : 16.0;   // tuning
+        while (edge / (double)(1 << alevel) > anchor_edge && alevel < PYGBE_MAXLEVEL) alevel++;
         std::vector<int> panel_anchor(R.np, 0);
         for (int c : leaves) {
             int a = c;
