@@ -73,7 +73,8 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
     {
         int occ = 1;
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_gm_arnoldi, GM_THREADS, 0));
-        arn_grid = (int)std::max(1L, std::min((long)occ * h->n_sm, (long)cdiv(n, 256)));
+        const long arn_rows = getenv("PYGBE_ARN_ROWS") ? std::max(32L, atol(getenv("PYGBE_ARN_ROWS"))) : 256L;   // tuning
+        arn_grid = (int)std::max(1L, std::min((long)occ * h->n_sm, (long)cdiv(n, arn_rows)));
     }
     CUDA_TRY(cudaMemsetAsync(G.h1, 0, (size_t)(G.m + 2) * sizeof(double), st));   // k_gm_arnoldi keeps h1 zero between steps
     const bool pc = h->precond == 1 && h->pinv != nullptr;
