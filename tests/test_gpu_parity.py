@@ -244,6 +244,32 @@ def test_treecode_error_decreases_with_order(env):
     assert all(b < a for a, b in zip(errs, errs[1:]))
 
 
+def test_group_mac_on_own_targets_is_within_the_bound_and_shortens_the_lists(env, monkeypatch):
+    """Reading A9: a cell is accepted for a group iff eq. (15) holds for every target.  The traversal decides that
+    from the group's bounding volume where it can and from the 64 points themselves where the bound is undecided;
+    with PYGBE_BOUND_MAC set it uses the bound alone.  Both must meet the 1e-4 bar; the exact test must give
+    shorter direct lists (every cell the bound accepts is also accepted by the exact minimum)."""
+    pg, torch, orc = env
+    prob = W.kirkwood_problem(4)
+    o = orc.Oracle(prob)
+    x = np.random.default_rng(21).normal(size=o.n)
+    yo = o.matvec(x)
+    res = {}
+    for mode in ("exact", "bound"):
+        if mode == "bound":
+            monkeypatch.setenv("PYGBE_BOUND_MAC", "1")
+        else:
+            monkeypatch.delenv("PYGBE_BOUND_MAC", raising=False)
+        h, y = gpu_matvec(pg, torch, prob, x, K=4, P=6, theta=0.5)
+        st = h.stats()
+        res[mode] = (rel(y, yo), st["p2p_pairs"], st["m2p_evals"])
+        h.close()
+    monkeypatch.delenv("PYGBE_BOUND_MAC", raising=False)
+    assert res["exact"][0] <= TOL_TREE and res["bound"][0] <= TOL_TREE
+    assert res["exact"][1] < 0.9 * res["bound"][1]
+    assert res["bound"][0] <= res["exact"][0]          # the bound is the stricter acceptance
+
+
 @pytest.mark.parametrize("maker,level", [(W.kirkwood_problem, 3), (W.stern_sphere_problem, 3)])
 def test_mixed_precision_other_orders(env, maker, level):
     """fp32 evaluation of the regrouped Taylor series (csrc/m2p.cuh) at orders other than the benchmark's, with
