@@ -1,8 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- headline benchmark of the treecode BEM matvec (BASELINE.json metric) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config kirkwood_l5]
-                    [--precision fp64|mixed]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config binding_complex]
+                    [--precision fp64|mixed] [--sweep]
 
 A step = one matvec y = A x (the hot loop of PAPER.md:169: "one evaluation of the treecode per iteration")
 of the whole coupled system: density weighting, P2M, upward pass, M2P, P2P, near-field corrections and
@@ -11,7 +11,10 @@ block combination for every region.  value = direct-equivalent interactions per 
 same through pygbe_matvec_host (pinned host buffers, copies inside the timed region).  The second half of
 the metric, GMRES time-to-solution, is reported under "solve" (create + rhs + GMRES + energy).
 L2 is flushed between timed iterations.  Multi-GPU: independent replicas of the workload, one per rank
-("replicas only"), no data-path collective.
+("replicas only"), no data-path collective.  The default workload is the largest single-GPU
+configuration of BASELINE.json (configs[4], the 1.08 M-panel complex of the binding-energy problem, P = 8,
+fp32 kernels with fp64 accumulation); --config selects the others, --sweep prints one line per configuration
+(create / matvec / solve times, energies: the table of BASELINE.md section 5).
 """
 import argparse
 import json
@@ -31,19 +34,43 @@ METRIC = "BEM matvec interactions/s (Laplace+Yukawa), direct-equivalent"
 UNIT = "interactions/s"
 
 
+CONFIGS = {
+    # name: (builder, create keywords, GMRES tol (fp64, mixed), description)
+    "born_l3": (lambda W: W.born_problem(3), dict(K=4, P=6, theta=0.0), (1e-8, 1e-5),
+                "BASELINE.json configs[0]: Born sphere, icosphere level 3 (1280 panels), K=4, direct summation (theta=0)"),
+    "kirkwood_l5": (lambda W: W.kirkwood_problem(5), dict(K=4, P=6, theta=0.5), (1e-6, 1e-5),
+                    "BASELINE.json configs[1]: Kirkwood sphere R=10 A, icosphere level 5 (20480 panels), K=4, P=6, theta=0.5"),
+    "kirkwood_l6": (lambda W: W.kirkwood_problem(6), dict(K=4, P=6, theta=0.5), (1e-6, 1e-5),
+                    "Kirkwood sphere level 6 (81920 panels), K=4, P=6, theta=0.5"),
+    "protein_1000": (lambda W: W.cached("protein_1000_s105", lambda: W.protein_problem(1000, spacing=1.05)),
+                     dict(K=4, P=6, theta=0.5), (1e-6, 1e-5),
+                     "BASELINE.json configs[2]: synthetic protein, 1000 atoms, 41.5 k panels, K=4, P=6, theta=0.5"),
+    "multisurface_3000": (lambda W: W.cached("multisurface_3000_s112", lambda: W.multisurface_problem(3000, spacing=1.12)),
+                          dict(K=4, P=6, theta=0.5), (1e-6, 1e-5),
+                          "BASELINE.json configs[3]: 3000 atoms, 2 cavities, Stern surface, 157 k panels, 4 regions, K=4, P=6, theta=0.5"),
+    "binding_complex": (lambda W: W.cached("binding_complex_5000_500_s055",
+                                           lambda: W.binding_problems(5000, 500, spacing=0.55, only=("complex",))[0]),
+                        dict(K=4, P=8, theta=0.5), (1e-4, 1e-4),
+                        "BASELINE.json configs[4], the complex: receptor 5000 + ligand 500 atoms at 3 A, two dielectric bodies + "
+                        "one Stern surface, 1.08 M panels (4.3 M Gauss points), 3 regions, K=4, P=8, theta=0.5"),
+    "binding_receptor": (lambda W: W.cached("binding_receptor_5000_500_s055",
+                                            lambda: W.binding_problems(5000, 500, spacing=0.55, only=("receptor",))[1]),
+                         dict(K=4, P=8, theta=0.5), (1e-4, 1e-4),
+                         "BASELINE.json configs[4], the receptor alone: 5000 atoms + Stern surface, 0.86 M panels, K=4, P=8, theta=0.5"),
+    "binding_ligand": (lambda W: W.cached("binding_ligand_5000_500_s055",
+                                          lambda: W.binding_problems(5000, 500, spacing=0.55, only=("ligand",))[2]),
+                       dict(K=4, P=8, theta=0.5), (1e-4, 1e-4),
+                       "BASELINE.json configs[4], the ligand alone: 500 atoms + Stern surface, 0.23 M panels, K=4, P=8, theta=0.5"),
+}
+DEFAULT_CONFIG = "binding_complex"       # the largest single-GPU configuration of BASELINE.json (configs[4])
+
+
 def make_problem(name):
     import workloads as W
-    if name == "kirkwood_l5":
-        return W.kirkwood_problem(5), dict(K=4, P=6, theta=0.5), "BASELINE.json configs[1]: Kirkwood sphere R=10 A, icosphere level 5 (20480 panels), K=4, P=6, theta=0.5"
-    if name == "born_l3":
-        return W.born_problem(3), dict(K=4, P=6, theta=0.0), "BASELINE.json configs[0]: Born sphere, 1280 panels, direct"
-    if name == "kirkwood_l6":
-        return W.kirkwood_problem(6), dict(K=4, P=6, theta=0.5), "Kirkwood sphere level 6 (81920 panels), K=4, P=6, theta=0.5"
-    if name == "protein_1000":
-        return W.protein_problem(1000, spacing=1.05), dict(K=4, P=6, theta=0.5), "BASELINE.json configs[2] recipe: synthetic protein, 1000 atoms, ~41.5 k panels, K=4, P=6, theta=0.5"
-    if name == "multisurface_3000":
-        return W.multisurface_problem(3000, spacing=1.12), dict(K=4, P=6, theta=0.5), "BASELINE.json configs[3] recipe: 3000 atoms, 2 cavities, Stern surface, ~157 k panels, 4 regions, K=4, P=6, theta=0.5"
-    raise SystemExit(f"unknown config {name}")
+    if name not in CONFIGS:
+        raise SystemExit(f"unknown config {name}; known: {', '.join(CONFIGS)}")
+    build, kw, tols, desc = CONFIGS[name]
+    return build(W), dict(kw), desc
 
 
 # ------------------------------------------------------------------------------------------ flop model
@@ -53,9 +80,9 @@ def m2p_nw(P):
 
 
 def m2p_flops(P, yukawa):
-    """Algorithmic flops of one (target, cell) Taylor evaluation as the kernel does it (m2p.cuh; multiply-add
-    = 2, rsqrt = exp = 1): offset and radius, the Nc - 1 monomials d^e, one FMA per W_{m,e} for every region
-    in `yukawa` (a tuple of booleans: one entry, or two for twin regions evaluated in one pass), and per
+    """Algorithmic flops of one (target, cell) Taylor evaluation as the regrouped kernels do it (m2p.cuh;
+    multiply-add = 2, rsqrt = exp = 1): offset and radius, the Nc - 1 monomials d^e, one FMA per W_{m,e} for every
+    region in `yukawa` (a tuple of booleans: one entry, or two for twin regions evaluated in one pass), and per
     region the P + 1 radial derivatives F^(m) and their dot product with Q_m.  DESIGN.md 'Flop model'."""
     if isinstance(yukawa, bool):
         yukawa = (yukawa,)
@@ -68,8 +95,33 @@ def m2p_flops(P, yukawa):
     return f
 
 
+def m2p_lap_flops(P):
+    """One (target, cell) evaluation of the Laplace form (k_m2p_lap): d (3), r^2 (5), rsqrt (1), 1/r^2 (1),
+    a / r^2 (1), u = d a / r^2 (3), Nc - 1 Horner FMAs, times 1/r (1), accumulate (1)."""
+    nc = (P + 1) * (P + 2) * (P + 3) // 6
+    return 16 + 2 * (nc - 1)
+
+
 P2P_FLOPS = {False: 19, True: 25}     # per (target, Gauss point) pair, Laplace / Yukawa (rsqrt, exp = 1)
 P2P_FLOPS_FUSED = 30                  # Laplace + Yukawa of twin regions sharing d, r^2, 1/r, n.d
+
+
+def launch_flops(rec, P, kappa):
+    """Algorithmic flops of one launch of a compute-bound kernel from the record of pygbe_launch_times."""
+    yA = float(kappa[rec["region"]]) > 0
+    twin = rec["twin_region"] >= 0
+    yB = twin and float(kappa[rec["twin_region"]]) > 0
+    if rec["stage"] == "p2p":
+        if twin:
+            per = P2P_FLOPS_FUSED if yA != yB else (2 * P2P_FLOPS[yA] - 9)      # shared d, r^2, 1/r, n.d
+        else:
+            per = P2P_FLOPS[yA]
+        return rec["units"] * per
+    if rec["stage"] == "m2p":
+        if "lap" in rec["kernel"]:
+            return rec["units"] * m2p_lap_flops(P)
+        return rec["units"] * m2p_flops(P, (yA, yB) if twin else yA)
+    return 0
 
 
 def clocks_sampler(stop, out):
@@ -97,8 +149,9 @@ def summarize_clocks(samples):
 
 # ------------------------------------------------------------------------------------- reference arm
 def oracle_sample(prob, kw, seconds_target=15.0):
-    """Time the oracle (as it stands, all host cores through its own OpenMP loop) on a bounded sample of
-    rows of the same matvec; returns (interactions/s, cores, description, seconds)."""
+    """Time the oracle (as it stands, through its own OpenMP loop over rows: all host cores unless OMP_NUM_THREADS
+    says otherwise) on a bounded sample of rows of the same matvec; returns (interactions/s, threads, description,
+    seconds)."""
     import oracle
     o = oracle.Oracle(prob, K=kw["K"])
     rng = np.random.default_rng(42)
@@ -110,7 +163,7 @@ def oracle_sample(prob, kw, seconds_target=15.0):
         npts[S.region_out] += kw["K"] * S.n_panels
     row_cost = np.concatenate([np.concatenate([np.full(S.n_panels, npts[S.region_in]), np.full(S.n_panels, npts[S.region_out])])
                                for S in prob.surfaces])
-    probe = np.sort(rng.choice(o.n, 64, replace=False))
+    probe = np.sort(rng.choice(o.n, min(64, o.n), replace=False))
     t = time.perf_counter(); o.matvec(x, probe); dt = time.perf_counter() - t
     nrows = int(min(o.n, max(64, 64 * seconds_target / max(dt, 1e-3))))
     rows = np.sort(rng.choice(o.n, nrows, replace=False))
@@ -125,6 +178,20 @@ def oracle_sample(prob, kw, seconds_target=15.0):
     return work / dt, oracle.num_threads(), f"{reps} x {nrows} of {o.n} seeded rows of one matvec ({work:.3g} interactions, {dt:.1f} s)", dt
 
 
+def oracle_single_thread(config, seconds=8.0):
+    """The same sample on ONE host thread ("single-threaded and with all cores"): a child process with
+    OMP_NUM_THREADS=1 running this file's reference arm, since the oracle reads its thread count at load."""
+    env = dict(os.environ, OMP_NUM_THREADS="1", RANK="0", WORLD_SIZE="1")
+    try:
+        r = subprocess.run([sys.executable, os.path.abspath(__file__), "--impl", "reference", "--config", config, "--steps", "1",
+                            "--warmup", "0", "--seconds", str(seconds)], capture_output=True, text=True, timeout=600, env=env)
+        line = json.loads(r.stdout.strip().splitlines()[-1])
+        return {"value": line["value"], "unit": UNIT, "cores": line["cpu_baseline"]["cores"], "kind": "oracle",
+                "sample": line["cpu_baseline"]["sample"]}
+    except Exception as e:                           # reported, never fatal for the GPU line
+        return {"value": None, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"failed: {e}"}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -133,9 +200,10 @@ def run_reference(args):
     vals, secs = [], []
     for _ in range(args.warmup):
         oracle_sample(prob, kw, seconds_target=1.0)
-    sample = ""
+    sample, cores = "", 0
+    per_step = args.seconds if args.seconds > 0 else max(2.0, 60.0 / max(args.steps, 1))
     for _ in range(args.steps):
-        v, cores, sample, dt = oracle_sample(prob, kw, seconds_target=max(2.0, 60.0 / max(args.steps, 1)))
+        v, cores, sample, dt = oracle_sample(prob, kw, seconds_target=per_step)
         vals.append(v); secs.append(dt)
     v = float(np.mean(vals))
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
@@ -177,6 +245,15 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     pg.lib()
+    if args.sweep:
+        if rank == 0:
+            for name in ("born_l3", "kirkwood_l5", "protein_1000", "multisurface_3000", "binding_complex", "binding_receptor",
+                         "binding_ligand"):
+                for prec in ("fp64", "mixed"):
+                    a = argparse.Namespace(**dict(vars(args), config=name))
+                    line = measure(a, prec, pg, torch, None, 1, 0, local, full=False, brief=True)
+                    print(json.dumps({"sweep": name, "precision": prec, **{k: line[k] for k in ("value", "ms_per_step", "config", "solve", "kernels", "hbm_passes")}}), flush=True)
+        return
     other = "fp64" if args.precision == "mixed" else "mixed"
     line = measure(args, args.precision, pg, torch, dist, world, rank, local, full=True)
     second = measure(args, other, pg, torch, dist, world, rank, local, full=False)
@@ -184,27 +261,32 @@ def run_ours(args):
         dist.barrier()
         dist.destroy_process_group()
     if line is not None:
-        keep = ("value", "ms_per_step", "dtype", "e2e", "gpu_launches", "roofline", "solve", "actual")
+        keep = ("value", "ms_per_step", "dtype", "e2e", "gpu_launches", "roofline", "kernels", "hbm_passes", "solve", "actual")
         line["other_precision"] = {k: second[k] for k in keep if k in second}
         line["other_precision"]["precision"] = other
         print(json.dumps(line))
 
 
-def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
+def measure(args, precision_name, pg, torch, dist, world, rank, local, full, brief=False):
     prob, kw, desc = make_problem(args.config)
+    tols = CONFIGS[args.config][2]
+    big = prob.n_panels > 300_000
     precision = pg.PRECISION_MIXED if precision_name == "mixed" else pg.PRECISION_FP64
-    # create is timed warm, like the kernels: the first handle of a process pays the CUDA module load and the
-    # growth of the stream-ordered memory pool (reported as create_first_ms)
+    # create is timed warm, like the kernels: the first handle of a process pays the CUDA module load and the growth
+    # of the memory pools (reported as create_first_ms).  A create through the binding's default path is the size
+    # query (pygbe_workspace_size, a dry run of the list sizing), one torch allocation, and pygbe_create into it.
     t0 = time.perf_counter()
     pg.Handle.from_problem(prob, precision=precision, device=local, **kw).close()
     torch.cuda.synchronize()
     create_first_ms = 1e3 * (time.perf_counter() - t0)
+    mem0 = torch.cuda.memory_allocated(local)
     t0 = time.perf_counter()
     h = pg.Handle.from_problem(prob, precision=precision, device=local, **kw)
     torch.cuda.synchronize()
-    create_ms = 1e3 * (time.perf_counter() - t0)
+    create_total_ms = 1e3 * (time.perf_counter() - t0)
     st = h.stats()
     n = h.n
+    torch_bytes = torch.cuda.memory_allocated(local) - mem0
     rng = np.random.default_rng(7)
     x = torch.tensor(rng.normal(size=n), device="cuda")
     y = torch.empty_like(x)
@@ -261,26 +343,16 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
 
     line = None
     if rank == 0:
-        # ---- per-stage timers (profiled matvecs are not the ones timed above)
+        # ---- per-launch timers (profiled matvecs run on one stream and are not the ones timed above)
+        psteps = max(3, min(args.steps, 10))
         h.profile(True)
-        for _ in range(args.steps):
+        for _ in range(psteps):
             flush.zero_()
             h.matvec(x, y)
         stages = h.stage_times()
+        recs = h.launch_times()
         h.profile(False)
-        nreg_launch = {k: v[1] / args.steps for k, v in stages.items()}
-        stage_ms = {k: v[0] / args.steps for k, v in stages.items()}
-        dom = max(("p2p", "m2p"), key=lambda k: stage_ms[k])
-        yuk = [float(k) > 0 for k in prob.kappa]
-        # algorithmic flops of the dominant stage per matvec (all regions), DESIGN.md "Flop model"
-        # single-surface configs: one Laplace and one Yukawa region with identical lists (twin regions,
-        # evaluated in one fused pass: 30 flops per geometric pair instead of 19 + 25)
-        nreg = len(yuk)
-        if dom == "p2p":
-            flops = st["p2p_pairs"] / nreg * (P2P_FLOPS_FUSED if nreg == 2 else sum(P2P_FLOPS[yk] for yk in yuk))
-        else:
-            # twin regions share one fused evaluation per (target, cell); otherwise one evaluation per region
-            flops = st["m2p_evals"] / nreg * (m2p_flops(kw["P"], tuple(yuk)) if nreg == 2 else sum(m2p_flops(kw["P"], yk) for yk in yuk))
+        stage_ms = {k: v[0] / psteps for k, v in stages.items()}
         peaks = pg.alu_peaks(local)
         mp = {}
         try:
@@ -288,69 +360,86 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full):
         except Exception:
             pass
         sm_max = float(mp.get("sm_max_mhz", 1965.0))
+        hbm_peak = float(mp.get("hbm_gbs", 6540.2))
         nominal = {"f64": 148 * 64 * 2 * sm_max * 1e6 / 1e12, "f32": 148 * 128 * 2 * sm_max * 1e6 / 1e12}
         dt = "f32" if precision == pg.PRECISION_MIXED else "f64"
-        achieved = flops / (stage_ms[dom] * 1e-3) / 1e12
-        # dram__bytes_read.sum + dram__bytes_write.sum of the stage's launches from the ncu --set full capture of this
-        # command (profiles/r3c_group_mac_path.md, config kirkwood_l5): bytes per matvec, both regions; else null
-        traffic = {("kirkwood_l5", "f32", "m2p"): 2.65e6, ("kirkwood_l5", "f32", "p2p"): 3.78e6}.get((args.config, dt, dom))
-        kname = {"m2p": "%s<%d,%s>" % ("k_m2p_twin2 / k_m2p_single2 (two targets per thread, packed f32x2)" if dt == "f32" else "k_m2p_dbl2 / k_m2p<double>", kw["P"],
-                                       "twin regions fused" if nreg == 2 else "per tree"),
-                 "p2p": "%s<%s>" % ("k_p2p_quad (packed f32x2)" if dt == "f32" and kw["K"] % 4 == 0 else "k_p2p<%s>" % ("float" if dt == "f32" else "double"),
-                                    "twin regions fused" if nreg == 2 else "per region")}[dom]
-        roofline = {"bound": "alu", "kernel": "%s, %d launches/matvec" % (kname, round(nreg_launch[dom])),
-                    "achieved": achieved, "peak": nominal[dt], "unit": "TFLOP/s", "frac": achieved / nominal[dt],
-                    "peak_kind": "derived: 148 SM x %d lanes x 2 x %.0f MHz (DESIGN.md); FMA micro-benchmark in this run: %.1f TFLOP/s"
+        kernels, passes = [], []
+        for r in recs:
+            per_ms = r["ms"] / max(r["launches"], 1)
+            base = {"kernel": r["kernel"], "stage": r["stage"], "region": r["region"], "twin_region": r["twin_region"],
+                    "ms_per_launch": per_ms, "units_per_launch": r["units"]}
+            if r["stage"] in ("p2p", "m2p"):
+                fl = launch_flops(r, kw["P"], prob.kappa)
+                tf = fl / (per_ms * 1e-3) / 1e12 if per_ms > 0 else 0.0
+                kernels.append({**base, "flops_per_launch": fl, "tflops": tf, "frac": tf / nominal[dt]})
+            else:
+                gbs = r["bytes"] / (per_ms * 1e-3) / 1e9 if per_ms > 0 else 0.0
+                passes.append({**base, "bytes_per_launch": r["bytes"], "gbs": gbs, "frac_of_hbm_peak": gbs / hbm_peak})
+        dom = max(kernels, key=lambda k: k["ms_per_launch"])
+        roofline = {"bound": "alu", "kernel": "%s, region %d%s, 1 launch/matvec" % (
+                        dom["kernel"].replace("<P", "<%d" % kw["P"]), dom["region"],
+                        (" + twin %d" % dom["twin_region"]) if dom["twin_region"] >= 0 else ""),
+                    "achieved": dom["tflops"], "peak": nominal[dt], "unit": "TFLOP/s", "frac": dom["frac"],
+                    "peak_kind": "derived: 148 SM x %d lanes x 2 x %.0f MHz (DESIGN.md 7); FMA micro-benchmark in this run: %.1f TFLOP/s"
                                  % (64 if dt == "f64" else 128, sm_max, peaks["fp64_tflops" if dt == "f64" else "fp32_tflops"]),
-                    "traffic": traffic, "stage_ms": stage_ms, "alu_peaks_measured": peaks,
-                    "flops_per_launchset": flops, "flop_model": "exact for twin regions" if nreg == 2 else "regions weighted equally (approximate)",
-                    "hbm_peak_gbs": mp.get("hbm_gbs")}
+                    "traffic": None, "ms_per_launch": dom["ms_per_launch"], "flops_per_launch": dom["flops_per_launch"],
+                    "units_per_launch": dom["units_per_launch"],
+                    "flop_model": "DESIGN.md 7 'Flop model' (bench.py launch_flops)", "stage_ms": stage_ms,
+                    "alu_peaks_measured": peaks, "hbm_peak_gbs": hbm_peak}
         if dt == "f32" and peaks.get("fp32_mix_tflops"):
             # context, not the denominator: what the FP32 pipe delivers on a register-resident FMUL + 3-register
-            # FFMA mix (pygbe_alu_peaks out[3]), the practical ceiling of the recurrences' mix
-            roofline["frac_of_mix_ceiling"] = achieved / peaks["fp32_mix_tflops"]
-        # ---- time-to-solution (second half of the metric): create + rhs + GMRES + energy, host buffers
-        # the first solve of a handle also grows the memory pool by the Krylov basis (reported as solve_first_ms);
-        # solve_ms is the median of three further complete solves, warm like create_ms
-        tol = 1e-6 if dt == "f64" else 1e-5
+            # FFMA mix (pygbe_alu_peaks out[3]), the practical ceiling of a mixed FMUL / FFMA stream
+            roofline["frac_of_mix_ceiling"] = dom["tflops"] / peaks["fp32_mix_tflops"]
+        # ---- time-to-solution (second half of the metric): create + rhs + GMRES + energy, host buffers.  The first
+        # solve of a handle is reported apart on the small configs (warm-up of the cooperative launch); the large
+        # ones run one solve
+        tol = tols[0] if dt == "f64" else tols[1]
         solve_times = []
-        for _ in range(4):
+        for _ in range(1 if (big or brief) else 4):
             t = time.perf_counter()
-            xs, iters, rr, es, ec = h.solve_host(tol=tol)
+            xs, iters, rr, es, ec = h.solve_host(tol=tol, max_iter=3000)
             solve_times.append(1e3 * (time.perf_counter() - t))
-        solve_first_ms, solve_ms = solve_times[0], sorted(solve_times[1:])[1]
-        solve = {"create_ms": create_ms, "create_first_ms": create_first_ms, "solve_ms": solve_ms, "solve_first_ms": solve_first_ms,
-                 "time_to_solution_ms": create_ms + solve_ms,
+        solve_first_ms = solve_times[0]
+        solve_ms = sorted(solve_times[1:])[1] if len(solve_times) >= 4 else solve_times[0]
+        solve = {"create_ms": create_total_ms, "create_first_ms": create_first_ms,
+                 "create_breakdown_ms": {"workspace_size_query": h.workspace_query_ms, "pygbe_create": st["create_ms"]},
+                 "solve_ms": solve_ms, "solve_first_ms": solve_first_ms, "time_to_solution_ms": create_total_ms + solve_ms,
                  "gmres_iters": iters, "rel_resid": rr, "tol": tol, "E_solv_kJ_mol": es, "E_coul_kJ_mol": ec,
-                 "preconditioner": "none (reading A16)"}
-        # the same with the optional block-diagonal right preconditioner (pygbe_options.precond = 1)
-        t = time.perf_counter()
-        h2 = pg.Handle.from_problem(prob, precision=precision, device=local, precond=1, **kw)
-        torch.cuda.synchronize()
-        c2 = 1e3 * (time.perf_counter() - t)
-        t = time.perf_counter()
-        _, it2, rr2, es2, ec2 = h2.solve_host(tol=tol, want_x=False)
-        s2 = 1e3 * (time.perf_counter() - t)
-        h2.close()
-        solve["block_diagonal"] = {"create_ms": c2, "solve_ms": s2, "time_to_solution_ms": c2 + s2, "gmres_iters": it2,
-                                   "rel_resid": rr2, "E_solv_kJ_mol": es2}
-        # ---- oracle on the host cores, bounded sample
-        cv, cores, sample = (None, None, None)
+                 "ms_per_iteration": solve_ms / max(iters, 1), "preconditioner": "none (reading A16)",
+                 "device_bytes": st["device_bytes"], "workspace_bytes": int(h.workspace.numel()) if h.workspace is not None else 0,
+                 "torch_allocated_delta_bytes": int(torch_bytes)}
+        if not brief:
+            # the same with the optional block-diagonal right preconditioner (pygbe_options.precond = 1)
+            t = time.perf_counter()
+            h2 = pg.Handle.from_problem(prob, precision=precision, device=local, precond=1, **kw)
+            torch.cuda.synchronize()
+            c2 = 1e3 * (time.perf_counter() - t)
+            t = time.perf_counter()
+            _, it2, rr2, es2, ec2 = h2.solve_host(tol=tol, want_x=False, max_iter=3000)
+            s2 = 1e3 * (time.perf_counter() - t)
+            h2.close()
+            solve["block_diagonal"] = {"create_ms": c2, "solve_ms": s2, "time_to_solution_ms": c2 + s2, "gmres_iters": it2,
+                                       "rel_resid": rr2, "E_solv_kJ_mol": es2}
+        # ---- oracle on the host cores, bounded samples: all cores and one thread
+        cpu = {"value": None, "unit": UNIT, "cores": None, "kind": "oracle", "sample": None}
         if full:
             cv, cores, sample, _ = oracle_sample(prob, kw, seconds_target=15.0)
+            cpu = {"value": cv, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                   "single_thread": oracle_single_thread(args.config)}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": dt, "data": "synthetic",
-                "config": {"workload": desc, "n_panels": st["n_panels"], "n_unknowns": st["n_unknowns"],
+                "config": {"workload": desc, "name": args.config, "n_panels": st["n_panels"], "n_unknowns": st["n_unknowns"],
+                           "n_regions": st["n_regions"], "n_charges": st["n_charges"],
                            "direct_equiv_interactions": st["direct_equiv"], "p2p_pairs": st["p2p_pairs"],
-                           "m2p_evals": st["m2p_evals"], "precision": precision_name,
+                           "m2p_evals": st["m2p_evals"], "precision": precision_name, **kw,
                            "l2": "flushed between timed iterations (256 MB write)",
                            "parallelism": "replicas only" if world > 1 else "single GPU"},
                 "clocks": summarize_clocks(samples),
                 "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n},
                 "gpu_launches": int(launches),
-                "roofline": roofline,
-                "cpu_baseline": {"value": cv, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+                "roofline": roofline, "kernels": kernels, "hbm_passes": passes,
+                "cpu_baseline": cpu,
                 "solve": solve,
                 "actual": {"p2p_pairs_per_s": st["p2p_pairs"] / (stage_ms["p2p"] * 1e-3) if stage_ms["p2p"] > 0 else None,
                            "m2p_evals_per_s": st["m2p_evals"] / (stage_ms["m2p"] * 1e-3) if stage_ms["m2p"] > 0 else None}}
@@ -364,8 +453,10 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="kirkwood_l5")
+    ap.add_argument("--config", default=DEFAULT_CONFIG, choices=sorted(CONFIGS))
     ap.add_argument("--precision", default="mixed", choices=["fp64", "mixed"])
+    ap.add_argument("--seconds", type=float, default=0.0, help="reference arm: CPU seconds per step (default 60 / steps)")
+    ap.add_argument("--sweep", action="store_true", help="one JSON line per configuration and precision (rank 0, one GPU)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

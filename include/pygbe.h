@@ -27,8 +27,14 @@
  *                Green's functions carry 1/(4 pi); the right-hand side is sum_k q_k G(x_i,r_k)/eps.
  *   Memory       pointers marked HOST are host memory, read during the call and never retained;
  *                pointers marked DEVICE are device memory on the handle's device, owned by the caller
- *                (e.g. torch tensors), fp64, pygbe_num_unknowns() long.  The library allocates its own
- *                internal device memory (reported by pygbe_stats) and frees it in pygbe_destroy.
+ *                (e.g. torch tensors), fp64, pygbe_num_unknowns() long.  Internal device memory: if
+ *                pygbe_options.workspace is given, EVERY device array of the handle (geometry, tree,
+ *                lists, corrections, multipoles, GMRES basis, staging) is carved out of that block and
+ *                the library allocates nothing else on the device; its size is queried first with
+ *                pygbe_workspace_size, and a block that is too small gives PYGBE_ENOMEM.  The block stays
+ *                owned by the caller and must outlive the handle.  Without a workspace the library takes
+ *                its memory from a pool of its own (never the device's default pool) and returns it in
+ *                pygbe_destroy.  pygbe_stats reports the bytes in use either way.
  *   Stream       all work of a handle is issued on the stream given in pygbe_options (a cudaStream_t,
  *                e.g. torch.cuda.current_stream().cuda_stream; NULL = legacy default stream).  Calls
  *                taking DEVICE pointers are asynchronous unless stated; one handle is not re-entrant.
@@ -48,8 +54,9 @@ extern "C" {
 
 #define PYGBE_OK        0
 #define PYGBE_EINVAL   (-1)  /* null pointer, bad size, unsupported K / P, theta < 0, bad region ids,  */
-                             /* open / inconsistently oriented mesh, zero-area triangle               */
-#define PYGBE_ENOMEM   (-2)  /* device or host allocation failed                                       */
+                             /* open / inconsistently oriented mesh, zero-area triangle, region graph  */
+                             /* (regions = nodes, surfaces = edges) not a tree                         */
+#define PYGBE_ENOMEM   (-2)  /* device or host allocation failed, or the workspace is too small         */
 #define PYGBE_ECUDA    (-3)  /* a CUDA call or kernel failed                                           */
 #define PYGBE_ENOCONV  (-4)  /* GMRES reached max_iter; x and the residual are still returned          */
 
@@ -89,7 +96,13 @@ typedef struct {
                         /* 1 block-diagonal: per panel the 2x2 block [[1/2, -V_ii^in], [1/2, c V_ii^out]] of   */
                         /* its two rows and two unknowns (self integrals only).  Same stopping test, since a   */
                         /* right preconditioner leaves the residual b - A x unchanged                          */
-    int32_t reserved[6];
+    int32_t group_mac;  /* MAC of a target group (reading A9): 0 eq. (15) for every target of the group, decided  */
+                        /* from the group's own points where its bounding volume cannot [0]; 1 bounding volume  */
+                        /* only (stricter: longer direct lists, smaller error)                                  */
+    void   *workspace;  /* DEVICE block that holds every internal array of the handle, or NULL [NULL]: see      */
+                        /* "Memory" above; 256-byte aligned, owned by the caller, must outlive the handle        */
+    size_t  workspace_bytes;   /* size of that block; at least what pygbe_workspace_size returned                */
+    int32_t reserved[4];
 } pygbe_options;
 
 /* Counters and timings filled by pygbe_stats. */
@@ -101,7 +114,8 @@ typedef struct {
     int64_t m2p_evals;           /* (target, accepted cell) Taylor evaluations per matvec              */
     int64_t direct_equiv;        /* sum_regions N_targets x N_points: interactions of the dense matvec */
     int64_t near_nnz;            /* entries of the singular / near-singular correction (a8)            */
-    int64_t device_bytes;        /* internal device memory held by the handle                          */
+    int64_t device_bytes;        /* internal device memory in use by the handle (workspace or pool)    */
+    int64_t workspace_high_water;/* workspace bytes the allocations made so far needed at their peak   */
     int64_t n_matvec;            /* matvecs executed so far                                            */
     int64_t kernels_per_matvec;  /* kernel launches one pygbe_matvec issues                            */
     int64_t kernel_launches;     /* all kernel launches issued by this handle so far                   */
@@ -128,6 +142,17 @@ int pygbe_create(const pygbe_surface *surfaces, int32_t n_surfaces, const pygbe_
 
 void pygbe_destroy(pygbe_handle *h);
 
+/* Size in bytes of the workspace that pygbe_create with the same arguments needs, including the buffers of
+ * pygbe_solve for a restart length of gmres_restart (<= 0: 100), of the *_host entry points and of
+ * pygbe_energy ("workspace supplied by the caller, size queried first").  The interaction lists depend on the
+ * geometry, so this is a dry run of create's sizing (tree, traversal, list and correction patterns; no
+ * values are computed) in memory of the library's own pool, released before returning.  opt->workspace is
+ * ignored.  Synchronous; same argument checks and error codes as pygbe_create. */
+int pygbe_workspace_size(const pygbe_surface *surfaces, int32_t n_surfaces, const pygbe_charges *charges,
+                         const double *eps, const double *kappa, int32_t n_regions,
+                         int32_t K, int32_t P, double theta, const pygbe_options *opt,
+                         int32_t gmres_restart, size_t *bytes);
+
 /* 2 * total number of panels; < 0 on a NULL handle. */
 int64_t pygbe_num_unknowns(const pygbe_handle *h);
 
@@ -143,10 +168,17 @@ int pygbe_matvec_host(pygbe_handle *h, const double *x_host, double *y_host);
  * b_dev: DEVICE.  Asynchronous. */
 int pygbe_rhs(pygbe_handle *h, double *b_dev);
 
-/* Restarted GMRES, x0 = 0, no preconditioner, stop at ||b - A x||/||b|| <= tol
- * (reading A16).  The whole iteration runs on the device; the host only polls a convergence flag.
- * x_dev: DEVICE, receives the solution.  iters, rel_resid: HOST, may be NULL.  Synchronous.
- * Returns PYGBE_ENOCONV if max_iter matvecs did not reach tol. */
+/* Restarted GMRES, x0 = 0, no preconditioner unless pygbe_options.precond, stop at
+ * ||b - A x|| / ||b|| <= tol (reading A16).  The whole iteration runs on the device; the host only polls flags.
+ * A cycle ends when the Arnoldi / Givens estimate of the residual reaches tol; convergence is DECLARED only when
+ * the residual recomputed from b - A x with one more matvec is within tol, and that recomputed value is what
+ * rel_resid returns.  If the two keep disagreeing (tol below what the operator's arithmetic attains: about 1e-6
+ * relative for PYGBE_PRECISION_MIXED, 1e-12 for FP64 with the treecode's non-deterministic summation order) the
+ * call returns PYGBE_ENOCONV.  A breakdown (zero pivot) leaves that direction out instead of dividing by zero.
+ * x_dev: DEVICE, receives the solution.  iters (matvecs inside Arnoldi steps), rel_resid: HOST, may be NULL.
+ * Synchronous.  Returns PYGBE_ENOCONV if max_iter iterations did not reach tol (x and rel_resid still returned).
+ * In a caller-supplied workspace the GMRES buffers were sized for the gmres_restart given to
+ * pygbe_workspace_size: a longer restart gives PYGBE_ENOMEM. */
 int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t max_iter, double *x_dev,
                 int32_t *iters, double *rel_resid);
 
@@ -183,6 +215,23 @@ int pygbe_stats(const pygbe_handle *h, pygbe_stats_t *out);
 int pygbe_profile(pygbe_handle *h, int enable);
 int pygbe_stage_times(pygbe_handle *h, double *ms, int64_t *launches);
 
+/* The same timers per kernel launch of a matvec, i.e. per (stage, tree): accumulated milliseconds and number
+ * of launches since pygbe_profile(h, 1), the work one launch does and the bytes it has to move at least
+ * (inputs read once + outputs written once), from which bench.py forms the roofline numbers.
+ * out: HOST array of max_out records; *n_out receives the number written.  Synchronises the stream. */
+typedef struct {
+    int32_t stage;       /* PYGBE_STAGE_*                                                                 */
+    int32_t region;      /* region id of the tree owner the launch works on                               */
+    int32_t twin_region; /* region fused into the same launch (twin regions), or -1                       */
+    int32_t launches;    /* launches accumulated                                                          */
+    double  ms;          /* accumulated milliseconds                                                      */
+    int64_t units;       /* per launch: P2P (target, Gauss point) pairs; M2P (target, cell) evaluations   */
+                         /* (a fused twin pair counts once here); P2M panels; M2M cells; else rows / points */
+    int64_t bytes;       /* per launch: algorithmic bytes (HBM-bound stages; 0 where not meaningful)      */
+    char    kernel[64];  /* kernel name                                                                   */
+} pygbe_launch_info;
+int pygbe_launch_times(pygbe_handle *h, pygbe_launch_info *out, int32_t max_out, int32_t *n_out);
+
 /* Thread-local message of the last failing call ("" if none). */
 const char *pygbe_last_error(void);
 
@@ -192,7 +241,7 @@ const char *pygbe_last_error(void);
  * recurrence-like instruction mix of M2P / P2P; FMA = 2 flops, MUL = 1).  out4: HOST, 4 doubles. */
 int pygbe_alu_peaks(int32_t device, double *out4);
 
-/* Library / build identification, e.g. "pygbe-b200 0.1 sm_100a". */
+/* Library / build identification, e.g. "pygbe-b200 0.3 sm_100a". */
 const char *pygbe_version(void);
 
 #ifdef __cplusplus

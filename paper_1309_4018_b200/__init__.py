@@ -38,16 +38,22 @@ class pygbe_charges(C.Structure):
 class pygbe_options(C.Structure):
     _fields_ = [("K_fine", C.c_int32), ("thres", C.c_double), ("N_k", C.c_int32), ("ncrit", C.c_int32),
                 ("precision", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p),
-                ("check_mesh", C.c_int32), ("precond", C.c_int32), ("reserved", C.c_int32 * 6)]
+                ("check_mesh", C.c_int32), ("precond", C.c_int32), ("group_mac", C.c_int32),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("reserved", C.c_int32 * 4)]
 
 
 class pygbe_stats_t(C.Structure):
     _fields_ = [(n, C.c_int64) for n in (
         "n_panels", "n_unknowns", "n_regions", "n_surfaces", "n_charges", "n_points", "n_cells", "n_leaves",
         "n_groups", "tree_depth", "p2p_pairs", "m2p_evals", "direct_equiv", "near_nnz", "device_bytes",
-        "n_matvec", "kernels_per_matvec", "kernel_launches")] + [
+        "workspace_high_water", "n_matvec", "kernels_per_matvec", "kernel_launches")] + [
         ("create_ms", C.c_double), ("last_solve_ms", C.c_double), ("last_iters", C.c_int32),
         ("P", C.c_int32), ("K", C.c_int32), ("precision", C.c_int32), ("theta", C.c_double)]
+
+
+class pygbe_launch_info(C.Structure):
+    _fields_ = [("stage", C.c_int32), ("region", C.c_int32), ("twin_region", C.c_int32), ("launches", C.c_int32),
+                ("ms", C.c_double), ("units", C.c_int64), ("bytes", C.c_int64), ("kernel", C.c_char * 64)]
 
 
 _lib = None
@@ -65,6 +71,8 @@ def lib():
     vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int32)
     L.pygbe_create.argtypes = [C.POINTER(pygbe_surface), C.c_int32, C.POINTER(pygbe_charges), dp, dp, C.c_int32,
                                C.c_int32, C.c_int32, C.c_double, C.POINTER(pygbe_options), C.POINTER(vp)]
+    L.pygbe_workspace_size.argtypes = L.pygbe_create.argtypes[:-1] + [C.c_int32, C.POINTER(C.c_size_t)]
+    L.pygbe_launch_times.argtypes = [vp, C.POINTER(pygbe_launch_info), C.c_int32, ip]
     L.pygbe_destroy.argtypes = [vp]
     L.pygbe_destroy.restype = None
     L.pygbe_num_unknowns.argtypes = [vp]
@@ -103,9 +111,14 @@ class Handle:
     """Owner of a pygbe_handle.  Methods mirror the C entry points one to one."""
 
     def __init__(self, surfaces, charges, eps, kappa, K=4, P=6, theta=0.5, K_fine=0, thres=0.0, N_k=0, ncrit=0,
-                 precision=PRECISION_FP64, device=0, stream=None, check_mesh=False, precond=0):
+                 precision=PRECISION_FP64, device=0, stream=None, check_mesh=False, precond=0, group_mac=0,
+                 workspace="torch", gmres_restart=100):
         """surfaces: list of (vertices [nv,3] f64, triangles [nt,3] i32, region_in, region_out);
-        charges: (xyz [nq,3], q [nq], region [nq] or None) or None."""
+        charges: (xyz [nq,3], q [nq], region [nq] or None) or None.
+        workspace: "torch" (default) -- query pygbe_workspace_size, allocate that block as a torch uint8 tensor
+        and hand it to pygbe_create, so that every byte of the handle lives in torch's allocator; a uint8 CUDA
+        tensor -- use it as the block; None -- let the library use its own pool.  gmres_restart sizes the GMRES
+        buffers inside the block."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("pygbe needs a CUDA device (there is no CPU fallback)")
@@ -133,11 +146,31 @@ class Handle:
         if stream is None:
             stream = torch.cuda.current_stream(device).cuda_stream
         opt = pygbe_options(K_fine=K_fine, thres=thres, N_k=N_k, ncrit=ncrit, precision=precision, device=device,
-                            stream=C.c_void_p(stream), check_mesh=int(check_mesh), precond=int(precond))
+                            stream=C.c_void_p(stream), check_mesh=int(check_mesh), precond=int(precond),
+                            group_mac=int(group_mac))
+        args = (arr, len(surfaces), C.byref(ch) if ch is not None else None,
+                eps.ctypes.data_as(C.POINTER(C.c_double)), kappa.ctypes.data_as(C.POINTER(C.c_double)),
+                len(eps), K, P, float(theta), C.byref(opt))
+        self.workspace = None
+        self.workspace_query_ms = 0.0
+        if isinstance(workspace, str):
+            if workspace != "torch":
+                raise ValueError("workspace must be 'torch', a uint8 CUDA tensor or None")
+            import time
+            t0 = time.perf_counter()
+            nbytes = C.c_size_t()
+            _check(L.pygbe_workspace_size(*args, int(gmres_restart), C.byref(nbytes)))
+            self.workspace_query_ms = 1e3 * (time.perf_counter() - t0)
+            workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=torch.device("cuda", device))
+        if workspace is not None:
+            if not (isinstance(workspace, torch.Tensor) and workspace.is_cuda and workspace.dtype == torch.uint8
+                    and workspace.is_contiguous()):
+                raise TypeError("workspace must be a contiguous uint8 CUDA tensor")
+            self.workspace = workspace                     # keeps the block alive as long as the handle
+            opt.workspace = C.c_void_p(workspace.data_ptr())
+            opt.workspace_bytes = workspace.numel()
         h = C.c_void_p()
-        _check(L.pygbe_create(arr, len(surfaces), C.byref(ch) if ch is not None else None,
-                              eps.ctypes.data_as(C.POINTER(C.c_double)), kappa.ctypes.data_as(C.POINTER(C.c_double)),
-                              len(eps), K, P, float(theta), C.byref(opt), C.byref(h)))
+        _check(L.pygbe_create(*args, C.byref(h)))
         self._h = h
         self.device = torch.device("cuda", device)
         self.n = int(L.pygbe_num_unknowns(h))
@@ -149,10 +182,17 @@ class Handle:
         surfaces = [(s.vertices, s.triangles, s.region_in, s.region_out) for s in p.surfaces]
         return cls(surfaces, (p.charge_xyz, p.charge_q, p.charge_region), p.eps, p.kappa, **kw)
 
+    @staticmethod
+    def workspace_size(p, gmres_restart=100, **kw):
+        """pygbe_workspace_size for a workloads.Problem-like object and the keyword arguments of Handle."""
+        kw = dict(kw, workspace=None)
+        return _workspace_size_of(p, gmres_restart, **kw)
+
     def close(self):
         if getattr(self, "_h", None):
             lib().pygbe_destroy(self._h)
             self._h = None
+        self.workspace = None
 
     def __del__(self):
         try:
@@ -225,10 +265,49 @@ class Handle:
         _check(lib().pygbe_stage_times(self._h, ms, ln))
         return {name: (ms[i], ln[i]) for i, name in enumerate(self.STAGES) if name != "reserved"}
 
+    def launch_times(self):
+        """Per kernel launch of the matvec since profile(True): list of dicts (stage, region, twin_region,
+        launches, ms, units, bytes, kernel); ms is accumulated over `launches` launches."""
+        buf = (pygbe_launch_info * 64)()
+        n = C.c_int32()
+        _check(lib().pygbe_launch_times(self._h, buf, 64, C.byref(n)))
+        return [dict(stage=self.STAGES[b.stage], region=b.region, twin_region=b.twin_region, launches=b.launches, ms=b.ms,
+                     units=b.units, bytes=b.bytes, kernel=b.kernel.decode()) for b in buf[:n.value]]
+
     def stats(self):
         s = pygbe_stats_t()
         _check(lib().pygbe_stats(self._h, C.byref(s)))
         return {name: getattr(s, name) for name, _ in pygbe_stats_t._fields_}
+
+
+def _workspace_size_of(p, gmres_restart, **kw):
+    """Marshalling for Handle.workspace_size (the arrays only need to live for the duration of the call)."""
+    L = lib()
+    surfaces = [(s.vertices, s.triangles, s.region_in, s.region_out) for s in p.surfaces]
+    keep = []
+    arr = (pygbe_surface * len(surfaces))()
+    for i, (v, t, rin, rout) in enumerate(surfaces):
+        v = np.ascontiguousarray(v, dtype=np.float64); t = np.ascontiguousarray(t, dtype=np.int32)
+        keep += [v, t]
+        arr[i] = pygbe_surface(v.ctypes.data_as(C.POINTER(C.c_double)), v.shape[0],
+                               t.ctypes.data_as(C.POINTER(C.c_int32)), t.shape[0], int(rin), int(rout))
+    ch = None
+    if len(p.charge_q) > 0:
+        xyz = np.ascontiguousarray(p.charge_xyz, dtype=np.float64).reshape(-1, 3)
+        q = np.ascontiguousarray(p.charge_q, dtype=np.float64).reshape(-1)
+        reg = np.ascontiguousarray(p.charge_region, dtype=np.int32).reshape(-1)
+        keep += [xyz, q, reg]
+        ch = pygbe_charges(xyz.ctypes.data_as(C.POINTER(C.c_double)), q.ctypes.data_as(C.POINTER(C.c_double)),
+                           reg.ctypes.data_as(C.POINTER(C.c_int32)), q.shape[0])
+    eps = np.ascontiguousarray(p.eps, dtype=np.float64); kappa = np.ascontiguousarray(p.kappa, dtype=np.float64)
+    K, P, theta = kw.pop("K", 4), kw.pop("P", 6), kw.pop("theta", 0.5)
+    kw.pop("workspace", None); kw.pop("stream", None)
+    opt = pygbe_options(**{k: (int(v) if k != "thres" else float(v)) for k, v in kw.items()})
+    nbytes = C.c_size_t()
+    _check(L.pygbe_workspace_size(arr, len(surfaces), C.byref(ch) if ch is not None else None,
+                                  eps.ctypes.data_as(C.POINTER(C.c_double)), kappa.ctypes.data_as(C.POINTER(C.c_double)),
+                                  len(eps), K, P, float(theta), C.byref(opt), int(gmres_restart), C.byref(nbytes)))
+    return nbytes.value
 
 
 def alu_peaks(device=0):

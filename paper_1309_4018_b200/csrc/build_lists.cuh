@@ -76,7 +76,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     std::vector<int> anchor_of(ncells, 0);
     if (mixed) {
         int alevel = 0;
-        const double anchor_edge = getenv("PYGBE_ANCHOR_EDGE") ? atof(getenv("PYGBE_ANCHOR_EDGE")) : 16.0;   // tuning
+        const double anchor_edge = tune_env("PYGBE_ANCHOR_EDGE") ? atof(tune_env("PYGBE_ANCHOR_EDGE")) : 16.0;   // tuning
         while (edge / (double)(1 << alevel) > anchor_edge && alevel < PYGBE_MAXLEVEL) alevel++;
         std::vector<int> panel_anchor(R.np, 0);
         for (int c : leaves) {
@@ -106,8 +106,10 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     // break-even between one Taylor evaluation and the direct sum over a leaf's points: a regrouped M2P
     // evaluation costs Nc - 1 + NW FMA-pipe instructions per region, a P2P pair ~14 per region, and the sweep of
     // profiles/r2a_regrouped_path.md puts the optimum at ~16 points for P = 6 (344 instructions) in both precisions
-    const int small_leaf = (int)(16.0 * (h->Nc + 2.0 * h->NW) / 344.0 / K);
-    const int exact_mac = getenv("PYGBE_BOUND_MAC") ? 0 : 1;     // tuning: 1 = group MAC on the group's own points
+    // (the Laplace form costs Nc - 1 FMAs)
+    int small_leaf = (int)(16.0 * (R.lap ? (double)h->Nc : h->Nc + 2.0 * h->NW) / 344.0 / K);
+    if (const char *e = tune_env("PYGBE_SMALL_LEAF")) small_leaf = atoi(e);                     // tuning
+    const int exact_mac = h->group_mac == 0 ? 1 : 0;             // 1 = group MAC on the group's own points
     LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.tpos, R.np, exact_mac, R.ggeo, R.cgeo, R.crange, R.cchild,
            h->theta, thres_guard, d_clmax, small_leaf, 0, d_mcnt, d_pcnt, nullptr, nullptr, nullptr, nullptr, d_over);
     std::vector<int> mcnt, pcnt;
@@ -142,6 +144,9 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
                 }
         R.n_m2m = (int)m2m_rec.size();
         R.n_p2m = (int)p2m_cells.size();
+        R.p2m_panels = 0; R.m2m_children = 0;
+        for (int c : p2m_cells) R.p2m_panels += crange_h[c].y - crange_h[c].x;
+        for (const int4 &m : m2m_rec) R.m2m_children += m.z;
         TRY(upload(h, &R.p2m_cells, p2m_cells)); TRY(upload(h, &R.m2m_rec, m2m_rec));
         std::vector<int4> p2m_rec;
         for (int c : p2m_cells) p2m_rec.push_back(make_int4(c, crange_h[c].x, crange_h[c].y, 0));
@@ -194,8 +199,9 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     // M2P CTAs keep only 8-20 warps per SM resident (72-127 registers): finer items even out the tail (config 1:
     // 4 cells per item 0.057 ms, 8 cells 0.060, 16 cells 0.068)
     int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[R.ng] / (6 * want_items)));
+    if (R.lap) m2p_item = std::max(m2p_item, 12);            // k_m2p_lap stages 12 cells at a time
     m2p_item = (m2p_item + 3) / 4 * 4;
-    if (const char *e = getenv("PYGBE_M2P_ITEM")) m2p_item = std::max(1, atoi(e));                 // tuning
+    if (const char *e = tune_env("PYGBE_M2P_ITEM")) m2p_item = std::max(1, atoi(e));                 // tuning
     // P2P tiles gather up to P2P_TILE source points from several panel ranges of one anchor cell: a group's near
     // field is ~30 short runs of Morton-consecutive panels (one or two leaves each), and tiles cut range by range
     // were 62 % full with a third of them under a quarter (config 1).  tile = (first segment, last segment + 1,
@@ -244,7 +250,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     {
         const long slots = 148L * 12;
         int per_item = (int)std::min(8L, std::max(1L, (long)sub.size() / (slots * 24)));
-        if (const char *e = getenv("PYGBE_P2P_ITEM_TILES")) per_item = std::max(1, atoi(e));      // tuning
+        if (const char *e = tune_env("PYGBE_P2P_ITEM_TILES")) per_item = std::max(1, atoi(e));      // tuning
         for (int g = 0; g < R.ng; g++)
             for (int t = gtile[g]; t < gtile[g + 1]; t += per_item) {
                 const int n = std::min(per_item, gtile[g + 1] - t);
@@ -253,7 +259,7 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
                 pitems.push_back(make_int4(g, t, t + n, acc));
             }
     }
-    if (getenv("PYGBE_DEBUG")) {
+    if (tune_env("PYGBE_DEBUG")) {
         long pts = 0, selft = 0; int hist[9] = {0};
         for (auto &t : sub) { pts += t.w >> 1; selft += t.w & 1; hist[std::min(8, (t.w >> 1) * 8 / P2P_TILE)]++; }
         fprintf(stderr, "[pygbe] region: groups %d ranges %zu items %zu tiles %zu fill %.3f self tiles %ld; tile fill hist:",

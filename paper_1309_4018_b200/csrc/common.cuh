@@ -10,6 +10,8 @@
 #include <vector>
 #include <algorithm>
 #include <chrono>
+#include <utility>
+#include <cstdlib>
 #include "../../include/pygbe.h"
 
 #define PYGBE_PMAX 12
@@ -47,42 +49,108 @@ void pygbe_set_error(const char *fmt, ...);
 static inline int nc_of(int P) { return (P + 1) * (P + 2) * (P + 3) / 6; }
 static inline int cdiv(long a, long b) { return (int)((a + b - 1) / b); }
 
+// Tuning knobs are environment variables only in builds with -DPYGBE_TUNING (experiments); the
+// product build compiles the defaults in and reads no environment.
+#ifdef PYGBE_TUNING
+static inline const char *tune_env(const char *name) { return getenv(name); }
+#else
+static inline const char *tune_env(const char *) { return nullptr; }
+#endif
+
 // ---------------------------------------------------------------------------------------------------
-// Device memory owned by a handle: blocks from the device's stream-ordered pool (cudaMallocAsync on the
-// handle's stream), freed together.  The pool keeps freed memory (release threshold raised at create), so
-// neither the scratch buffers of create nor a second handle pay cudaMalloc / cudaFree and their device-wide
-// synchronisation (create of config 1: 21 ms -> see profiles/r2a_regrouped_path.md).  Buffers are also read on the
-// handle's side streams, always after an event recorded on the main stream, and destroy synchronises every
-// stream before freeing.
+// Device memory owned by a handle.  Two sources (include/pygbe.h "Memory"):
+//   workspace  one block supplied by the caller (pygbe_options.workspace, e.g. a torch uint8 tensor), carved
+//              up by a host-side first-fit allocator with coalescing free list (a few hundred blocks per
+//              handle; every alloc / free is a host call, the device never sees the bookkeeping);
+//   pool       no workspace given: blocks from a library-owned stream-ordered pool (cudaMallocFromPoolAsync),
+//              never the device's default pool, released in pygbe_destroy.
+// In both modes the same allocator runs on offsets, so high_water is the workspace size that the sequence of
+// allocations made so far needs: pygbe_workspace_size is a dry run in pool mode that reads it.  Blocks are
+// 256-byte aligned.  Freed blocks are reused at once: everything that touches them is ordered on the handle's
+// stream (side streams join it through events before any free).
 struct DeviceArena {
-    std::vector<void *> blocks;
-    size_t bytes = 0;
+    struct Block { size_t off, size; void *ptr; };
+    std::vector<Block> used;                    // live blocks
+    std::vector<std::pair<size_t, size_t>> holes;   // free (offset, size) below top, sorted by offset
+    size_t top = 0;                             // end of the highest live block
+    size_t bytes = 0;                           // live bytes (rounded to the alignment)
+    size_t high_water = 0;                      // max of top so far
+    char *base = nullptr;                       // workspace mode: caller's block
+    size_t capacity = 0;
+    cudaMemPool_t pool = nullptr;               // pool mode
     cudaStream_t stream = nullptr;
+    static size_t round_up(size_t n) { return (n + 255) & ~(size_t)255; }
+    size_t place(size_t n)                      // first fit; returns the offset
+    {
+        for (size_t i = 0; i < holes.size(); i++)
+            if (holes[i].second >= n) {
+                const size_t off = holes[i].first;
+                if (holes[i].second == n) holes.erase(holes.begin() + i);
+                else { holes[i].first += n; holes[i].second -= n; }
+                return off;
+            }
+        const size_t off = top;
+        top += n;
+        high_water = std::max(high_water, top);
+        return off;
+    }
+    void unplace(size_t off, size_t n)
+    {
+        size_t i = 0;
+        while (i < holes.size() && holes[i].first < off) i++;
+        holes.insert(holes.begin() + i, std::make_pair(off, n));
+        if (i + 1 < holes.size() && holes[i].first + holes[i].second == holes[i + 1].first) {
+            holes[i].second += holes[i + 1].second; holes.erase(holes.begin() + i + 1);
+        }
+        if (i > 0 && holes[i - 1].first + holes[i - 1].second == holes[i].first) {
+            holes[i - 1].second += holes[i].second; holes.erase(holes.begin() + i);
+        }
+        if (!holes.empty() && holes.back().first + holes.back().second == top) { top = holes.back().first; holes.pop_back(); }
+    }
     template <class T> int alloc(T **p, size_t n)
     {
         *p = nullptr;
         if (n == 0) n = 1;
+        const size_t sz = round_up(n * sizeof(T));
+        const size_t off = place(sz);
         void *q = nullptr;
-        cudaError_t e = cudaMallocAsync(&q, n * sizeof(T), stream);
-        if (e != cudaSuccess) {
-            pygbe_set_error("cudaMallocAsync of %zu bytes failed: %s", n * sizeof(T), cudaGetErrorString(e));
-            return PYGBE_ENOMEM;
+        if (base) {
+            if (off + sz > capacity) {
+                unplace(off, sz);
+                pygbe_set_error("workspace too small: %zu bytes given, at least %zu needed (pygbe_workspace_size)", capacity, off + sz);
+                return PYGBE_ENOMEM;
+            }
+            q = base + off;
+        } else {
+            cudaError_t e = pool ? cudaMallocFromPoolAsync(&q, sz, pool, stream) : cudaMallocAsync(&q, sz, stream);
+            if (e != cudaSuccess) {
+                unplace(off, sz);
+                pygbe_set_error("device allocation of %zu bytes failed: %s", sz, cudaGetErrorString(e));
+                return PYGBE_ENOMEM;
+            }
         }
-        blocks.push_back(q);
-        bytes += n * sizeof(T);
+        used.push_back({off, sz, q});
+        bytes += sz;
         *p = (T *)q;
         return PYGBE_OK;
     }
     void release_one(void *q)
     {
-        for (size_t i = 0; i < blocks.size(); i++)
-            if (blocks[i] == q) { cudaFreeAsync(q, stream); blocks.erase(blocks.begin() + i); return; }
+        if (!q) return;
+        for (size_t i = 0; i < used.size(); i++)
+            if (used[i].ptr == q) {
+                if (!base) cudaFreeAsync(q, stream);
+                bytes -= used[i].size;
+                unplace(used[i].off, used[i].size);
+                used.erase(used.begin() + i);
+                return;
+            }
     }
     void release()
     {
-        for (void *q : blocks) cudaFreeAsync(q, stream);
-        blocks.clear();
-        bytes = 0;
+        if (!base) for (const Block &b : used) cudaFreeAsync(b.ptr, stream);
+        used.clear(); holes.clear();
+        top = 0; bytes = 0;
     }
 };
 
@@ -148,6 +216,8 @@ struct Region {
     long p2p_pairs = 0, m2p_evals = 0;
     // multipoles ------------------------------------------------------------------------------------
     double *mom = nullptr;          // [ncells][2][Nc]: MV, MK (farfield.cuh), shared by twin regions
+    bool lap = false;               // tree owner, kappa = 0, no twin: wc holds the Nc coefficients C'_f of k_m2p_lap instead
+    long p2m_panels = 0, m2m_children = 0;   // panels streamed by one P2M launch, child cells read by one M2M launch
     void *wc = nullptr;             // tree owner: [ncells][m2p_stride(P, twin)] regrouped multipoles W_{m,e} of this region and,
                                     // interleaved, of its twin, in float or double (m2p.cuh; written by P2M / M2M)
     // singular / near-singular corrections (CSR over targets) ----------------------------------------
@@ -192,12 +262,16 @@ struct pygbe_handle {
     struct IndexTables *itab = nullptr;   // device copy of the multi-index tables
     int NW = 0;                           // W_{m,e} per moment set (m2p_nw(P)) and the table that forms them (tables.cuh)
     int *wt_off = nullptr; short *wt_k = nullptr; double *wt_c = nullptr;
+    int *lt_off = nullptr; short *lt_k = nullptr, *lt_deg = nullptr; double *lt_c = nullptr;   // Laplace form (build_lap_table), Nc entries
     cudaStream_t side = nullptr;    // far-field chain (P2M, M2M, M2P) runs here, concurrently with P2P
     cudaStream_t side2 = nullptr;   // near-field correction SpMV runs here
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_join2 = nullptr;
     bool overlap = true;
     // optional block-diagonal right preconditioner of GMRES (pygbe_options.precond)
     int precond = 0;
+    bool dry = false;               // size query (pygbe_workspace_size): allocate as create does, compute no values
+    int group_mac = 0;              // pygbe_options.group_mac
+    double *dq = nullptr;           // [nq] charges in the caller's order (energy)
     double4 *pinv = nullptr;        // per global panel: inverse of [[1/2, -V_in], [1/2, c V_out]] as (a, b, c, d)
     int2 *pidx = nullptr;           // per global panel: positions of (phi, dphi) = (row_in, row_out) in x / y
     double *zbuf = nullptr;         // [2 npan] scratch
@@ -212,6 +286,9 @@ struct pygbe_handle {
     bool profile = false;
     std::vector<cudaEvent_t> ev_pool;
     std::vector<int> ev_stage;          // stage started at event i (-1 = end marker)
+    std::vector<int> ev_region;         // tree owner the launch after event i works on (-1: none)
+    struct LaunchAcc { int stage, region; double ms; int launches; };
+    std::vector<LaunchAcc> launch_acc;  // per (stage, region) accumulators of pygbe_launch_times
     size_t ev_used = 0;
     double stage_ms[PYGBE_N_STAGES] = {0};
     long stage_launches[PYGBE_N_STAGES] = {0};

@@ -19,15 +19,20 @@
 // with A's when there is one), in the arithmetic type of the M2P, row stride padded to a multiple of 4.
 // Written by the kernel that finishes the cell (P2M for leaves, M2M otherwise) from the sparse table
 // (wt_off, wt_k, wt_c) built at create (tables.cuh): entry p of the stream is sum_i wt_c[i] M^(wt_k[i]).
+// Laplace regions without a twin take the single polynomial of k_m2p_lap instead (m2p.cuh): same mechanism with
+// the table of build_lap_table, each entry divided by the cell edge to the power wt_deg[p].
 struct MomOut {
     void *wc;
     double caA, cbA, caB, cbB;
     int fp32, stride, twin, NW;
     const int *wt_off; const short *wt_k; const double *wt_c;
+    const short *wt_deg;            // Laplace form: degree of entry p; nullptr otherwise
+    const double4 *cgeo;            // cell geometry (edge length in .w)
 };
 // mv, mk: the cell's two moment sets in shared memory; all nthreads threads of the CTA call this
 __device__ __forceinline__ void wc_store(const MomOut &o, long cell, const double *mv, const double *mk, int tid, int nthreads)
 {
+    const double inv_edge = o.wt_deg ? 1.0 / o.cgeo[cell].w : 1.0;
     for (int p = tid; p < o.NW; p += nthreads) {
         double wv = 0.0, wk = 0.0;
         for (int i = o.wt_off[p]; i < o.wt_off[p + 1]; i++) {
@@ -35,7 +40,12 @@ __device__ __forceinline__ void wc_store(const MomOut &o, long cell, const doubl
             const double c = o.wt_c[i];
             wv += c * mv[k]; wk += c * mk[k];
         }
-        const double a = o.caA * wv + o.cbA * wk, b = o.caB * wv + o.cbB * wk;
+        double a = o.caA * wv + o.cbA * wk, b = o.caB * wv + o.cbB * wk;
+        if (o.wt_deg) {                                            // C'_f = C_f / edge^|f|
+            double s = 1.0;
+            for (int d = o.wt_deg[p]; d > 0; d--) s *= inv_edge;
+            a *= s; b *= s;
+        }
         const long at = cell * o.stride + (o.twin ? 2 * p : p);
         if (o.fp32) { ((float *)o.wc)[at] = (float)a; if (o.twin) ((float *)o.wc)[at + 1] = (float)b; }
         else { ((double *)o.wc)[at] = a; if (o.twin) ((double *)o.wc)[at + 1] = b; }
@@ -90,16 +100,17 @@ k_panel_moments(int P, int Nc, int K, const IndexTables *__restrict__ tab, const
 static inline int p2m_nsplit(int Nc) { return Nc >= 192 ? 1 : (Nc >= 96 ? 2 : (256 / Nc > 8 ? 8 : 256 / Nc)); }
 static inline int p2m_threads(int Nc) { return (p2m_nsplit(Nc) * Nc + 31) / 32 * 32; }
 __global__ void __launch_bounds__(P2M_MAXT)
-k_p2m(const int *__restrict__ skip, int Nc, int nsplit, const int4 *__restrict__ rec, const double2 *__restrict__ pq,
+k_p2m(const int *__restrict__ skip, int Nc, int nsplit, int n_leaves, const int4 *__restrict__ rec, const double2 *__restrict__ pq,
       const double *__restrict__ pmom, double *__restrict__ mom, MomOut mo)
 {
     __shared__ double s_part[2][P2M_MAXT];
     if (skip && *skip) return;
-    const int4 rc = rec[blockIdx.x];                               // (cell, first panel, end panel, -)
-    const int cell = rc.x;
     const int t = threadIdx.x;
     const int sp = t / Nc, k = t - sp * Nc;
     const bool active = sp < nsplit;
+    for (int leaf = blockIdx.x; leaf < n_leaves; leaf += gridDim.x) {
+    const int4 rc = rec[leaf];                                     // (cell, first panel, end panel, -)
+    const int cell = rc.x;
     double aV = 0.0, aK = 0.0;
     if (active) {
 #pragma unroll 4
@@ -120,6 +131,8 @@ k_p2m(const int *__restrict__ skip, int Nc, int nsplit, const int4 *__restrict__
     if (active && sp == 0) { s_part[0][k] = aV; s_part[1][k] = aK; }
     __syncthreads();
     wc_store(mo, cell, s_part[0], s_part[1], t, blockDim.x);
+    __syncthreads();                                               // s_part is rewritten by the next leaf
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ M2M

@@ -2,7 +2,11 @@
 // evaluation of the treecode per iteration"; tolerances Tables 1, 3 (:197-203, :223-227); reading A16.
 // Arnoldi with classical Gram-Schmidt applied twice (CGS2: two batched dot passes instead of j
 // sequential ones), Givens rotations and the convergence test run in kernels; every kernel returns
-// immediately once flags[0] ("done") is set, so the host can queue iterations ahead and only polls.
+// immediately once flags[0] ("stop") is set, so the host can queue iterations ahead and only polls.
+// flags: [0] stop -- the Arnoldi estimate |g_(j+1)| / |b| reached tol, or the recomputed residual did; [1] columns
+// built in the current cycle; [2] iterations (matvecs inside Arnoldi steps) so far; [3] converged -- set only by
+// k_gm_begin, i.e. only when the residual b - A x recomputed with a matvec is within tol (the estimate alone
+// does not see the rounding of the operator: fp32 kernels, treecode, atomics).
 #pragma once
 #include "common.cuh"
 #include "tables.cuh"
@@ -12,56 +16,6 @@
 #define GM_THREADS 256
 #define GM_ROWS_PER_CTA 2048
 #define GM_MAXVEC 256              // Gram-Schmidt coefficients staged in shared memory per pass of k_gm_arnoldi
-
-// out[i] += V_i . w for i < nvec (out pre-zeroed); V row-major [nvec][n].
-__global__ void __launch_bounds__(GM_THREADS)
-k_gm_dots(const int *__restrict__ flags, const double *__restrict__ V, long n, int nvec,
-          const double *__restrict__ w, double *__restrict__ out)
-{
-    if (flags[0]) return;
-    typedef cub::BlockReduce<double, GM_THREADS> Red;
-    __shared__ typename Red::TempStorage tmp;
-    long lo = (long)blockIdx.x * GM_ROWS_PER_CTA, hi = min(n, lo + GM_ROWS_PER_CTA);
-    double wr[GM_ROWS_PER_CTA / GM_THREADS];
-#pragma unroll
-    for (int k = 0; k < GM_ROWS_PER_CTA / GM_THREADS; k++) {
-        long r = lo + threadIdx.x + (long)k * GM_THREADS;
-        wr[k] = r < hi ? w[r] : 0.0;
-    }
-    for (int i = 0; i < nvec; i++) {
-        const double *v = V + (long)i * n;
-        double acc = 0.0;
-#pragma unroll
-        for (int k = 0; k < GM_ROWS_PER_CTA / GM_THREADS; k++) {
-            long r = lo + threadIdx.x + (long)k * GM_THREADS;
-            if (r < hi) acc += v[r] * wr[k];
-        }
-        double s = Red(tmp).Sum(acc);
-        if (threadIdx.x == 0) atomicAdd(out + i, s);
-        __syncthreads();
-    }
-}
-
-// w -= sum_i h[i] V_i
-__global__ void __launch_bounds__(GM_THREADS)
-k_gm_axpys(const int *__restrict__ flags, const double *__restrict__ V, long n, int nvec,
-           const double *__restrict__ h, double *__restrict__ w)
-{
-    if (flags[0]) return;
-    long r = (long)blockIdx.x * GM_THREADS + threadIdx.x;
-    if (r >= n) return;
-    double acc = w[r];
-    for (int i = 0; i < nvec; i++) acc -= h[i] * V[(long)i * n + r];
-    w[r] = acc;
-}
-
-__global__ void k_gm_zero(const int *__restrict__ flags, double *a, int na, double *b, int nb, double *c, int nc)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < na) a[i] = 0.0;
-    if (i < nb) b[i] = 0.0;
-    if (i < nc) c[i] = 0.0;
-}
 
 // Start of a cycle: r = b - w (w = A x, or 0 on the first cycle); beta^2 accumulated in scal[3].
 __global__ void __launch_bounds__(GM_THREADS)
@@ -89,7 +43,8 @@ __global__ void k_gm_begin(int *flags, double *scal, double *g, int m, int first
     scal[2] = bn > 0.0 ? beta / bn : 0.0;
     for (int i = 0; i <= m; i++) g[i] = 0.0;
     g[0] = beta;
-    if (bn == 0.0 || beta / bn <= tol) { flags[0] = 1; flags[1] = 0; }
+    flags[1] = 0;
+    if (bn == 0.0 || beta / bn <= tol) { flags[0] = 1; flags[3] = 1; }
     scal[3] = 0.0;
 }
 
@@ -105,34 +60,6 @@ k_gm_scale(const int *__restrict__ flags, long n, const double *__restrict__ src
     dst[i] = s > 0.0 ? src[i] / s : 0.0;
 }
 
-// Column j of the Hessenberg matrix: H[0..j][j] = h1 + h2, H[j+1][j] = sqrt(nrm2); apply the previous
-// rotations, form the new one, update g; rel = |g[j+1]| / bnorm; raise done when rel <= tol.
-__global__ void k_gm_givens(int *flags, int j, int m, const double *__restrict__ h1, const double *__restrict__ h2,
-                            const double *__restrict__ nrm2, double *H, double *cs, double *sn, double *g,
-                            double *scal, double tol)
-{
-    if (flags[0]) return;
-    double *col = H + (long)j * (m + 1);
-    for (int i = 0; i <= j; i++) col[i] = h1[i] + h2[i];
-    col[j + 1] = sqrt(*nrm2);
-    for (int i = 0; i < j; i++) {
-        double t = cs[i] * col[i] + sn[i] * col[i + 1];
-        col[i + 1] = -sn[i] * col[i] + cs[i] * col[i + 1];
-        col[i] = t;
-    }
-    double d = hypot(col[j], col[j + 1]);
-    double c = d > 0.0 ? col[j] / d : 1.0, s = d > 0.0 ? col[j + 1] / d : 0.0;
-    cs[j] = c; sn[j] = s;
-    col[j] = d; col[j + 1] = 0.0;
-    g[j + 1] = -s * g[j];
-    g[j] = c * g[j];
-    double rel = fabs(g[j + 1]) / scal[0];
-    scal[2] = rel;
-    flags[1] = j + 1;
-    flags[2] += 1;                       // total iterations
-    if (rel <= tol) flags[0] = 1;
-}
-
 // Back substitution R y = g for the k = flags[1] columns built in this cycle (single thread, k <= m).
 __global__ void k_gm_solve_small(const int *__restrict__ flags, int m, const double *__restrict__ H,
                                  const double *__restrict__ g, double *__restrict__ yk)
@@ -141,7 +68,8 @@ __global__ void k_gm_solve_small(const int *__restrict__ flags, int m, const dou
     for (int i = k - 1; i >= 0; i--) {
         double s = g[i];
         for (int c = i + 1; c < k; c++) s -= H[(long)c * (m + 1) + i] * yk[c];
-        yk[i] = s / H[(long)i * (m + 1) + i];
+        const double piv = H[(long)i * (m + 1) + i];
+        yk[i] = piv != 0.0 ? s / piv : 0.0;              // zero pivot: breakdown on a singular operator, leave the direction out
     }
 }
 
@@ -199,8 +127,7 @@ k_precond_apply(const int *__restrict__ flags, int respect_done, long npan, cons
 //   2  w -= sum_i h1[i] V_i on the slice, then h2[i] += V_i . w            (second Gram-Schmidt pass, CGS2)
 //   3  w -= sum_i h2[i] V_i, nrm2 += |w|^2
 //   4  V_(j+1) = w / sqrt(nrm2) on the slice; one thread: Hessenberg column, Givens, convergence test
-// Same arithmetic as k_gm_dots / k_gm_axpys / k_gm_scale / k_gm_givens; only the summation order of the
-// partials differs (atomics either way, reading A19).
+// The summation order of the partial dot products is not fixed (atomics, reading A19).
 #include <cooperative_groups.h>
 __global__ void __launch_bounds__(GM_THREADS)
 k_gm_arnoldi(int *flags, double *V, long n, int j, int m, double *w, double *h1, double *h2, double *nrm2, double *H,

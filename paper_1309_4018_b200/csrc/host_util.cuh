@@ -11,7 +11,7 @@ static inline double now_ms()
 // PYGBE_DEBUG=1: host milliseconds since the previous checkpoint (create-time diagnostics on stderr)
 static inline void dbg_t(const char *what)
 {
-    static const bool on = getenv("PYGBE_DEBUG") != nullptr;
+    static const bool on = tune_env("PYGBE_DEBUG") != nullptr;
     static double last = 0.0;
     if (!on) return;
     const double t = now_ms();

@@ -44,6 +44,8 @@ struct M2PArgs {
     const void *wc;            // W_{m,e} of the tree owner (and twin), already combined and in T (farfield.cuh)
     double kappaA, kappaB; double *outA, *outB;
     int twin; int fp32; cudaStream_t stream;
+    int lap;                   // Laplace form (k_m2p_lap): wc holds the C'_f; ggeo = target group centres
+    const double4 *ggeo;
 };
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
@@ -587,4 +589,209 @@ k_m2p_dbl2(const int *__restrict__ skip, const int4 *__restrict__ items, const i
     }
     if (ok0) { atomicAdd(outA + t0, aA0); if (TWIN) atomicAdd(outB + t0, aB0); }
     if (ok1) { atomicAdd(outA + t1, aA1); if (TWIN) atomicAdd(outB + t1, aB1); }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Laplace regions without a twin (kappa = 0: the protein interior and the Stern layer of the multi-surface
+// problems): the same truncated series in a form that needs no monomials and no radial
+// recurrence.  For G = 1/r every radial derivative is a pure power, F^(m)(s) = (-1)^m (2m-1)!! / r^(2m+1), so
+// with the inverted offset u = d / r^2 (|u| = 1/r, d^e = u^e r^(2|e|), r^(-2J) = (ux^2 + uy^2 + uz^2)^J)
+//     sum_{|k| <= P} a^k M^k  =  (1/r) sum_{|f| <= P} C_f u^f,
+//     C_f = sum_{2i <= f, e = f - 2i, J = |i|}  (J! / i!)  sum_{|j| = J} (-1)^J (2(|e| + J) - 1)!! / (e! 2^J j!)  M^(e + 2j):
+// ONE trivariate polynomial of degree P with Nc coefficients per cell (the detraced multipoles; degree-n
+// coefficients come from degree-n moments only), evaluated by nested Horner steps in uz, uy, ux: Nc - 1 FMAs per
+// (target, cell) -- 164 at P = 8 against 164 multiplies + 295 FMAs of the regrouped form above.  The C_f are formed
+// where the W are (P2M / M2M epilogue, farfield.cuh; table built at create, tables.cuh), stored in Horner order
+// (ex, ey, ez descending) and normalised by the cell edge a, C'_f = C_f / a^|f| with u' = a d / r^2 (|u'| = a / r
+// < theta), so that every intermediate is O(monopole) whatever the units.
+//
+// Four targets per thread: each coefficient read from shared memory feeds four FMAs (fp32: two packed FFMA2),
+// because a broadcast LDS.128 costs two wavefronts for four coefficients and one coefficient per FMA pair would
+// tie the shared-memory pipe with the FMA pipe.  A CTA of one warp serves one 64-target group: thread
+// (sub, l16) = (tid / 16, tid % 16) owns targets l16 + 16 k, k = 0..3, and the cells sub, sub + 2, ... of every
+// staged batch (two cells in flight per warp, warp-level synchronisation only); the partial sums per target
+// meet in shared memory at the end of the item.  Offsets are
+// formed from group-relative coordinates: x - G in T per target, c - G computed in fp64 and rounded once per
+// staged cell, so that the fp32 path subtracts numbers of the size of r, not of the molecule (relative error of
+// d about 1e-7; no fp64 arithmetic or conversions in the loop over cells except the accumulation).
+static inline __host__ __device__ constexpr int m2p_lap_stride(int P) { return ((P + 1) * (P + 2) * (P + 3) / 6 + 3) / 4 * 4; }
+
+template <typename T> struct LapVec;
+template <> struct LapVec<float> {
+    f2_t lo, hi;                                                     // targets (0, 1) and (2, 3)
+    static __device__ __forceinline__ LapVec make(float a, float b, float c, float d) { LapVec v; v.lo = f2_pack(a, b); v.hi = f2_pack(c, d); return v; }
+    static __device__ __forceinline__ LapVec set(float w) { LapVec v; v.lo = f2_pack(w, w); v.hi = v.lo; return v; }
+    static __device__ __forceinline__ LapVec fmaw(const LapVec &a, const LapVec &u, float w)      // a u + w
+    { const f2_t w2 = f2_pack(w, w); LapVec v; v.lo = f2_fma(a.lo, u.lo, w2); v.hi = f2_fma(a.hi, u.hi, w2); return v; }
+    static __device__ __forceinline__ LapVec fmav(const LapVec &a, const LapVec &u, const LapVec &c)   // a u + c
+    { LapVec v; v.lo = f2_fma(a.lo, u.lo, c.lo); v.hi = f2_fma(a.hi, u.hi, c.hi); return v; }
+    static __device__ __forceinline__ LapVec mul(const LapVec &a, const LapVec &b) { LapVec v; v.lo = f2_mul(a.lo, b.lo); v.hi = f2_mul(a.hi, b.hi); return v; }
+    static __device__ __forceinline__ LapVec sub(const LapVec &a, float c) { const f2_t c2 = f2_pack(c, c); LapVec v; v.lo = f2_sub(a.lo, c2); v.hi = f2_sub(a.hi, c2); return v; }
+    __device__ __forceinline__ void get(float (&o)[4]) const { f2_unpack(lo, o[0], o[1]); f2_unpack(hi, o[2], o[3]); }
+};
+template <> struct LapVec<double> {
+    double v[4];
+    static __device__ __forceinline__ LapVec make(double a, double b, double c, double d) { LapVec r; r.v[0] = a; r.v[1] = b; r.v[2] = c; r.v[3] = d; return r; }
+    static __device__ __forceinline__ LapVec set(double w) { return make(w, w, w, w); }
+    static __device__ __forceinline__ LapVec fmaw(const LapVec &a, const LapVec &u, double w)
+    { LapVec r;
+#pragma unroll
+      for (int i = 0; i < 4; i++) r.v[i] = fma(a.v[i], u.v[i], w);
+      return r; }
+    static __device__ __forceinline__ LapVec fmav(const LapVec &a, const LapVec &u, const LapVec &c)
+    { LapVec r;
+#pragma unroll
+      for (int i = 0; i < 4; i++) r.v[i] = fma(a.v[i], u.v[i], c.v[i]);
+      return r; }
+    static __device__ __forceinline__ LapVec mul(const LapVec &a, const LapVec &b)
+    { LapVec r;
+#pragma unroll
+      for (int i = 0; i < 4; i++) r.v[i] = a.v[i] * b.v[i];
+      return r; }
+    static __device__ __forceinline__ LapVec sub(const LapVec &a, double c)
+    { LapVec r;
+#pragma unroll
+      for (int i = 0; i < 4; i++) r.v[i] = a.v[i] - c;
+      return r; }
+    __device__ __forceinline__ void get(double (&o)[4]) const
+    {
+#pragma unroll
+        for (int i = 0; i < 4; i++) o[i] = v[i];
+    }
+};
+
+// sum_f C'_f u^f by nested Horner steps; w: the cell's coefficients in Horner order (ex, ey, ez descending)
+template <int P, typename T>
+__device__ __forceinline__ LapVec<T> lap_poly(const LapVec<T> &ux, const LapVec<T> &uy, const LapVec<T> &uz, const T *__restrict__ w)
+{
+    typedef LapVec<T> V;
+    constexpr int EPC = Chunk<T>::N;
+    T cur[EPC];
+    int idx = 0;
+    V ax = V::set(T(0));
+#pragma unroll
+    for (int ex = P; ex >= 0; ex--) {
+        V ay = V::set(T(0));
+#pragma unroll
+        for (int ey = P - ex; ey >= 0; ey--) {
+            V az = V::set(T(0));
+#pragma unroll
+            for (int ez = P - ex - ey; ez >= 0; ez--) {
+                if (idx % EPC == 0) Chunk<T>::get(w + idx, cur);
+                const T c = cur[idx % EPC];
+                idx++;
+                if (ez == P - ex - ey) az = V::set(c); else az = V::fmaw(az, uz, c);
+            }
+            if (ey == P - ex) ay = az; else ay = V::fmav(ay, uy, az);
+        }
+        if (ex == P) ax = ay; else ax = V::fmav(ax, ux, ay);
+    }
+    return ax;
+}
+
+#ifndef M2PL_THREADS
+#define M2PL_THREADS 32                                              // one warp: two cells in flight, no CTA barrier
+#endif
+#define M2PL_NSUB (M2PL_THREADS / 16)
+// cells per staged batch: a multiple of the subs, at most 12, two buffers within M2PL_SMEM bytes of static shared memory
+#ifndef M2PL_SMEM
+#define M2PL_SMEM 12288
+#endif
+template <int P, typename T> struct LapBatch {
+    static constexpr int ROW = m2p_lap_stride(P) * (int)sizeof(T);
+    static constexpr int FIT = M2PL_SMEM / ROW / 4 * 4;
+    static constexpr int CB = FIT < 4 ? 4 : (FIT > 12 ? 12 : FIT);
+};
+#ifdef M2PL_MINB
+#define M2PL_BOUNDS __launch_bounds__(M2PL_THREADS, M2PL_MINB)
+#else
+#define M2PL_BOUNDS __launch_bounds__(M2PL_THREADS)
+#endif
+__device__ __forceinline__ void lap_sync()
+{
+#if M2PL_THREADS == 32
+    __syncwarp();
+#else
+    __syncthreads();
+#endif
+}
+template <int P, typename T>
+__global__ void M2PL_BOUNDS
+k_m2p_lap(const int *__restrict__ skip, const int4 *__restrict__ items, const int *__restrict__ m2p_cell, int np,
+          const double4 *__restrict__ tpos, const double4 *__restrict__ ggeo, const double4 *__restrict__ cgeo,
+          const T *__restrict__ wc, double *__restrict__ out)
+{
+    typedef LapVec<T> V;
+    typedef typename Real<T>::vec4 V4;
+    constexpr int STRIDE = m2p_lap_stride(P);
+    constexpr int EPC = 16 / (int)sizeof(T);
+    constexpr int CH = STRIDE / EPC;                                 // 16-byte chunks per cell
+    constexpr int M2PL_CB = LapBatch<P, T>::CB;
+    __shared__ __align__(16) T s_W[2][M2PL_CB][STRIDE];
+    __shared__ __align__(16) V4 s_c[2][M2PL_CB];                     // (c - G, edge)
+    __shared__ double s_red[M2PL_NSUB][PYGBE_TG_M2P];
+    if (skip && *skip) return;
+    const int4 it = items[blockIdx.x];
+    const int sub = threadIdx.x >> 4, l16 = threadIdx.x & 15;
+    const double4 G = ggeo[2 * it.x];
+    T xt[4], yt[4], zt[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        const int t = it.x * PYGBE_TG_M2P + l16 + 16 * k;
+        const double4 X = t < np ? tpos[t] : make_double4(1e30, 1e30, 1e30, 0);
+        xt[k] = (T)(X.x - G.x); yt[k] = (T)(X.y - G.y); zt[k] = (T)(X.z - G.z);
+    }
+    const V X4 = V::make(xt[0], xt[1], xt[2], xt[3]), Y4 = V::make(yt[0], yt[1], yt[2], yt[3]), Z4 = V::make(zt[0], zt[1], zt[2], zt[3]);
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    double4 pc = make_double4(0, 0, 0, 1);                           // centre of this thread's cell of the batch after the staged one
+    auto prefetch = [&](int s0) { if (threadIdx.x < M2PL_CB && s0 + (int)threadIdx.x < it.z) pc = cgeo[m2p_cell[s0 + threadIdx.x]]; };
+    auto stage = [&](int buf, int s0) {
+        const int nb = min(M2PL_CB, it.z - s0);
+        for (int i = threadIdx.x; i < nb * CH; i += M2PL_THREADS) {
+            const int c_ = i / CH, j = i - c_ * CH;
+            cp_async16(&s_W[buf][c_][j * EPC], wc + (long)m2p_cell[s0 + c_] * STRIDE + j * EPC);
+        }
+        if ((int)threadIdx.x < nb) {
+            V4 v; v.x = (T)(pc.x - G.x); v.y = (T)(pc.y - G.y); v.z = (T)(pc.z - G.z); v.w = (T)pc.w;
+            s_c[buf][threadIdx.x] = v;
+        }
+        cp_async_commit();
+    };
+    prefetch(it.y);
+    stage(0, it.y);
+    prefetch(it.y + M2PL_CB);
+    int buf = 0;
+    for (int s0 = it.y; s0 < it.z; s0 += M2PL_CB, buf ^= 1) {
+        const int nb = min(M2PL_CB, it.z - s0);
+        const bool more = s0 + M2PL_CB < it.z;
+        if (more) { stage(buf ^ 1, s0 + M2PL_CB); prefetch(s0 + 2 * M2PL_CB); cp_async_wait<1>(); } else { cp_async_wait<0>(); }
+        lap_sync();
+#pragma unroll 1                                             // one copy of the straight-line body (instruction cache)
+        for (int c_ = sub; c_ < nb; c_ += M2PL_NSUB) {
+            const V4 c = s_c[buf][c_];
+            const V dx = V::sub(X4, c.x), dy = V::sub(Y4, c.y), dz = V::sub(Z4, c.z);
+            const V r2 = V::fmav(dz, dz, V::fmav(dy, dy, V::mul(dx, dx)));
+            T r2s[4], ri[4], sc[4];
+            r2.get(r2s);
+#pragma unroll
+            for (int k = 0; k < 4; k++) { ri[k] = Real<T>::rsqrt_(r2s[k]); sc[k] = c.w * (ri[k] * ri[k]); }
+            const V S = V::make(sc[0], sc[1], sc[2], sc[3]);
+            const V p = lap_poly<P, T>(V::mul(dx, S), V::mul(dy, S), V::mul(dz, S), s_W[buf][c_]);
+            T pv[4];
+            p.get(pv);
+#pragma unroll
+            for (int k = 0; k < 4; k++) acc[k] += (double)(pv[k] * ri[k]);
+        }
+        lap_sync();                                          // buf is refilled two iterations from now
+    }
+#pragma unroll
+    for (int k = 0; k < 4; k++) s_red[sub][l16 + 16 * k] = acc[k];
+    lap_sync();
+    for (int i = threadIdx.x; i < PYGBE_TG_M2P; i += M2PL_THREADS) {
+        const int t = it.x * PYGBE_TG_M2P + i;
+        double v = 0.0;
+#pragma unroll
+        for (int q = 0; q < M2PL_NSUB; q++) v += s_red[q][i];
+        if (t < np) atomicAdd(out + t, v);
+    }
 }

@@ -18,7 +18,13 @@ template <bool TWIN, typename T> static void launch(const M2PArgs &a)
 
 int CAT(pygbe_m2p_launch_, M2P_P)(const M2PArgs &a)
 {
-    if (a.fp32 && a.twin) {               // two targets per thread, packed fp32
+    if (a.lap && a.fp32) {                // kappa = 0, no twin: one polynomial in d / r^2 by Horner steps, four targets per thread
+        k_m2p_lap<M2P_P, float><<<a.n_items, M2PL_THREADS, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.ggeo, a.cgeo,
+                                                                          (const float *)a.wc, a.outA);
+    } else if (a.lap) {
+        k_m2p_lap<M2P_P, double><<<a.n_items, M2PL_THREADS, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.ggeo, a.cgeo,
+                                                                           (const double *)a.wc, a.outA);
+    } else if (a.fp32 && a.twin) {        // two targets per thread, packed fp32
         k_m2p_twin2<M2P_P><<<a.n_items, M2P2_THREADS, 0, a.stream>>>(a.skip, a.items, a.m2p_cell, a.np, a.tpos, a.cgeo, (const float *)a.wc,
                                                                   a.kappaA, Real<float>::kscale(a.kappaA), a.kappaB,
                                                                   Real<float>::kscale(a.kappaB), a.outA, a.outB);

@@ -9,7 +9,7 @@
 #include "m2p.cuh"
 
 // Stage timers: an event is recorded where a stage starts; the time to the next event belongs to it.
-static void stage_mark(pygbe_handle *h, int stage)
+static void stage_mark(pygbe_handle *h, int stage, int region)
 {
     if (!h->profile) return;
     if (h->ev_used == h->ev_pool.size()) {
@@ -17,18 +17,56 @@ static void stage_mark(pygbe_handle *h, int stage)
         if (cudaEventCreate(&e) != cudaSuccess) return;
         h->ev_pool.push_back(e);
         h->ev_stage.push_back(-1);
+        h->ev_region.push_back(-1);
     }
     h->ev_stage[h->ev_used] = stage;
+    h->ev_region[h->ev_used] = region;
     cudaEventRecord(h->ev_pool[h->ev_used], h->stream);
     h->ev_used++;
 }
-#define STAGE(h, st) do { stage_mark(h, st); if ((h)->profile) (h)->stage_launches[st] -= (h)->launches; } while (0)
+// one mark per kernel launch: (stage, region of the tree owner)
+#define STAGE(h, st, reg) do { stage_mark(h, st, reg); if ((h)->profile) (h)->stage_launches[st] -= (h)->launches; } while (0)
 #define STAGE_END(h, st) do { if ((h)->profile) (h)->stage_launches[st] += (h)->launches; } while (0)
+
+// Folds the recorded events into the per-stage and per-(stage, region) accumulators.  Stream must be idle.
+static void stage_collect(pygbe_handle *h)
+{
+    for (size_t i = 0; i + 1 < h->ev_used; i++) {
+        const int st = h->ev_stage[i], reg = h->ev_region[i];
+        if (st < 0 || st >= PYGBE_N_STAGES) continue;
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, h->ev_pool[i], h->ev_pool[i + 1]) != cudaSuccess) continue;
+        h->stage_ms[st] += t;
+        bool found = false;
+        for (auto &a : h->launch_acc)
+            if (a.stage == st && a.region == reg) { a.ms += t; a.launches++; found = true; break; }
+        if (!found) h->launch_acc.push_back({st, reg, (double)t, 1});
+    }
+    h->ev_used = 0;
+}
 
 #define M2P_DECL(PP) int pygbe_m2p_launch_##PP(const M2PArgs &);
 M2P_DECL(1) M2P_DECL(2) M2P_DECL(3) M2P_DECL(4) M2P_DECL(5) M2P_DECL(6)
 M2P_DECL(7) M2P_DECL(8) M2P_DECL(9) M2P_DECL(10) M2P_DECL(11) M2P_DECL(12)
 #undef M2P_DECL
+
+// elements per row of wc for the tree owner A (m2p.cuh)
+static inline int m2p_row_elems(int P, const Region &A) { return A.lap ? m2p_lap_stride(P) : m2p_stride(P, A.twin >= 0); }
+
+static const char *m2p_kernel_name(const pygbe_handle *h, const Region &A, const Region *B)
+{
+    const bool f32 = h->precision == PYGBE_PRECISION_MIXED;
+    if (A.lap) return f32 ? "k_m2p_lap<P,float>" : "k_m2p_lap<P,double>";
+    if (f32) return B ? "k_m2p_twin2<P>" : "k_m2p_single2<P>";
+    if (h->P <= 7) return B ? "k_m2p_dbl2<P,twin>" : "k_m2p_dbl2<P,single>";
+    return B ? "k_m2p<P,twin,double>" : "k_m2p<P,single,double>";
+}
+static const char *p2p_kernel_name(const pygbe_handle *h, const Region &A, const Region *B)
+{
+    if (h->precision != PYGBE_PRECISION_MIXED) return B ? "k_p2p<double,twin>" : "k_p2p<double>";
+    if (!A.quad) return B ? "k_p2p<float,twin>" : "k_p2p<float>";
+    return B ? "k_p2p_quad<twin>" : "k_p2p_quad2";
+}
 
 // M2P of the tree owner A and its twin B (if any) in one pass, on stream st; A.wc was written by P2M / M2M.
 static int launch_m2p(pygbe_handle *h, Region &A, Region *B, const int *skip, cudaStream_t st)
@@ -39,6 +77,7 @@ static int launch_m2p(pygbe_handle *h, Region &A, Region *B, const int *skip, cu
     a.tpos = A.tpos; a.cgeo = A.cgeo; a.wc = A.wc; a.kappaA = A.kappa; a.outA = A.out;
     a.twin = B ? 1 : 0; a.kappaB = B ? B->kappa : 0.0; a.outB = B ? B->out : nullptr;
     a.fp32 = h->precision == PYGBE_PRECISION_MIXED; a.stream = st;
+    a.lap = A.lap ? 1 : 0; a.ggeo = A.ggeo;
     typedef int (*fn_t)(const M2PArgs &);
     static const fn_t table[PYGBE_PMAX + 1] = {nullptr, pygbe_m2p_launch_1, pygbe_m2p_launch_2, pygbe_m2p_launch_3,
         pygbe_m2p_launch_4, pygbe_m2p_launch_5, pygbe_m2p_launch_6, pygbe_m2p_launch_7, pygbe_m2p_launch_8,
@@ -58,7 +97,7 @@ static void launch_p2p(pygbe_handle *h, Region &A, Region *B, const int *skip)
     const double kA = A.kappa, kB = B ? B->kappa : 0.0, rV = B ? A.twin_rV : 1.0;
     double *oA = A.out, *oB = B ? B->out : nullptr;
     const bool quad = sizeof(T) == 4 && A.quad;
-    static const int two = getenv("PYGBE_P2P_TWO") ? atoi(getenv("PYGBE_P2P_TWO")) : 1;    // tuning: 0 never, 1 single regions, 2 always
+    static const int two = tune_env("PYGBE_P2P_TWO") ? atoi(tune_env("PYGBE_P2P_TWO")) : 1;    // tuning: 0 never, 1 single regions, 2 always
     const bool quad2 = quad && (two == 2 || (two == 1 && !B));
 #define P2P_GO(YA, TW, YB)                                                                                     \
     do { if (quad2) { auto kern = k_p2p_quad2<YA, TW, YB>;                                                     \
@@ -96,14 +135,14 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
     const bool fork = h->overlap && !h->profile && h->side != nullptr && h->side2 != nullptr;
     cudaStream_t main_st = h->stream;
 
-    STAGE(h, PYGBE_STAGE_PREP);
     for (auto &w : work) {
         Region &A = *w.first; Region *B = w.second;
+        STAGE(h, PYGBE_STAGE_PREP, A.id);
         LAUNCH(h, k_prep, cdiv((long)A.np * h->K, 256), 256, 0, skip, A.np, h->K, x, A.phi_idx, A.dphi_idx, A.cV, A.cK, A.pnrm,
                A.spos, mixed ? (double4 *)nullptr : A.schg, mixed ? A.schgf : (float4 *)nullptr, A.quad ? 1 : 0, A.pphi, A.pdphi,
                A.pq, A.out, B ? B->out : (double *)nullptr);
+        STAGE_END(h, PYGBE_STAGE_PREP);
     }
-    STAGE_END(h, PYGBE_STAGE_PREP);
     if (fork) {
         cudaEventRecord(h->ev_fork, main_st);
         cudaStreamWaitEvent(h->side, h->ev_fork, 0);
@@ -112,13 +151,13 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
 
     // singular / near-singular corrections: need the gathered densities only
     h->stream = fork ? h->side2 : main_st;                 // LAUNCH issues on h->stream
-    STAGE(h, PYGBE_STAGE_NEAR);
     for (auto &w : work) {
         Region &A = *w.first; Region *B = w.second;
+        STAGE(h, PYGBE_STAGE_NEAR, A.id);
         LAUNCH(h, k_near, cdiv((long)A.np * NEAR_LANES, 128), 128, 0, skip, A.np, A.corr_off, A.corr_col, A.corr_val,
                B ? B->corr_val : (const double2 *)nullptr, A.pphi, A.pdphi, A.corr, B ? B->corr : (double *)nullptr);
+        STAGE_END(h, PYGBE_STAGE_NEAR);
     }
-    STAGE_END(h, PYGBE_STAGE_NEAR);
     if (fork) cudaEventRecord(h->ev_join2, h->side2);
 
     // far field: upward passes of all trees, then their M2P
@@ -130,16 +169,20 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
             // multipoles leave P2M / M2M regrouped and combined for the M2P of A (MV - MK) and of its twin (rV MV + MK)
             MomOut mo;
             mo.wc = A.wc; mo.caA = 1.0; mo.cbA = -1.0; mo.caB = A.twin_rV; mo.cbB = 1.0;
-            mo.fp32 = mixed ? 1 : 0; mo.twin = B ? 1 : 0; mo.stride = m2p_stride(h->P, B != nullptr); mo.NW = h->NW;
-            mo.wt_off = h->wt_off; mo.wt_k = h->wt_k; mo.wt_c = h->wt_c;
-            STAGE(h, PYGBE_STAGE_P2M);
-            if (A.n_p2m > 0)
-                LAUNCH(h, k_p2m, A.n_p2m, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.p2m_rec, A.pq, A.pmom, A.mom, mo);
+            mo.fp32 = mixed ? 1 : 0; mo.twin = B ? 1 : 0; mo.stride = m2p_row_elems(h->P, A); mo.cgeo = A.cgeo;
+            if (A.lap) { mo.NW = h->Nc; mo.wt_off = h->lt_off; mo.wt_k = h->lt_k; mo.wt_c = h->lt_c; mo.wt_deg = h->lt_deg; }
+            else { mo.NW = h->NW; mo.wt_off = h->wt_off; mo.wt_k = h->wt_k; mo.wt_c = h->wt_c; mo.wt_deg = nullptr; }
+            STAGE(h, PYGBE_STAGE_P2M, A.id);
+            if (A.n_p2m > 0) {
+                int p2m_grid = A.n_p2m;
+                if (const char *e = tune_env("PYGBE_P2M_GRID")) p2m_grid = std::min(A.n_p2m, std::max(1, atoi(e)));   // tuning
+                LAUNCH(h, k_p2m, p2m_grid, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.n_p2m, A.p2m_rec, A.pq, A.pmom, A.mom, mo);
+            }
             STAGE_END(h, PYGBE_STAGE_P2M);
-            STAGE(h, PYGBE_STAGE_M2M);
+            STAGE(h, PYGBE_STAGE_M2M, A.id);
             if (A.n_m2m > 0) {
                 M2MLaunch ml;
-                ml.skip = skip; ml.P = h->P; ml.Nc = h->Nc; ml.n_cells = A.n_m2m; ml.grid = std::min(A.n_m2m, 3 * h->n_sm);
+                ml.skip = skip; ml.P = h->P; ml.Nc = h->Nc; ml.n_cells = A.n_m2m; ml.grid = std::min(A.n_m2m, (tune_env("PYGBE_M2M_GRID") ? atoi(tune_env("PYGBE_M2M_GRID")) : 3) * h->n_sm);   // tuning
                 ml.rec = A.m2m_rec; ml.tab = h->itab; ml.cgeo = A.cgeo; ml.mom = A.mom; ml.mo = mo; ml.sync = A.up_sync;
                 ml.ready = A.cready; ml.epoch = (int)(h->n_matvec + 1); ml.stream = h->stream;
                 m2m_launch(ml);
@@ -147,34 +190,34 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
             }
             STAGE_END(h, PYGBE_STAGE_M2M);
         }
-        STAGE(h, PYGBE_STAGE_M2P);
         for (auto &w : work) {
             Region &A = *w.first; Region *B = w.second;
             if (A.n_m2p_items == 0) continue;
+            STAGE(h, PYGBE_STAGE_M2P, A.id);
             int rc = launch_m2p(h, A, B, skip, h->stream);
             if (rc != PYGBE_OK) { h->stream = main_st; return rc; }
+            STAGE_END(h, PYGBE_STAGE_M2P);
         }
-        STAGE_END(h, PYGBE_STAGE_M2P);
     }
     if (fork) cudaEventRecord(h->ev_join, h->side);
 
     h->stream = main_st;
-    STAGE(h, PYGBE_STAGE_P2P);
     for (auto &w : work) {
         Region &A = *w.first; Region *B = w.second;
         if (A.n_p2p_items == 0) continue;
+        STAGE(h, PYGBE_STAGE_P2P, A.id);
         if (mixed) launch_p2p<float>(h, A, B, skip); else launch_p2p<double>(h, A, B, skip);
+        STAGE_END(h, PYGBE_STAGE_P2P);
     }
-    STAGE_END(h, PYGBE_STAGE_P2P);
     if (fork) { cudaStreamWaitEvent(main_st, h->ev_join, 0); cudaStreamWaitEvent(main_st, h->ev_join2, 0); }
-    STAGE(h, PYGBE_STAGE_COMBINE);
     for (auto &w : work) {
         Region &A = *w.first; Region *B = w.second;
+        STAGE(h, PYGBE_STAGE_COMBINE, A.id);
         LAUNCH(h, k_combine, cdiv(A.np, 256), 256, 0, skip, A.np, A.pphi, A.out, B ? B->out : (const double *)nullptr, A.corr,
                B ? B->corr : (const double *)nullptr, A.row_idx, B ? B->row_idx : (const int *)nullptr, y);
+        STAGE_END(h, PYGBE_STAGE_COMBINE);
     }
-    STAGE_END(h, PYGBE_STAGE_COMBINE);
-    stage_mark(h, -1);
+    stage_mark(h, -1, -1);
     h->kernels_per_matvec = h->launches - before;
     h->n_matvec++;
     return PYGBE_OK;

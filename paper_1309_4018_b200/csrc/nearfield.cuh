@@ -271,7 +271,8 @@ k_rhs(int np, const double4 *__restrict__ tpos, const int *__restrict__ row_idx,
 // ------------------------------------------------------------------------------- reaction potential
 // phi_reac(r_k) = sum_{S in dOmega} sigma_S [ c_S V dphi_S - K phi_S ](r_k)  with the plain K-point rule
 // (eq. 4; discretised :119).  The point charges schg come from k_prep with the solution.
-// grid = (source chunks, charges); block reduce, one atomicAdd per CTA.
+// grid = (charges, source chunks): the charges are on grid.x, which has no practical limit (a region may hold
+// more than the 65535 that grid.y allows); block reduce, one atomicAdd per CTA.
 #define EN_THREADS 256
 #define EN_CHUNK 4096
 template <bool YUKAWA>
@@ -282,9 +283,9 @@ k_reaction(int npts, const double4 *__restrict__ spos, const double4 *__restrict
 {
     typedef cub::BlockReduce<double, EN_THREADS> Red;
     __shared__ typename Red::TempStorage tmp;
-    int k = blockIdx.y;
+    int k = blockIdx.x;
     double4 X = qpos[k];
-    long lo = (long)blockIdx.x * EN_CHUNK, hi = min((long)npts, lo + EN_CHUNK);
+    long lo = (long)blockIdx.y * EN_CHUNK, hi = min((long)npts, lo + EN_CHUNK);
     double acc = 0.0;
     for (long i = lo + threadIdx.x; i < hi; i += EN_THREADS) {
         double4 a = spos[i], c = schg[i];

@@ -21,7 +21,7 @@ void pygbe_set_error(const char *fmt, ...)
 }
 
 extern "C" const char *pygbe_last_error(void) { return g_err; }
-extern "C" const char *pygbe_version(void) { return "pygbe-b200 0.2 sm_100a"; }
+extern "C" const char *pygbe_version(void) { return "pygbe-b200 0.3 sm_100a"; }
 
 // Pinned host blocks (128 B: GMRES flags and scalars read back each poll) are kept for the life of the
 // process and handed from handle to handle: cudaMallocHost costs 2-3 ms, a third of create at config 1.
@@ -96,6 +96,7 @@ extern "C" int pygbe_profile(pygbe_handle *h, int enable)
     if (!h) { pygbe_set_error("profile: null handle"); return PYGBE_EINVAL; }
     h->profile = enable != 0;
     h->ev_used = 0;
+    h->launch_acc.clear();
     for (int i = 0; i < PYGBE_N_STAGES; i++) { h->stage_ms[i] = 0; h->stage_launches[i] = 0; }
     return PYGBE_OK;
 }
@@ -105,14 +106,67 @@ extern "C" int pygbe_stage_times(pygbe_handle *h, double *ms, int64_t *launches)
     if (!h || !ms) { pygbe_set_error("stage_times: null pointer"); return PYGBE_EINVAL; }
     CUDA_TRY(cudaSetDevice(h->device));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
-    for (size_t i = 0; i + 1 < h->ev_used; i++) {
-        int st = h->ev_stage[i];
-        if (st < 0 || st >= PYGBE_N_STAGES) continue;
-        float t = 0.f;
-        if (cudaEventElapsedTime(&t, h->ev_pool[i], h->ev_pool[i + 1]) == cudaSuccess) h->stage_ms[st] += t;
-    }
-    h->ev_used = 0;
+    stage_collect(h);
     for (int i = 0; i < PYGBE_N_STAGES; i++) { ms[i] = h->stage_ms[i]; if (launches) launches[i] = h->stage_launches[i]; }
+    return PYGBE_OK;
+}
+
+// What one launch of (stage, tree owner A) does: kernel name, work units, algorithmic bytes.
+static void describe_launch(const pygbe_handle *h, int stage, const Region &A, pygbe_launch_info *o)
+{
+    const Region *B = A.twin >= 0 ? &h->regions[A.twin] : nullptr;
+    const bool mixed = h->precision == PYGBE_PRECISION_MIXED;
+    const int64_t np = A.np, npts = A.npts, Nc = h->Nc, nreg = B ? 2 : 1;
+    const int64_t wrow = (int64_t)m2p_row_elems(h->P, A) * (mixed ? 4 : 8);
+    o->twin_region = B ? B->id : -1;
+    const char *name = "";
+    switch (stage) {
+    case PYGBE_STAGE_PREP:
+        name = "k_prep"; o->units = npts;
+        // per panel: x (2 x 8) through two indices (2 x 4), cV, cK, normal + area; writes phi, dphi, (cV dphi, cK phi), zeroed out
+        // per point: weight (8 of the 32-byte record), writes the charge record (16 B fp32 / 32 B fp64)
+        o->bytes = np * (16 + 8 + 16 + 32 + 8 + 8 + 16 + 8 * nreg) + npts * (8 + (mixed ? 16 : 32));
+        break;
+    case PYGBE_STAGE_P2M: {
+        name = "k_p2m"; o->units = A.p2m_panels;
+        // per panel of a needed leaf: its two moment sets (pmom) and its two weights; per leaf: mom and the wc row written
+        o->bytes = A.p2m_panels * (2 * Nc * 8 + 16) + (int64_t)A.n_p2m * (2 * Nc * 8 + wrow);
+        break; }
+    case PYGBE_STAGE_M2M:
+        name = "k_m2m"; o->units = A.n_m2m;
+        o->bytes = A.m2m_children * (2 * Nc * 8) + (int64_t)A.n_m2m * (2 * Nc * 8 + wrow + 32);
+        break;
+    case PYGBE_STAGE_M2P: name = m2p_kernel_name(h, A, B); o->units = A.m2p_evals; o->bytes = 0; break;
+    case PYGBE_STAGE_P2P: name = p2p_kernel_name(h, A, B); o->units = A.p2p_pairs; o->bytes = 0; break;
+    case PYGBE_STAGE_NEAR:
+        name = "k_near"; o->units = np;
+        o->bytes = A.corr_nnz * (4 + 16 * nreg) + np * (4 + 16 + 8 * nreg);
+        break;
+    case PYGBE_STAGE_COMBINE:
+        name = "k_combine"; o->units = np;
+        o->bytes = np * (8 + nreg * (8 + 8 + 4 + 8));
+        break;
+    default: break;
+    }
+    snprintf(o->kernel, sizeof(o->kernel), "%s", name);
+}
+
+extern "C" int pygbe_launch_times(pygbe_handle *h, pygbe_launch_info *out, int32_t max_out, int32_t *n_out)
+{
+    if (!h || !out || !n_out || max_out < 0) { pygbe_set_error("launch_times: null pointer"); return PYGBE_EINVAL; }
+    CUDA_TRY(cudaSetDevice(h->device));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    stage_collect(h);
+    int n = 0;
+    for (const auto &a : h->launch_acc) {
+        if (n >= max_out) break;
+        if (a.region < 0 || a.region >= h->nreg) continue;
+        pygbe_launch_info *o = out + n++;
+        memset(o, 0, sizeof(*o));
+        o->stage = a.stage; o->region = a.region; o->launches = a.launches; o->ms = a.ms;
+        describe_launch(h, a.stage, h->regions[a.region], o);
+    }
+    *n_out = n;
     return PYGBE_OK;
 }
 
@@ -131,6 +185,7 @@ extern "C" int pygbe_stats(const pygbe_handle *h, pygbe_stats_t *s)
         s->near_nnz += R.corr_nnz;
     }
     s->device_bytes = (int64_t)h->mem.bytes;
+    s->workspace_high_water = (int64_t)h->mem.high_water;
     s->n_matvec = h->n_matvec; s->kernels_per_matvec = h->kernels_per_matvec; s->kernel_launches = h->launches;
     s->create_ms = h->create_ms; s->last_solve_ms = h->last_solve_ms; s->last_iters = h->last_iters;
     s->P = h->P; s->K = h->K; s->precision = h->precision; s->theta = h->theta;

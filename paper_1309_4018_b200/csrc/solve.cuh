@@ -9,6 +9,15 @@ static int ensure_host_staging(pygbe_handle *h)
     return PYGBE_OK;
 }
 
+static int ensure_energy_scratch(pygbe_handle *h)
+{
+    if (!h->dq && h->nq > 0) {
+        TRY(h->mem.alloc(&h->dq, h->nq));
+        CUDA_TRY(cudaMemcpyAsync(h->dq, h->qq.data(), h->nq * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    }
+    return PYGBE_OK;
+}
+
 
 // ---------------------------------------------------------------------------------------------- rhs
 extern "C" int pygbe_rhs(pygbe_handle *h, double *b_dev)
@@ -73,30 +82,45 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
     {
         int occ = 1;
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_gm_arnoldi, GM_THREADS, 0));
-        const long arn_rows = getenv("PYGBE_ARN_ROWS") ? std::max(32L, atol(getenv("PYGBE_ARN_ROWS"))) : 256L;   // tuning
+        const long arn_rows = tune_env("PYGBE_ARN_ROWS") ? std::max(32L, atol(tune_env("PYGBE_ARN_ROWS"))) : 256L;   // tuning
         arn_grid = (int)std::max(1L, std::min((long)occ * h->n_sm, (long)cdiv(n, arn_rows)));
     }
     CUDA_TRY(cudaMemsetAsync(G.h1, 0, (size_t)(G.m + 2) * sizeof(double), st));   // k_gm_arnoldi keeps h1 zero between steps
     const bool pc = h->precond == 1 && h->pinv != nullptr;
-    int total = 0, done = 0;
+    // Cycle = [residual b - A x by a matvec, convergence test on it] + up to m Arnoldi steps + update of x.  A cycle
+    // ends early when the Arnoldi estimate reaches tol; convergence is declared only by the next cycle's recomputed
+    // residual (one extra matvec per solve).  If that residual is above tol the iteration simply goes on; after
+    // three such disagreements tol is below what the operator's arithmetic attains and the solve returns ENOCONV
+    // with the true residual (PRECISION_MIXED: about 1e-6 relative).
+    int total = 0, converged = 0, disagreements = 0;
     bool first = true;
-    while (total < max_iter && !done) {
-        const int mc = std::min(m, max_iter - total);
-        if (!first) TRY(matvec_impl(h, x_dev, G.w, G.flags));
+    while (!converged) {
+        if (!first) {
+            CUDA_TRY(cudaMemsetAsync(G.flags, 0, sizeof(int), st));             // clear "stop", keep the counters
+            CUDA_TRY(cudaMemsetAsync(G.scal + 3, 0, sizeof(double), st));
+            TRY(matvec_impl(h, x_dev, G.w, nullptr));
+        }
         LAUNCH(h, k_gm_residual, gridn, GM_THREADS, 0, G.flags, n, G.b, G.w, first ? 0 : 1, G.V, G.scal);
         LAUNCH(h, k_gm_begin, 1, 1, 0, G.flags, G.scal, G.g, G.m, first ? 1 : 0, tol);
         LAUNCH(h, k_gm_scale, gridn, GM_THREADS, 0, G.flags, n, G.V, G.scal + 1, 0, G.V);
+        const int mc = std::min(m, max_iter - total);
+        if (!first || mc <= 0) {                          // the verdict of k_gm_begin on the recomputed residual, before queueing a cycle
+            CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaMemcpyAsync(h->pinned_scal, G.scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            if (h->pinned_flags[3]) { converged = 1; break; }
+            if (mc <= 0) break;                           // out of iterations
+        }
         first = false;
-        int j = 0;
-        for (; j < mc; j++) {
-            double *vj = G.V + (size_t)j * n, *vn = G.V + (size_t)(j + 1) * n;
+        for (int j = 0; j < mc; j++) {
+            double *vj = G.V + (size_t)j * n;
             if (pc) {           // right preconditioning: w = A (M^-1 v_j)
                 LAUNCH(h, k_precond_apply, cdiv(h->npan, GM_THREADS), GM_THREADS, 0, G.flags, 1, h->npan, h->pinv, h->pidx, vj, 0, h->zbuf);
                 TRY(matvec_impl(h, h->zbuf, G.w, G.flags));
             } else {
                 TRY(matvec_impl(h, vj, G.w, G.flags));
             }
-            {   // one cooperative launch: CGS2, normalisation, Givens, convergence test (gmres.cuh)
+            {   // one cooperative launch: CGS2, normalisation, Givens, convergence estimate (gmres.cuh)
                 long nn = n; int jj = j, mm = G.m; double tl = tol;
                 double *nrm2 = G.scal + 3;
                 void *args[] = {&G.flags, &G.V, &nn, &jj, &mm, &G.w, &G.h1, &G.h2, &nrm2, &G.H, &G.cs, &G.sn, &G.g, &G.scal, &tl};
@@ -106,7 +130,7 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
             if ((j + 1) % poll == 0 || j + 1 == mc) {
                 CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
                 CUDA_TRY(cudaStreamSynchronize(st));
-                if (h->pinned_flags[0]) { done = 1; break; }
+                if (h->pinned_flags[0]) break;
             }
         }
         LAUNCH(h, k_gm_solve_small, 1, 1, 0, G.flags, G.m, G.H, G.g, G.yk);
@@ -120,11 +144,19 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
         CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(cudaMemcpyAsync(h->pinned_scal, G.scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
         CUDA_TRY(cudaStreamSynchronize(st));
-        done = h->pinned_flags[0];
         total = h->pinned_flags[2];
-        if (!done) {
-            // new cycle: rotations and g restart; flags[1] is rewritten by the next givens
+        if (h->pinned_flags[3]) { converged = 1; break; }                       // b = 0, or the recomputed residual was within tol
+        if (h->pinned_flags[0] && ++disagreements > 3) {                        // the estimate keeps saying "done", the residual does not
+            CUDA_TRY(cudaMemsetAsync(G.flags, 0, sizeof(int), st));
             CUDA_TRY(cudaMemsetAsync(G.scal + 3, 0, sizeof(double), st));
+            TRY(matvec_impl(h, x_dev, G.w, nullptr));
+            LAUNCH(h, k_gm_residual, gridn, GM_THREADS, 0, G.flags, n, G.b, G.w, 1, G.V, G.scal);
+            LAUNCH(h, k_gm_begin, 1, 1, 0, G.flags, G.scal, G.g, G.m, 0, tol);
+            CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaMemcpyAsync(h->pinned_scal, G.scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            converged = h->pinned_flags[3];
+            break;
         }
     }
     CUDA_TRY(cudaGetLastError());
@@ -132,7 +164,11 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
     h->last_solve_ms = now_ms() - t0;
     if (iters) *iters = total;
     if (rel_resid) *rel_resid = h->pinned_scal[2];
-    if (!done) { pygbe_set_error("GMRES: %d iterations, relative residual %.3e > tol %.3e", total, h->pinned_scal[2], tol); return PYGBE_ENOCONV; }
+    if (!converged) {
+        pygbe_set_error("GMRES: %d iterations, relative residual %.3e > tol %.3e%s", total, h->pinned_scal[2], tol,
+                        disagreements > 3 ? " (the Arnoldi estimate is below tol but the recomputed residual b - A x is not: tol is below what this precision attains)" : "");
+        return PYGBE_ENOCONV;
+    }
     return PYGBE_OK;
 }
 
@@ -147,7 +183,10 @@ extern "C" int pygbe_reaction_potential(pygbe_handle *h, const double *x_dev, do
         if (R.nq == 0) continue;
         LAUNCH(h, k_prep, cdiv((long)R.np * h->K, 256), 256, 0, nullptr, R.np, h->K, x_dev, R.phi_idx, R.dphi_idx, R.cV, R.cK, R.pnrm,
                R.spos, R.schg, (float4 *)nullptr, 0, R.pphi, R.pdphi, R.pq, R.out, (double *)nullptr);
-        dim3 grid(cdiv(R.npts, EN_CHUNK), R.nq);
+        // chunks of Gauss points on grid.y: at most 65535 of them
+        const long en_chunks = cdiv(R.npts, EN_CHUNK);
+        if (en_chunks > 65535) { pygbe_set_error("reaction potential: region %d has too many Gauss points (%d)", R.id, R.npts); return PYGBE_EINVAL; }
+        dim3 grid(R.nq, (unsigned)en_chunks);
         if (R.yukawa) LAUNCH(h, k_reaction<true>, grid, EN_THREADS, 0, R.npts, R.spos, R.schg, R.nq, R.qpos, R.qid, R.kappa, phi_dev);
         else LAUNCH(h, k_reaction<false>, grid, EN_THREADS, 0, R.npts, R.spos, R.schg, R.nq, R.qpos, R.qid, R.kappa, phi_dev);
     }
@@ -171,13 +210,10 @@ extern "C" int pygbe_energy(pygbe_handle *h, const double *x_dev, double *E_solv
     if (h->nq == 0) return PYGBE_OK;
     if (E_solv) {
         TRY(pygbe_reaction_potential(h, x_dev, h->phi_reac));
-        double *d_q;
-        TRY(h->mem.alloc(&d_q, h->nq));
-        CUDA_TRY(cudaMemcpyAsync(d_q, h->qq.data(), h->nq * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-        LAUNCH(h, k_dot_q, 1, 256, 0, (int)h->nq, d_q, h->phi_reac, h->scratch);
+        TRY(ensure_energy_scratch(h));
+        LAUNCH(h, k_dot_q, 1, 256, 0, (int)h->nq, h->dq, h->phi_reac, h->scratch);
         CUDA_TRY(cudaMemcpyAsync(h->pinned_scal, h->scratch, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
         CUDA_TRY(cudaStreamSynchronize(h->stream));
-        h->mem.release_one(d_q);
         *E_solv = 0.5 * C0 * h->pinned_scal[0];
     }
     if (E_coul) {

@@ -142,6 +142,7 @@ struct WTable {
     std::vector<int> off;
     std::vector<short> k;
     std::vector<double> c;
+    std::vector<short> deg;          // Laplace form only: |f| of entry p (the power of the cell edge it is divided by)
 };
 static void build_w_table(int P, const IndexTables &t, WTable *w)
 {
@@ -163,5 +164,43 @@ static void build_w_table(int P, const IndexTables &t, WTable *w)
                         }
                     w->off.push_back((int)w->k.size());
                 }
+            }
+}
+
+// The Laplace form of the series (m2p.cuh, k_m2p_lap): entry p of the stream -- ex, ey, ez DESCENDING with
+// |f| <= P, the order the nested Horner scheme consumes them -- is the coefficient of u^f, u = d / r^2,
+//     C_f = sum_{2i <= f, e = f - 2i, J = |i|} (J! / i!) sum_{|j| = J} (-1)^J (2(|e| + J) - 1)!! / (e! 2^J j!) M^(e + 2j),
+// again a sparse row over the canonical moment index (1293 non-zeros at P = 8).  (-1)!! = 1.
+static void build_lap_table(int P, const IndexTables &t, WTable *w)
+{
+    double fact[PYGBE_PMAX + 1], dfact[2 * PYGBE_PMAX + 2];
+    fact[0] = 1.0;
+    for (int i = 1; i <= PYGBE_PMAX; i++) fact[i] = fact[i - 1] * i;
+    for (int n = 0; n <= PYGBE_PMAX; n++) {                          // dfact[n] = (2n - 1)!!
+        dfact[n] = 1.0;
+        for (int q = 2 * n - 1; q > 1; q -= 2) dfact[n] *= q;
+    }
+    w->off.assign(1, 0); w->k.clear(); w->c.clear(); w->deg.clear();
+    std::vector<double> row(PYGBE_NCMAX);
+    for (int fx = P; fx >= 0; fx--)
+        for (int fy = P - fx; fy >= 0; fy--)
+            for (int fz = P - fx - fy; fz >= 0; fz--) {
+                std::fill(row.begin(), row.end(), 0.0);
+                for (int ix = 0; ix <= fx / 2; ix++)
+                    for (int iy = 0; iy <= fy / 2; iy++)
+                        for (int iz = 0; iz <= fz / 2; iz++) {
+                            const int J = ix + iy + iz, ex = fx - 2 * ix, ey = fy - 2 * iy, ez = fz - 2 * iz, ne = ex + ey + ez;
+                            const double pre = ((J & 1) ? -1.0 : 1.0) * dfact[ne + J] * fact[J] /
+                                               (fact[ex] * fact[ey] * fact[ez] * std::ldexp(1.0, J) * fact[ix] * fact[iy] * fact[iz]);
+                            for (int jx = J; jx >= 0; jx--)
+                                for (int jy = J - jx; jy >= 0; jy--) {
+                                    const int jz = J - jx - jy;
+                                    row[t.idx3[ex + 2 * jx][ey + 2 * jy][ez + 2 * jz]] += pre / (fact[jx] * fact[jy] * fact[jz]);
+                                }
+                        }
+                for (int k = 0; k < PYGBE_NCMAX; k++)
+                    if (row[k] != 0.0) { w->k.push_back((short)k); w->c.push_back(row[k]); }
+                w->off.push_back((int)w->k.size());
+                w->deg.push_back((short)(fx + fy + fz));
             }
 }

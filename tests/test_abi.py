@@ -83,3 +83,65 @@ def test_no_cpu_fallback():
         import workloads as W
         with pytest.raises(RuntimeError):
             pg.Handle.from_problem(W.born_problem(1))
+
+
+def _create_args(surfs, n_regions, eps=None, kappa=None):
+    import numpy as np
+    import workloads as W
+    keep = []
+    arr = (pg.pygbe_surface * len(surfs))()
+    for i, (level, radius, rin, rout) in enumerate(surfs):
+        v, t = W.icosphere(level, radius)
+        v = np.ascontiguousarray(v, dtype=np.float64); t = np.ascontiguousarray(t, dtype=np.int32)
+        keep += [v, t]
+        arr[i] = pg.pygbe_surface(v.ctypes.data_as(C.POINTER(C.c_double)), v.shape[0],
+                                  t.ctypes.data_as(C.POINTER(C.c_int32)), t.shape[0], rin, rout)
+    eps = np.array(eps if eps is not None else [4.0] + [80.0] * (n_regions - 1), dtype=np.float64)
+    kappa = np.array(kappa if kappa is not None else [0.0] * n_regions, dtype=np.float64)
+    keep += [eps, kappa]
+    dp = C.POINTER(C.c_double)
+    return keep, (arr, len(surfs), None, eps.ctypes.data_as(dp), kappa.ctypes.data_as(dp), n_regions, 4, 6, 0.5)
+
+
+def test_region_graph_must_be_a_tree(built_lib):
+    """SURVEY 8(b) EINVAL list: 'region graph not a tree'.  Checked on the host before any CUDA call."""
+    h = C.c_void_p(1)
+    # three nested spheres whose region ids close a cycle: 0-1, 1-2, 2-0
+    keep, args = _create_args([(1, 2.0, 0, 1), (1, 4.0, 1, 2), (1, 6.0, 2, 0)], 3)
+    assert built_lib.pygbe_create(*args, None, C.byref(h)) == pg.PYGBE_EINVAL and h.value is None
+    assert b"not a tree" in built_lib.pygbe_last_error()
+    # two components that no surface joins: 0-1 and 2-3
+    keep, args = _create_args([(1, 2.0, 0, 1), (1, 4.0, 2, 3)], 4)
+    assert built_lib.pygbe_create(*args, None, C.byref(h)) == pg.PYGBE_EINVAL
+    assert b"not a tree" in built_lib.pygbe_last_error()
+    # the same pair in opposite directions
+    keep, args = _create_args([(1, 2.0, 0, 1), (1, 4.0, 1, 0)], 2)
+    assert built_lib.pygbe_create(*args, None, C.byref(h)) == pg.PYGBE_EINVAL
+    # the size query validates its arguments the same way
+    n = C.c_size_t(7)
+    keep, args = _create_args([(1, 2.0, 0, 1), (1, 4.0, 1, 2), (1, 6.0, 2, 0)], 3)
+    assert built_lib.pygbe_workspace_size(*args, None, 100, C.byref(n)) == pg.PYGBE_EINVAL and n.value == 0
+    assert built_lib.pygbe_workspace_size(*args, None, 100, None) == pg.PYGBE_EINVAL
+
+
+def test_options_reject_bad_workspace_and_group_mac(built_lib):
+    h = C.c_void_p(1)
+    keep, args = _create_args([(1, 2.0, 0, 1)], 2)
+    opt = pg.pygbe_options(group_mac=2)
+    assert built_lib.pygbe_create(*args, C.byref(opt), C.byref(h)) == pg.PYGBE_EINVAL
+    opt = pg.pygbe_options(workspace=C.c_void_p(0x1001), workspace_bytes=1 << 20)     # not 256-byte aligned
+    assert built_lib.pygbe_create(*args, C.byref(opt), C.byref(h)) == pg.PYGBE_EINVAL
+    assert b"aligned" in built_lib.pygbe_last_error()
+    opt = pg.pygbe_options(workspace_bytes=1 << 20)                                   # size without a block
+    assert built_lib.pygbe_create(*args, C.byref(opt), C.byref(h)) == pg.PYGBE_EINVAL
+
+
+def test_no_environment_knobs_in_the_product_build():
+    """Tuning knobs are compiled out unless -DPYGBE_TUNING: the only getenv of the library sits behind that flag."""
+    csrc = os.path.join(ROOT, "paper_1309_4018_b200", "csrc")
+    hits = []
+    for f in sorted(os.listdir(csrc)):
+        for i, line in enumerate(open(os.path.join(csrc, f)), 1):
+            if re.search(r"\bgetenv\s*\(", line) and not line.strip().startswith("//"):
+                hits.append((f, i))
+    assert hits == [("common.cuh", hits[0][1])] and len(hits) == 1

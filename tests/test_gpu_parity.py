@@ -136,7 +136,7 @@ def test_gmres_basis_longer_than_one_coefficient_pass(env):
     one, and its residual must hold when recomputed from b - A x with one more matvec."""
     pg, torch, orc = env
     prob = W.protein_problem(250, spacing=1.1, seed=31)
-    h = pg.Handle.from_problem(prob, K=4, P=6, theta=0.5)
+    h = pg.Handle.from_problem(prob, K=4, P=6, theta=0.5, gmres_restart=600)
     xa, ita, rra, _ = h.solve(tol=1e-11, restart=600, max_iter=600)
     assert ita > 256 and rra <= 1e-11
     b = h.rhs()
@@ -244,10 +244,10 @@ def test_treecode_error_decreases_with_order(env):
     assert all(b < a for a, b in zip(errs, errs[1:]))
 
 
-def test_group_mac_on_own_targets_is_within_the_bound_and_shortens_the_lists(env, monkeypatch):
+def test_group_mac_on_own_targets_is_within_the_bound_and_shortens_the_lists(env):
     """Reading A9: a cell is accepted for a group iff eq. (15) holds for every target.  The traversal decides that
     from the group's bounding volume where it can and from the 64 points themselves where the bound is undecided;
-    with PYGBE_BOUND_MAC set it uses the bound alone.  Both must meet the 1e-4 bar; the exact test must give
+    with pygbe_options.group_mac = 1 it uses the bound alone.  Both must meet the 1e-4 bar; the exact test must give
     shorter direct lists (every cell the bound accepts is also accepted by the exact minimum)."""
     pg, torch, orc = env
     prob = W.kirkwood_problem(4)
@@ -256,15 +256,10 @@ def test_group_mac_on_own_targets_is_within_the_bound_and_shortens_the_lists(env
     yo = o.matvec(x)
     res = {}
     for mode in ("exact", "bound"):
-        if mode == "bound":
-            monkeypatch.setenv("PYGBE_BOUND_MAC", "1")
-        else:
-            monkeypatch.delenv("PYGBE_BOUND_MAC", raising=False)
-        h, y = gpu_matvec(pg, torch, prob, x, K=4, P=6, theta=0.5)
+        h, y = gpu_matvec(pg, torch, prob, x, K=4, P=6, theta=0.5, group_mac=1 if mode == "bound" else 0)
         st = h.stats()
         res[mode] = (rel(y, yo), st["p2p_pairs"], st["m2p_evals"])
         h.close()
-    monkeypatch.delenv("PYGBE_BOUND_MAC", raising=False)
     assert res["exact"][0] <= TOL_TREE and res["bound"][0] <= TOL_TREE
     assert res["exact"][1] < 0.9 * res["bound"][1]
     assert res["bound"][0] <= res["exact"][0]          # the bound is the stricter acceptance
@@ -615,3 +610,132 @@ def test_binding_energy_small(env):
     dd_ours = ours[0] - ours[1] - ours[2]
     dd_ref = ref[0] - ref[1] - ref[2]
     assert abs(dd_ours - dd_ref) <= 1e-8 * abs(ref[0])
+
+
+# --------------------------------------------------------------- full-size configs 2 and 4 (sampled oracle rows)
+def _full_size_checks(pg, torch, orc, prob, kw, nrows, seed):
+    """Sampled-row parity at a configuration's full size: oracle rows one by one for a seeded
+    input vector, both precisions through the treecode; the right-hand side on sampled rows; the Gauss identity
+    (phi = 1, dphi/dn = 0 gives 0 on the rows of the region enclosed by the first surface) as a property."""
+    o = orc.Oracle(prob, K=kw["K"])
+    rng = np.random.default_rng(seed)
+    x = rng.normal(size=o.n)
+    rows = np.sort(rng.choice(o.n, nrows, replace=False))
+    yo = o.matvec(x, rows)
+    out = {}
+    for name, prec in (("fp64", pg.PRECISION_FP64), ("mixed", pg.PRECISION_MIXED)):
+        h = pg.Handle.from_problem(prob, precision=prec, **kw)
+        st = h.stats()
+        assert st["m2p_evals"] > 0 and st["p2p_pairs"] < 0.05 * st["direct_equiv"]
+        y = h.matvec(torch.tensor(x, device="cuda")).cpu().numpy()
+        err = rel(y[rows], yo)
+        out[name] = err
+        assert err <= TOL_TREE, (name, err)
+        assert np.max(np.abs(y[rows] - yo)) <= 1e-3 * np.max(np.abs(yo)), name
+        if name == "fp64":
+            assert rel(h.rhs().cpu().numpy(), o.rhs()) <= 1e-13          # every row: N x n_charges oracle evaluations
+            S0 = prob.surfaces[0]
+            ones = np.zeros(o.n)
+            at = 0
+            for S in prob.surfaces:                            # phi = 1 on every surface bounding region_in(S0)
+                if S.region_in == S0.region_in:
+                    ones[at:at + S.n_panels] = 1.0
+                at += 2 * S.n_panels
+            g = h.matvec(torch.tensor(ones, device="cuda")).cpu().numpy()
+            gi = np.abs(g[:S0.n_panels])
+            # slivers of the marching surfaces defeat the centroid-distance near-field rule locally (max), not
+            # globally (median, as in the oracle's own pin in test_workloads.py); the worst rows are a property of
+            # the discretisation D0, not of the treecode: the oracle gives the same values there
+            assert np.median(gi) < 2e-3
+            worst = np.sort(np.argsort(gi)[-40:])
+            go = o.matvec(ones, worst)
+            assert np.max(np.abs(g[worst] - go)) <= 1e-4 * max(1.0, np.max(np.abs(go)))
+        h.close()
+    return out
+
+
+def test_protein_full_size_sampled_rows(env):
+    """BASELINE.json configs[2] at full size: synthetic protein, 1000 atoms, 41.5 k panels, K = 4, P = 6,
+    theta = 0.5, fp64 and mixed; 2000 oracle rows."""
+    pg, torch, orc = env
+    prob = W.cached("protein_1000_s105", lambda: W.protein_problem(1000, spacing=1.05))
+    assert 38_000 < prob.n_panels < 46_000
+    errs = _full_size_checks(pg, torch, orc, prob, dict(K=4, P=6, theta=0.5), 2000, 52)
+    print("configs[2] rel-L2 vs oracle rows:", errs)
+
+
+def test_binding_complex_full_size_sampled_rows(env):
+    """BASELINE.json configs[4] at full size, the complex (the configuration bench.py times): receptor 5000 +
+    ligand 500 atoms, 1.08 M panels, three regions without twins (k_m2p_lap on the two Laplace regions, the
+    regrouped single-set kernel on the solvent), K = 4, P = 8, theta = 0.5, mixed and fp64; 2000 oracle rows
+    (4.3 M Green evaluations each), right-hand side, Gauss identity."""
+    pg, torch, orc = env
+    prob = W.cached("binding_complex_5000_500_s055",
+                    lambda: W.binding_problems(5000, 500, spacing=0.55, only=("complex",))[0])
+    assert 1_000_000 < prob.n_panels < 1_150_000 and len(prob.surfaces) == 3
+    errs = _full_size_checks(pg, torch, orc, prob, dict(K=4, P=8, theta=0.5), 2000, 54)
+    print("configs[4] complex rel-L2 vs oracle rows:", errs)
+
+
+# ------------------------------------------------------------------------------------------ workspace (8(b))
+def test_workspace_contract(env):
+    """pygbe_workspace_size + pygbe_options.workspace: with the binding's default every byte of the handle is a
+    torch allocation; a block that is too small is refused with PYGBE_ENOMEM; results do not depend on where the
+    memory comes from."""
+    pg, torch, orc = env
+    prob = W.kirkwood_problem(4)
+    kw = dict(K=4, P=6, theta=0.5)
+    need = pg.Handle.workspace_size(prob, gmres_restart=50, **kw)
+    assert need > 0
+    torch.cuda.synchronize()
+    m0 = torch.cuda.memory_allocated()
+    h = pg.Handle.from_problem(prob, gmres_restart=50, **kw)
+    assert h.workspace is not None and h.workspace.numel() == need
+    assert torch.cuda.memory_allocated() - m0 >= need
+    x = torch.tensor(np.random.default_rng(1).normal(size=h.n), device="cuda")
+    y = h.matvec(x).cpu().numpy()
+    xs, it, rr, rc = h.solve(tol=1e-6, restart=50)
+    es, ec = h.energy(xs)
+    yh = h.matvec_host(x.cpu().numpy())
+    st = h.stats()
+    assert 0 < st["device_bytes"] <= st["workspace_high_water"] <= need
+    h.close()
+    # the library's own pool gives the same numbers
+    h2 = pg.Handle.from_problem(prob, workspace=None, **kw)
+    assert h2.workspace is None
+    assert rel(h2.matvec(x).cpu().numpy(), y) < 1e-12
+    xs2, it2, _, _ = h2.solve(tol=1e-6, restart=50)
+    assert abs(h2.energy(xs2)[0] - es) <= 1e-7 * abs(es)
+    h2.close()
+    # too small: refused, no handle
+    small = torch.empty(need // 3, dtype=torch.uint8, device="cuda")
+    with pytest.raises(pg.PygbeError) as ei:
+        pg.Handle.from_problem(prob, workspace=small, **kw)
+    assert ei.value.code == pg.PYGBE_ENOMEM and "workspace" in str(ei.value)
+    # sized for create only (restart 1): a longer GMRES basis does not fit and says so
+    tight = torch.empty(pg.Handle.workspace_size(prob, gmres_restart=1, **kw), dtype=torch.uint8, device="cuda")
+    h3 = pg.Handle.from_problem(prob, workspace=tight, **kw)
+    with pytest.raises(pg.PygbeError) as ei:
+        h3.solve(tol=1e-6, restart=400)
+    assert ei.value.code == pg.PYGBE_ENOMEM
+    assert rel(h3.matvec(x).cpu().numpy(), y) < 1e-12           # the handle is still usable
+    h3.close()
+
+
+def test_many_charges_reaction_potential(env):
+    """More than 65535 charges in one region (grid dimension limit of the first version of k_reaction): energy
+    against the oracle's functional on the same x."""
+    pg, torch, orc = env
+    v, t = W.icosphere(2, 6.0)
+    rng = np.random.default_rng(8)
+    nq = 70_000
+    pts = rng.normal(size=(nq, 3)); pts *= (rng.uniform(0, 4.0, size=(nq, 1)) / np.linalg.norm(pts, axis=1, keepdims=True))
+    q = rng.uniform(-1, 1, size=nq) * 1e-2
+    prob = W.Problem([W.Surface(v, t, 0, 1)], [4.0, 80.0], [0.0, 0.125], pts, q, np.zeros(nq, dtype=np.int32))
+    h = pg.Handle.from_problem(prob, K=4, theta=0.0)
+    x = torch.tensor(rng.normal(size=h.n), device="cuda")
+    es, _ = h.energy(x)
+    o = orc.Oracle(prob)
+    eo = o.solvation_energy(x.cpu().numpy())
+    assert abs(es - eo) <= 1e-10 * abs(eo)
+    h.close()

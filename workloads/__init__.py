@@ -10,6 +10,7 @@ from .spheres import (icosphere, born_problem, kirkwood_problem, stern_sphere_pr
 from .problem import Problem, Surface, concat_problem_arrays
 from .molecule import (saw_molecule, density_surface, marching_tetrahedra, validate_closed_mesh,
                        protein_problem, multisurface_problem, binding_problems)
+from .cache import cached, save_problem, load_problem
 
 SEED0 = 13094018
 
@@ -18,4 +19,5 @@ __all__ = [
     "nested_sphere_problem",
     "Problem", "Surface", "concat_problem_arrays", "saw_molecule", "density_surface", "marching_tetrahedra",
     "validate_closed_mesh", "protein_problem", "multisurface_problem", "binding_problems", "SEED0",
+    "cached", "save_problem", "load_problem",
 ]
