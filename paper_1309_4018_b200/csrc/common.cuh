@@ -197,7 +197,8 @@ struct Region {
     int *p2m_cells = nullptr; int n_p2m = 0;        // needed leaves (P2M)
     int4 *p2m_rec = nullptr;                        // per needed leaf: (cell, first panel, end panel, 0)
     int4 *m2m_rec = nullptr; int n_m2m = 0;         // needed internal cells, deepest level first: (cell, first child, n children, internal-child mask)
-    double *pmom = nullptr;                         // [np][2][Nc] geometry-only panel moments about the panel's leaf centre (P2M)
+    double *pmom = nullptr;                         // [np][2][Nc] geometry-only panel moments about the panel's leaf centre (P2M), fp64
+    float *pmomf = nullptr;                         // the same in fp32 (mixed precision; pmom is then not allocated)
     int *up_sync = nullptr;                         // [2] ticket and exit counters of the upward pass
     int *cready = nullptr;                          // [ncells] matvec number at which the cell's multipoles were built
     double Lmax = 0;                // max panel length sqrt(2A) on this region's boundary
@@ -267,6 +268,12 @@ struct pygbe_handle {
     cudaStream_t side2 = nullptr;   // near-field correction SpMV runs here
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_join2 = nullptr;
     bool overlap = true;
+    // Large problems: the upward pass (P2M stream, M2M) is bandwidth- and latency-bound and runs beside the
+    // FMA-bound P2P; at full width its CTAs (high priority, 350-512 threads, few of them busy) take the thread
+    // slots of every SM and the P2P waits, so the two run one after the other.  Capped at 2 (P2M) / 1 (M2M) CTAs
+    // per SM they share the SMs: 16.5 -> 15.5 ms per matvec on the 1.08 M-panel complex.  Small problems keep the
+    // full width: there the far-field chain is the critical path.
+    bool narrow_upward = false;
     // optional block-diagonal right preconditioner of GMRES (pygbe_options.precond)
     int precond = 0;
     bool dry = false;               // size query (pygbe_workspace_size): allocate as create does, compute no values

@@ -62,12 +62,15 @@ __device__ __forceinline__ void wc_store(const MomOut &o, long cell, const doubl
 // then a streaming product: 2 Nc doubles read per panel, coalesced, two FMAs per 16 bytes -- HBM / L2 bound
 // as SURVEY 8(d) puts it (27.5 MB at 20 480 panels and P = 6) instead of the ALU- and latency-bound
 // monomial loop over the Gauss points of the first versions (29 us -> see profiles/r2a_regrouped_path.md).
-// pmom[panel][set][Nc], panels in the region's Morton order.
+// pmom[panel][set][Nc], panels in the region's Morton order; fp64, or fp32 in mixed precision (TM = float: the
+// M2P reads fp32 coefficients anyway, the stream is half as long -- 1.4 instead of 2.85 GB for the 1.08 M panels of
+// the Stern-layer region of config 4 at P = 8 -- and the sums over the panels of a leaf stay fp64).
 #define PMOM_THREADS 128
+template <typename TM>
 __global__ void __launch_bounds__(PMOM_THREADS)
 k_panel_moments(int P, int Nc, int K, const IndexTables *__restrict__ tab, const int *__restrict__ leaf_cell,
                 const double4 *__restrict__ cgeo, const int2 *__restrict__ crange,
-                const double4 *__restrict__ spos, const double4 *__restrict__ pnrm, double *__restrict__ pmom)
+                const double4 *__restrict__ spos, const double4 *__restrict__ pnrm, TM *__restrict__ pmom)
 {
     const int cell = leaf_cell[blockIdx.x];
     const double4 cg = cgeo[cell];
@@ -89,8 +92,8 @@ k_panel_moments(int P, int Nc, int K, const IndexTables *__restrict__ tab, const
             gv += s.w * X * Y * Z;
             gk += s.w * (n.x * kx * X1 * Y * Z + n.y * ky * X * Y1 * Z + n.z * kz * X * Y * Z1);
         }
-        pmom[((long)j * 2) * Nc + k] = gv;
-        pmom[((long)j * 2 + 1) * Nc + k] = gk;
+        pmom[((long)j * 2) * Nc + k] = (TM)gv;
+        pmom[((long)j * 2 + 1) * Nc + k] = (TM)gk;
     }
 }
 
@@ -99,9 +102,10 @@ k_panel_moments(int P, int Nc, int K, const IndexTables *__restrict__ tab, const
 #define P2M_MAXT 512
 static inline int p2m_nsplit(int Nc) { return Nc >= 192 ? 1 : (Nc >= 96 ? 2 : (256 / Nc > 8 ? 8 : 256 / Nc)); }
 static inline int p2m_threads(int Nc) { return (p2m_nsplit(Nc) * Nc + 31) / 32 * 32; }
+template <typename TM>
 __global__ void __launch_bounds__(P2M_MAXT)
 k_p2m(const int *__restrict__ skip, int Nc, int nsplit, int n_leaves, const int4 *__restrict__ rec, const double2 *__restrict__ pq,
-      const double *__restrict__ pmom, double *__restrict__ mom, MomOut mo)
+      const TM *__restrict__ pmom, double *__restrict__ mom, MomOut mo)
 {
     __shared__ double s_part[2][P2M_MAXT];
     if (skip && *skip) return;
@@ -113,11 +117,11 @@ k_p2m(const int *__restrict__ skip, int Nc, int nsplit, int n_leaves, const int4
     const int cell = rc.x;
     double aV = 0.0, aK = 0.0;
     if (active) {
-#pragma unroll 4
+#pragma unroll 8
         for (int j = rc.y + sp; j < rc.z; j += nsplit) {
             const double2 q = pq[j];                               // (cV dphi, cK phi) of panel j, from k_prep
-            aV += q.x * pmom[((long)j * 2) * Nc + k];
-            aK += q.y * pmom[((long)j * 2 + 1) * Nc + k];
+            aV += q.x * (double)pmom[((long)j * 2) * Nc + k];
+            aK += q.y * (double)pmom[((long)j * 2 + 1) * Nc + k];
         }
         if (sp > 0) { s_part[0][t] = aV; s_part[1][t] = aK; }
     }

@@ -174,15 +174,17 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
             else { mo.NW = h->NW; mo.wt_off = h->wt_off; mo.wt_k = h->wt_k; mo.wt_c = h->wt_c; mo.wt_deg = nullptr; }
             STAGE(h, PYGBE_STAGE_P2M, A.id);
             if (A.n_p2m > 0) {
-                int p2m_grid = A.n_p2m;
+                // leaves are taken grid-stride; on large problems the grid is capped (see h->narrow_upward)
+                int p2m_grid = h->narrow_upward ? std::min(A.n_p2m, 2 * h->n_sm) : A.n_p2m;
                 if (const char *e = tune_env("PYGBE_P2M_GRID")) p2m_grid = std::min(A.n_p2m, std::max(1, atoi(e)));   // tuning
-                LAUNCH(h, k_p2m, p2m_grid, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.n_p2m, A.p2m_rec, A.pq, A.pmom, A.mom, mo);
+                if (mixed) LAUNCH(h, k_p2m<float>, p2m_grid, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.n_p2m, A.p2m_rec, A.pq, A.pmomf, A.mom, mo);
+                else LAUNCH(h, k_p2m<double>, p2m_grid, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.n_p2m, A.p2m_rec, A.pq, A.pmom, A.mom, mo);
             }
             STAGE_END(h, PYGBE_STAGE_P2M);
             STAGE(h, PYGBE_STAGE_M2M, A.id);
             if (A.n_m2m > 0) {
                 M2MLaunch ml;
-                ml.skip = skip; ml.P = h->P; ml.Nc = h->Nc; ml.n_cells = A.n_m2m; ml.grid = std::min(A.n_m2m, (tune_env("PYGBE_M2M_GRID") ? atoi(tune_env("PYGBE_M2M_GRID")) : 3) * h->n_sm);   // tuning
+                ml.skip = skip; ml.P = h->P; ml.Nc = h->Nc; ml.n_cells = A.n_m2m; ml.grid = std::min(A.n_m2m, (tune_env("PYGBE_M2M_GRID") ? atoi(tune_env("PYGBE_M2M_GRID")) : (h->narrow_upward ? 1 : 3)) * h->n_sm);   // tuning
                 ml.rec = A.m2m_rec; ml.tab = h->itab; ml.cgeo = A.cgeo; ml.mom = A.mom; ml.mo = mo; ml.sync = A.up_sync;
                 ml.ready = A.cready; ml.epoch = (int)(h->n_matvec + 1); ml.stream = h->stream;
                 m2m_launch(ml);

@@ -128,9 +128,9 @@ static void describe_launch(const pygbe_handle *h, int stage, const Region &A, p
         o->bytes = np * (16 + 8 + 16 + 32 + 8 + 8 + 16 + 8 * nreg) + npts * (8 + (mixed ? 16 : 32));
         break;
     case PYGBE_STAGE_P2M: {
-        name = "k_p2m"; o->units = A.p2m_panels;
+        name = mixed ? "k_p2m<float>" : "k_p2m<double>"; o->units = A.p2m_panels;
         // per panel of a needed leaf: its two moment sets (pmom) and its two weights; per leaf: mom and the wc row written
-        o->bytes = A.p2m_panels * (2 * Nc * 8 + 16) + (int64_t)A.n_p2m * (2 * Nc * 8 + wrow);
+        o->bytes = A.p2m_panels * (2 * Nc * (mixed ? 4 : 8) + 16) + (int64_t)A.n_p2m * (2 * Nc * 8 + wrow);
         break; }
     case PYGBE_STAGE_M2M:
         name = "k_m2m"; o->units = A.n_m2m;
