@@ -329,3 +329,49 @@ def test_transparent_interfaces(orc):
     cav80 = orc.Oracle(W.cavity_sphere_problem(2))
     xc8, _, _ = cav80.solve(tol=1e-10)
     assert abs(cav80.solvation_energy(xc8) - Er) / abs(Er) > 0.03      # a real cavity does matter
+
+
+# ------------------------------------------------------------- two small branches ("unpinned (mine)")
+def test_rhs_of_a_charge_in_a_screened_region(orc):
+    """orc_rhs with a charge sitting in a kappa != 0 region (eq. 9/11 with the Yukawa Green's function,
+    PAPER.md:55-58, :98): rows of that region are q exp(-kappa r) / (4 pi eps r), rows of the other region 0.
+    Every other test keeps its charges in kappa = 0 regions, so the exp(-kappa r) factor would go unnoticed."""
+    p = W.born_problem(1)
+    pos = np.array([[0.0, 0.0, 7.0], [5.0, -6.0, 1.0]])
+    q = np.array([0.75, -1.25])
+    p.charge_xyz, p.charge_q, p.charge_region = pos, q, np.array([1, 1], dtype=np.int32)
+    o = orc.Oracle(p)
+    c, _, _ = o.geometry()
+    b = o.rhs()
+    N = o.npan
+    kappa, eps2 = 0.125, 80.0
+    want = sum(qk * np.exp(-kappa * np.linalg.norm(c - rk, axis=1)) / (4 * math.pi * eps2 * np.linalg.norm(c - rk, axis=1))
+               for qk, rk in zip(q, pos))
+    assert np.all(b[:N] == 0.0)
+    assert np.allclose(b[N:], want, rtol=1e-14, atol=0)
+    # and it is not the Laplace value: the screening changes the rows by tens of per cent at these distances
+    lap = sum(qk / (4 * math.pi * eps2 * np.linalg.norm(c - rk, axis=1)) for qk, rk in zip(q, pos))
+    assert np.max(np.abs(b[N:] - lap) / np.abs(lap)) > 0.2
+
+
+def test_near_singular_rule_switches_at_thres_squared_times_2A(orc):
+    """Reading A7: the K_fine-point rule replaces the K-point rule iff |x_i - c_j|^2 < thres^2 * 2 A_j,
+    strictly, with L_j = sqrt(2 A_j).  Constructed pair: source = right triangle with legs 1 (2A = 1 exactly),
+    target = the same triangle lifted by 2 in z (centroid distance exactly 2, d^2 = 4 exactly).  The two candidate
+    values come from the oracle itself with the rule forced on (thres huge) and off (thres 0)."""
+    src = np.array([[0.0, 0, 0], [1.0, 0, 0], [0.0, 1, 0]])
+    tgt = src + np.array([0.0, 0.0, 2.0])
+    verts = np.concatenate([src, tgt])
+    tris = np.array([[0, 1, 2], [3, 4, 5]], dtype=np.int32)
+    p = W.Problem([W.Surface(verts, tris, 0, 1)], [4.0, 80.0], [0.0, 0.125], np.zeros((1, 3)), [1.0], [0])
+
+    def entry(thres, region=1):
+        return orc.Oracle(p, K=4, K_fine=19, thres=thres).entry(region, 1, 0)      # target panel 1, source panel 0
+
+    fine, coarse = entry(1e9), entry(0.0)
+    assert abs(fine[0] - coarse[0]) > 1e-6 * abs(fine[0])                        # the two rules differ measurably here
+    assert entry(2.0) == coarse                      # d^2 = 4 = thres^2 * 2A: strict '<', the K-point rule stays
+    assert entry(2.0 * (1 + 1e-15)) == fine          # one ulp above: K_fine
+    assert entry(2.5) == fine                        # thres^2 * 2A = 6.25 > 4;  with L^2 = A it would be 3.125 < 4
+    assert entry(1.99) == coarse
+    assert entry(2.9, region=0) == orc.Oracle(p, thres=1e9).entry(0, 1, 0)       # same switch under the Laplace kernel
