@@ -118,7 +118,9 @@ typedef struct {
     int64_t workspace_high_water;/* workspace bytes the allocations made so far needed at their peak   */
     int64_t n_matvec;            /* matvecs executed so far                                            */
     int64_t kernels_per_matvec;  /* kernel launches one pygbe_matvec issues                            */
-    int64_t kernel_launches;     /* all kernel launches issued by this handle so far                   */
+    int64_t kernel_launches;     /* all kernel launches issued by this handle so far (inside graphs too) */
+    int64_t graph_launches;      /* cudaGraphLaunch calls so far: a matvec is one graph, `poll` GMRES  */
+                                 /* iterations are one graph; 0 if capture is unavailable              */
     double  create_ms, last_solve_ms;
     int32_t last_iters;
     int32_t P, K, precision;

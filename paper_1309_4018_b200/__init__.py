@@ -46,7 +46,7 @@ class pygbe_stats_t(C.Structure):
     _fields_ = [(n, C.c_int64) for n in (
         "n_panels", "n_unknowns", "n_regions", "n_surfaces", "n_charges", "n_points", "n_cells", "n_leaves",
         "n_groups", "tree_depth", "p2p_pairs", "m2p_evals", "direct_equiv", "near_nnz", "device_bytes",
-        "workspace_high_water", "n_matvec", "kernels_per_matvec", "kernel_launches")] + [
+        "workspace_high_water", "n_matvec", "kernels_per_matvec", "kernel_launches", "graph_launches")] + [
         ("create_ms", C.c_double), ("last_solve_ms", C.c_double), ("last_iters", C.c_int32),
         ("P", C.c_int32), ("K", C.c_int32), ("precision", C.c_int32), ("theta", C.c_double)]
 

@@ -151,8 +151,8 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
         std::vector<int4> p2m_rec;
         for (int c : p2m_cells) p2m_rec.push_back(make_int4(c, crange_h[c].x, crange_h[c].y, 0));
         TRY(upload(h, &R.p2m_rec, p2m_rec));
-        TRY(h->mem.alloc(&R.up_sync, 2)); TRY(h->mem.alloc(&R.cready, (size_t)ncells));
-        CUDA_TRY(cudaMemsetAsync(R.up_sync, 0, 2 * sizeof(int), h->stream));
+        TRY(h->mem.alloc(&R.up_sync, 4)); TRY(h->mem.alloc(&R.cready, (size_t)ncells));
+        CUDA_TRY(cudaMemsetAsync(R.up_sync, 0, 4 * sizeof(int), h->stream));
         CUDA_TRY(cudaMemsetAsync(R.cready, 0, (size_t)ncells * sizeof(int), h->stream));
     }
     int over = 0;

@@ -199,7 +199,7 @@ struct Region {
     int4 *m2m_rec = nullptr; int n_m2m = 0;         // needed internal cells, deepest level first: (cell, first child, n children, internal-child mask)
     double *pmom = nullptr;                         // [np][2][Nc] geometry-only panel moments about the panel's leaf centre (P2M), fp64
     float *pmomf = nullptr;                         // the same in fp32 (mixed precision; pmom is then not allocated)
-    int *up_sync = nullptr;                         // [2] ticket and exit counters of the upward pass
+    int *up_sync = nullptr;                         // [4] ticket and exit counters of the upward pass, number of passes so far
     int *cready = nullptr;                          // [ncells] matvec number at which the cell's multipoles were built
     double Lmax = 0;                // max panel length sqrt(2A) on this region's boundary
     double root_c[3] = {0, 0, 0}, root_edge = 1;
@@ -229,6 +229,30 @@ struct Region {
     int nq = 0;
     double4 *qpos = nullptr;        // (x, y, z, q)
     int *qid = nullptr;             // caller's charge index
+};
+
+// A vector that a kernel reads or writes, resolved on the device so that one captured launch (CUDA graph) serves
+// every caller buffer and every Krylov vector: base pointer taken from a device slot (or given directly), plus
+// sel[0] * stride elements (the column of the Krylov basis the iteration is at).
+struct VecRef {
+    const double *const *slot;      // device slot holding the base pointer, or nullptr
+    const double *ptr;              // base pointer when slot == nullptr
+    const int *sel; long stride;    // optional column selector
+    __device__ __forceinline__ const double *get() const
+    {
+        const double *b = slot ? *slot : ptr;
+        return b + (sel ? (long)sel[0] * stride : 0L);
+    }
+};
+static inline VecRef vec_direct(const double *p) { VecRef v; v.slot = nullptr; v.ptr = p; v.sel = nullptr; v.stride = 0; return v; }
+static inline VecRef vec_slot(const double *const *s, const int *sel = nullptr, long stride = 0) { VecRef v; v.slot = s; v.ptr = nullptr; v.sel = sel; v.stride = stride; return v; }
+
+// An instantiated CUDA graph of a fixed launch sequence, with what identifies the sequence (pointers, sizes, tol)
+struct GraphSlot {
+    cudaGraphExec_t exec = nullptr;
+    long key[6] = {0, 0, 0, 0, 0, 0};
+    long nlaunch = 0, nmatvec = 0;
+    bool failed = false;            // capture or instantiation failed once: direct launches from then on
 };
 
 struct GmresWork {
@@ -267,6 +291,16 @@ struct pygbe_handle {
     cudaStream_t side = nullptr;    // far-field chain (P2M, M2M, M2P) runs here, concurrently with P2P
     cudaStream_t side2 = nullptr;   // near-field correction SpMV runs here
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_join2 = nullptr;
+    // CUDA graphs: the kernel sequence of a matvec (7+ launches on three streams) and of a block of GMRES iterations is
+    // captured once on capst and replayed with one cudaGraphLaunch on the caller's stream (which may be the legacy
+    // default stream, where capture itself is not allowed)
+    cudaStream_t capst = nullptr;
+    bool use_graphs = true;
+    const double **io = nullptr;    // device slots: [0], [1] x and y of pygbe_matvec; [2], [3] input base and output of the GMRES iteration
+    const double *io_host[4] = {nullptr, nullptr, nullptr, nullptr};   // what the slots hold
+    GraphSlot g_matvec, g_iter;
+    long graph_launches = 0;
+    char graph_note[160] = "";      // why a capture failed, if one did
     bool overlap = true;
     // Large problems: the upward pass (P2M stream, M2M) is bandwidth- and latency-bound and runs beside the
     // FMA-bound P2P; at full width its CTAs (high priority, 350-512 threads, few of them busy) take the thread

@@ -210,13 +210,16 @@ template <int PM>
 __global__ void __launch_bounds__(M2M_THREADS)
 k_m2m(const int *__restrict__ skip, int P, int Nc, int n_cells, const int4 *__restrict__ rec,
       const IndexTables *__restrict__ tab, const double4 *__restrict__ cgeo, double *mom, MomOut mo,
-      int *sync, int *ready, int epoch)
+      int *sync, int *ready)
 {
     extern __shared__ double s_m[];
     __shared__ short s_idx3[PYGBE_PMAX + 1][PYGBE_PMAX + 1][PYGBE_PMAX + 1];
     __shared__ double s_sh[8][3];
     __shared__ int s_ticket;
     if (skip && *skip) return;
+    // ready flags hold the number of the upward pass that built the cell; sync[2] counts the passes and is advanced by
+    // the last CTA to leave (after every CTA has read it), so that a captured launch needs no per-launch argument
+    const int epoch = ld_acquire(sync + 2) + 1;
     const int n2 = 2 * Nc, nl = (P + 1) * (P + 2) / 2;
     for (int i = threadIdx.x; i < (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1) * (PYGBE_PMAX + 1); i += M2M_THREADS)
         (&s_idx3[0][0][0])[i] = (&tab->idx3[0][0][0])[i];
@@ -271,18 +274,18 @@ k_m2m(const int *__restrict__ skip, int P, int Nc, int n_cells, const int4 *__re
     }
     if (threadIdx.x == 0) {
         const int d = atomicAdd(&sync[1], 1);
-        if (d == (int)gridDim.x - 1) { sync[1] = 0; __threadfence(); sync[0] = 0; }
+        if (d == (int)gridDim.x - 1) { sync[2] = epoch; sync[1] = 0; __threadfence(); sync[0] = 0; }
     }
 }
 
 struct M2MLaunch {
     const int *skip; int P, Nc, n_cells, grid; const int4 *rec; const IndexTables *tab; const double4 *cgeo;
-    double *mom; MomOut mo; int *sync, *ready; int epoch; cudaStream_t stream;
+    double *mom; MomOut mo; int *sync, *ready; cudaStream_t stream;
 };
 template <int PM> static void m2m_go(const M2MLaunch &a)
 {
     k_m2m<PM><<<a.grid, M2M_THREADS, m2m_smem_bytes(a.Nc), a.stream>>>(a.skip, a.P, a.Nc, a.n_cells, a.rec, a.tab, a.cgeo,
-                                                                      a.mom, a.mo, a.sync, a.ready, a.epoch);
+                                                                      a.mom, a.mo, a.sync, a.ready);
 }
 static void m2m_launch(const M2MLaunch &a)
 {

@@ -107,11 +107,12 @@ __global__ void k_precond_build(long npan, QuadTables q, const double *__restric
 // z (= or +=) M^-1 u, panel by panel.
 __global__ void __launch_bounds__(GM_THREADS)
 k_precond_apply(const int *__restrict__ flags, int respect_done, long npan, const double4 *__restrict__ pinv,
-                const int2 *__restrict__ pidx, const double *__restrict__ u, int add, double *__restrict__ z)
+                const int2 *__restrict__ pidx, VecRef ur, int add, double *__restrict__ z)
 {
     if (respect_done && flags[0]) return;
     long j = (long)blockIdx.x * GM_THREADS + threadIdx.x;
     if (j >= npan) return;
+    const double *__restrict__ u = ur.get();
     const int2 ix = pidx[j];
     const double4 m = pinv[j];
     const double u0 = u[ix.x], u1 = u[ix.y];
@@ -130,12 +131,15 @@ k_precond_apply(const int *__restrict__ flags, int respect_done, long npan, cons
 // The summation order of the partial dot products is not fixed (atomics, reading A19).
 #include <cooperative_groups.h>
 __global__ void __launch_bounds__(GM_THREADS)
-k_gm_arnoldi(int *flags, double *V, long n, int j, int m, double *w, double *h1, double *h2, double *nrm2, double *H,
+k_gm_arnoldi(int *flags, double *V, long n, int m, double *w, double *h1, double *h2, double *nrm2, double *H,
              double *cs, double *sn, double *g, double *scal, double tol)
 {
     namespace cgx = cooperative_groups;
     if (flags[0]) return;                                    // uniform: set before this launch or not at all
     cgx::grid_group grid = cgx::this_grid();
+    // the step number is the count of columns built so far; it is read here by every CTA and rewritten only after
+    // the last grid-wide barrier, so one captured launch serves every step
+    const int j = flags[1];
     typedef cub::BlockReduce<double, GM_THREADS> Red;
     __shared__ typename Red::TempStorage tmp;
     const int nvec = j + 1;

@@ -121,7 +121,7 @@ static void launch_p2p(pygbe_handle *h, Region &A, Region *B, const int *skip)
 //   side2 :            near-field corrections (all) -----------------^
 // Issuing every region's latency-bound kernels (prep, P2M, M2M, corrections) first lets them run beside the
 // compute-bound P2P / M2P of the regions before them instead of between them.
-static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *skip)
+static int matvec_impl(pygbe_handle *h, VecRef x, VecRef y, const int *skip)
 {
     const long before = h->launches;
     const bool mixed = h->precision == PYGBE_PRECISION_MIXED;
@@ -186,7 +186,7 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
                 M2MLaunch ml;
                 ml.skip = skip; ml.P = h->P; ml.Nc = h->Nc; ml.n_cells = A.n_m2m; ml.grid = std::min(A.n_m2m, (tune_env("PYGBE_M2M_GRID") ? atoi(tune_env("PYGBE_M2M_GRID")) : (h->narrow_upward ? 1 : 3)) * h->n_sm);   // tuning
                 ml.rec = A.m2m_rec; ml.tab = h->itab; ml.cgeo = A.cgeo; ml.mom = A.mom; ml.mo = mo; ml.sync = A.up_sync;
-                ml.ready = A.cready; ml.epoch = (int)(h->n_matvec + 1); ml.stream = h->stream;
+                ml.ready = A.cready; ml.stream = h->stream;
                 m2m_launch(ml);
                 h->launches++;
             }
@@ -223,4 +223,64 @@ static int matvec_impl(pygbe_handle *h, const double *x, double *y, const int *s
     h->kernels_per_matvec = h->launches - before;
     h->n_matvec++;
     return PYGBE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- CUDA graphs
+// Used on the small, launch-latency-bound problems only (h->use_graphs): stream capture does not carry a stream's
+// priority into the kernel nodes, and on the large problems the priorities of the side streams are what lets the
+// narrowed upward pass run beside the P2P (measured on the 1.08 M-panel complex: captured matvec 16.8 ms, like the
+// one without priorities; direct launches 15.5 ms; setting the node attribute after capture changed nothing).
+// body() issues launches through LAUNCH / matvec_impl; they are captured on h->capst (the caller's stream may be the
+// legacy default stream, which cannot capture) and instantiated.  Returns false if graphs are unavailable; the
+// caller then launches directly.
+template <class F> static bool graph_capture(pygbe_handle *h, GraphSlot &g, F &&body)
+{
+    if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+    cudaStream_t user = h->stream;
+    const long launches0 = h->launches, nmv0 = h->n_matvec, kpm0 = h->kernels_per_matvec;
+    auto why = [&](const char *what, cudaError_t e) {
+        snprintf(h->graph_note, sizeof(h->graph_note), "%s: %s", what, cudaGetErrorString(e));
+        if (tune_env("PYGBE_DEBUG")) fprintf(stderr, "[pygbe] graph capture failed: %s\n", h->graph_note);
+        cudaGetLastError(); g.failed = true;
+    };
+    { const cudaError_t e0 = cudaStreamBeginCapture(h->capst, cudaStreamCaptureModeThreadLocal); if (e0 != cudaSuccess) { why("begin capture", e0); return false; } }
+    h->stream = h->capst;
+    const int rc = body();
+    h->stream = user;
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(h->capst, &graph);
+    g.nlaunch = h->launches - launches0; g.nmatvec = h->n_matvec - nmv0;
+    h->launches = launches0; h->n_matvec = nmv0; h->kernels_per_matvec = kpm0;      // nothing has run yet
+    if (rc != PYGBE_OK || e != cudaSuccess || !graph) { if (graph) cudaGraphDestroy(graph); why(rc != PYGBE_OK ? pygbe_last_error() : "end capture", e); return false; }
+    const cudaError_t ei = cudaGraphInstantiate(&g.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess) { g.exec = nullptr; why("instantiate", ei); return false; }
+    return true;
+}
+static int graph_launch(pygbe_handle *h, GraphSlot &g)
+{
+    CUDA_TRY(cudaGraphLaunch(g.exec, h->stream));
+    h->launches += g.nlaunch; h->n_matvec += g.nmatvec; h->graph_launches++;
+    return PYGBE_OK;
+}
+static int set_slots(pygbe_handle *h, int first, const double *a, const double *b)
+{
+    if (h->io_host[first] == a && h->io_host[first + 1] == b) return PYGBE_OK;
+    LAUNCH(h, k_set_slots, 1, 1, 0, h->io, first, a, b);
+    h->io_host[first] = a; h->io_host[first + 1] = b;
+    return PYGBE_OK;
+}
+
+// y = A x for caller buffers: one graph launch (captured on first use), or direct launches while the stage timers
+// are on or when graphs are unavailable
+static int matvec_run(pygbe_handle *h, const double *x, double *y)
+{
+    TRY(set_slots(h, 0, x, y));
+    const VecRef xr = vec_slot(h->io), yr = vec_slot(h->io + 1);
+    if (h->profile || !h->use_graphs || h->g_matvec.failed) return matvec_impl(h, xr, yr, nullptr);
+    if (!h->g_matvec.exec) {
+        if (!graph_capture(h, h->g_matvec, [&]() { return matvec_impl(h, xr, yr, nullptr); })) return matvec_impl(h, xr, yr, nullptr);
+    }
+    h->kernels_per_matvec = h->g_matvec.nlaunch;
+    return graph_launch(h, h->g_matvec);
 }

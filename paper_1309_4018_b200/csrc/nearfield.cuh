@@ -28,10 +28,13 @@ __device__ __forceinline__ double pair_f64(double dx, double dy, double dz, doub
 }
 
 // ------------------------------------------------------------------------------- per-matvec weighting
+// the device slots that VecRef reads (one tiny launch whenever the caller's buffers change)
+__global__ void k_set_slots(const double **io, int first, const double *a, const double *b) { io[first] = a; io[first + 1] = b; }
+
 // Gather the densities of the region's panels from x and turn them into point "charges":
 //   mV_g = w_g A_j/(4pi) sigma_S c_S dphi_j,   mK_g = w_g A_j/(4pi) sigma_S phi_j n_j     (reading A4)
 // and clear the accumulator.
-__global__ void k_prep(const int *__restrict__ skip, int np, int K, const double *__restrict__ x, const int *__restrict__ phi_idx,
+__global__ void k_prep(const int *__restrict__ skip, int np, int K, VecRef xr, const int *__restrict__ phi_idx,
                        const int *__restrict__ dphi_idx, const double *__restrict__ cV,
                        const double *__restrict__ cK, const double4 *__restrict__ pnrm,
                        const double4 *__restrict__ spos, double4 *__restrict__ schg,
@@ -43,6 +46,7 @@ __global__ void k_prep(const int *__restrict__ skip, int np, int K, const double
     const long i = blockIdx.x * (long)blockDim.x + threadIdx.x;      // Gauss point
     if (i >= (long)np * K) return;
     const int p = (int)(i / K), g = (int)(i - (long)p * K);
+    const double *__restrict__ x = xr.get();
     const double phi = x[phi_idx[p]], dphi = x[dphi_idx[p]];
     const double qV = cV[p] * dphi, qK = cK[p] * phi;
     if (g == 0) {
@@ -232,11 +236,12 @@ k_near(const int *__restrict__ skip, int np, const int *__restrict__ off, const 
 __global__ void k_combine(const int *__restrict__ skip, int np, const double *__restrict__ pphi,
                           const double *__restrict__ outA, const double *__restrict__ outB,
                           const double *__restrict__ corrA, const double *__restrict__ corrB,
-                          const int *__restrict__ rowA, const int *__restrict__ rowB, double *__restrict__ y)
+                          const int *__restrict__ rowA, const int *__restrict__ rowB, VecRef yr)
 {
     if (skip && *skip) return;
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= np) return;
+    double *__restrict__ y = const_cast<double *>(yr.get());
     const double half_phi = 0.5 * pphi[t];
     y[rowA[t]] = half_phi - (outA[t] + corrA[t]);
     if (outB) y[rowB[t]] = half_phi - (outB[t] + corrB[t]);

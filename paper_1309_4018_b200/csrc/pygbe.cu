@@ -50,6 +50,9 @@ static void free_handle(pygbe_handle *h)
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->ev_join) cudaEventDestroy(h->ev_join);
     if (h->ev_join2) cudaEventDestroy(h->ev_join2);
+    if (h->g_matvec.exec) cudaGraphExecDestroy(h->g_matvec.exec);
+    if (h->g_iter.exec) cudaGraphExecDestroy(h->g_iter.exec);
+    if (h->capst) cudaStreamDestroy(h->capst);
     if (h->side) cudaStreamDestroy(h->side);
     if (h->side2) cudaStreamDestroy(h->side2);
     delete h;
@@ -73,7 +76,7 @@ extern "C" int pygbe_matvec(pygbe_handle *h, const double *x_dev, double *y_dev)
 {
     if (!h || !x_dev || !y_dev || x_dev == y_dev) { pygbe_set_error("matvec: null or aliased pointers"); return PYGBE_EINVAL; }
     CUDA_TRY(cudaSetDevice(h->device));
-    TRY(matvec_impl(h, x_dev, y_dev, nullptr));
+    TRY(matvec_run(h, x_dev, y_dev));
     CUDA_TRY(cudaGetLastError());
     return PYGBE_OK;
 }
@@ -85,7 +88,7 @@ extern "C" int pygbe_matvec_host(pygbe_handle *h, const double *x_host, double *
     TRY(ensure_host_staging(h));
     size_t bytes = 2 * h->npan * sizeof(double);
     CUDA_TRY(cudaMemcpyAsync(h->xh, x_host, bytes, cudaMemcpyHostToDevice, h->stream));
-    TRY(matvec_impl(h, h->xh, h->yh, nullptr));
+    TRY(matvec_run(h, h->xh, h->yh));
     CUDA_TRY(cudaMemcpyAsync(y_host, h->yh, bytes, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     return PYGBE_OK;
@@ -186,6 +189,7 @@ extern "C" int pygbe_stats(const pygbe_handle *h, pygbe_stats_t *s)
     }
     s->device_bytes = (int64_t)h->mem.bytes;
     s->workspace_high_water = (int64_t)h->mem.high_water;
+    s->graph_launches = h->graph_launches;
     s->n_matvec = h->n_matvec; s->kernels_per_matvec = h->kernels_per_matvec; s->kernel_launches = h->launches;
     s->create_ms = h->create_ms; s->last_solve_ms = h->last_solve_ms; s->last_iters = h->last_iters;
     s->P = h->P; s->K = h->K; s->precision = h->precision; s->theta = h->theta;

@@ -87,6 +87,7 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
     }
     CUDA_TRY(cudaMemsetAsync(G.h1, 0, (size_t)(G.m + 2) * sizeof(double), st));   // k_gm_arnoldi keeps h1 zero between steps
     const bool pc = h->precond == 1 && h->pinv != nullptr;
+    TRY(set_slots(h, 2, G.V, G.w));                                 // input base and output of the iteration's matvec
     // Cycle = [residual b - A x by a matvec, convergence test on it] + up to m Arnoldi steps + update of x.  A cycle
     // ends early when the Arnoldi estimate reaches tol; convergence is declared only by the next cycle's recomputed
     // residual (one extra matvec per solve).  If that residual is above tol the iteration simply goes on; after
@@ -98,7 +99,7 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
         if (!first) {
             CUDA_TRY(cudaMemsetAsync(G.flags, 0, sizeof(int), st));             // clear "stop", keep the counters
             CUDA_TRY(cudaMemsetAsync(G.scal + 3, 0, sizeof(double), st));
-            TRY(matvec_impl(h, x_dev, G.w, nullptr));
+            TRY(matvec_run(h, x_dev, G.w));
         }
         LAUNCH(h, k_gm_residual, gridn, GM_THREADS, 0, G.flags, n, G.b, G.w, first ? 0 : 1, G.V, G.scal);
         LAUNCH(h, k_gm_begin, 1, 1, 0, G.flags, G.scal, G.g, G.m, first ? 1 : 0, tol);
@@ -112,32 +113,45 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
             if (mc <= 0) break;                           // out of iterations
         }
         first = false;
-        for (int j = 0; j < mc; j++) {
-            double *vj = G.V + (size_t)j * n;
+        // One Arnoldi step = [M^-1 v_j] + matvec + one cooperative launch (CGS2, normalisation, Givens, convergence
+        // estimate; gmres.cuh).  The step number lives on the device (flags[1]), so the same launches serve every
+        // step: `poll` of them are captured once as a CUDA graph and replayed; the host reads the flags in between.
+        auto one_step = [&]() -> int {
             if (pc) {           // right preconditioning: w = A (M^-1 v_j)
-                LAUNCH(h, k_precond_apply, cdiv(h->npan, GM_THREADS), GM_THREADS, 0, G.flags, 1, h->npan, h->pinv, h->pidx, vj, 0, h->zbuf);
-                TRY(matvec_impl(h, h->zbuf, G.w, G.flags));
+                LAUNCH(h, k_precond_apply, cdiv(h->npan, GM_THREADS), GM_THREADS, 0, G.flags, 1, h->npan, h->pinv, h->pidx,
+                       vec_slot(h->io + 2, G.flags + 1, n), 0, h->zbuf);
+                TRY(matvec_impl(h, vec_direct(h->zbuf), vec_slot(h->io + 3), G.flags));
             } else {
-                TRY(matvec_impl(h, vj, G.w, G.flags));
+                TRY(matvec_impl(h, vec_slot(h->io + 2, G.flags + 1, n), vec_slot(h->io + 3), G.flags));
             }
-            {   // one cooperative launch: CGS2, normalisation, Givens, convergence estimate (gmres.cuh)
-                long nn = n; int jj = j, mm = G.m; double tl = tol;
-                double *nrm2 = G.scal + 3;
-                void *args[] = {&G.flags, &G.V, &nn, &jj, &mm, &G.w, &G.h1, &G.h2, &nrm2, &G.H, &G.cs, &G.sn, &G.g, &G.scal, &tl};
-                CUDA_TRY(cudaLaunchCooperativeKernel((const void *)k_gm_arnoldi, dim3(arn_grid), dim3(GM_THREADS), args, 0, st));
-                h->launches++;
+            long nn = n; int mm = G.m; double tl = tol;
+            double *nrm2 = G.scal + 3;
+            void *args[] = {&G.flags, &G.V, &nn, &mm, &G.w, &G.h1, &G.h2, &nrm2, &G.H, &G.cs, &G.sn, &G.g, &G.scal, &tl};
+            CUDA_TRY(cudaLaunchCooperativeKernel((const void *)k_gm_arnoldi, dim3(arn_grid), dim3(GM_THREADS), args, 0, h->stream));
+            h->launches++;
+            return PYGBE_OK;
+        };
+        bool graph = h->use_graphs && !h->profile && !h->g_iter.failed;
+        if (graph) {
+            long tolbits; memcpy(&tolbits, &tol, sizeof(tolbits));
+            const long key[6] = {(long)(uintptr_t)G.V, (long)G.m, tolbits, (long)poll, (long)pc, (long)arn_grid};
+            if (!h->g_iter.exec || memcmp(key, h->g_iter.key, sizeof(key)) != 0) {
+                graph = graph_capture(h, h->g_iter, [&]() -> int { for (int q = 0; q < poll; q++) TRY(one_step()); return PYGBE_OK; });
+                if (graph) memcpy(h->g_iter.key, key, sizeof(key));
             }
-            if ((j + 1) % poll == 0 || j + 1 == mc) {
-                CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
-                CUDA_TRY(cudaStreamSynchronize(st));
-                if (h->pinned_flags[0]) break;
-            }
+        }
+        for (int j = 0; j < mc;) {
+            if (graph && j + poll <= mc) { TRY(graph_launch(h, h->g_iter)); j += poll; }
+            else { TRY(one_step()); j++; if (j % poll != 0 && j != mc) continue; }
+            CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            if (h->pinned_flags[0]) break;
         }
         LAUNCH(h, k_gm_solve_small, 1, 1, 0, G.flags, G.m, G.H, G.g, G.yk);
         if (pc) {               // x += M^-1 (V y)
             CUDA_TRY(cudaMemsetAsync(h->zbuf, 0, n * sizeof(double), st));
             LAUNCH(h, k_gm_update, gridn, GM_THREADS, 0, G.flags, n, G.V, G.yk, h->zbuf);
-            LAUNCH(h, k_precond_apply, cdiv(h->npan, GM_THREADS), GM_THREADS, 0, G.flags, 0, h->npan, h->pinv, h->pidx, h->zbuf, 1, x_dev);
+            LAUNCH(h, k_precond_apply, cdiv(h->npan, GM_THREADS), GM_THREADS, 0, G.flags, 0, h->npan, h->pinv, h->pidx, vec_direct(h->zbuf), 1, x_dev);
         } else {
             LAUNCH(h, k_gm_update, gridn, GM_THREADS, 0, G.flags, n, G.V, G.yk, x_dev);
         }
@@ -149,7 +163,7 @@ extern "C" int pygbe_solve(pygbe_handle *h, double tol, int32_t restart, int32_t
         if (h->pinned_flags[0] && ++disagreements > 3) {                        // the estimate keeps saying "done", the residual does not
             CUDA_TRY(cudaMemsetAsync(G.flags, 0, sizeof(int), st));
             CUDA_TRY(cudaMemsetAsync(G.scal + 3, 0, sizeof(double), st));
-            TRY(matvec_impl(h, x_dev, G.w, nullptr));
+            TRY(matvec_run(h, x_dev, G.w));
             LAUNCH(h, k_gm_residual, gridn, GM_THREADS, 0, G.flags, n, G.b, G.w, 1, G.V, G.scal);
             LAUNCH(h, k_gm_begin, 1, 1, 0, G.flags, G.scal, G.g, G.m, 0, tol);
             CUDA_TRY(cudaMemcpyAsync(h->pinned_flags, G.flags, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -181,7 +195,7 @@ extern "C" int pygbe_reaction_potential(pygbe_handle *h, const double *x_dev, do
     CUDA_TRY(cudaMemsetAsync(phi_dev, 0, h->nq * sizeof(double), h->stream));
     for (Region &R : h->regions) {
         if (R.nq == 0) continue;
-        LAUNCH(h, k_prep, cdiv((long)R.np * h->K, 256), 256, 0, nullptr, R.np, h->K, x_dev, R.phi_idx, R.dphi_idx, R.cV, R.cK, R.pnrm,
+        LAUNCH(h, k_prep, cdiv((long)R.np * h->K, 256), 256, 0, nullptr, R.np, h->K, vec_direct(x_dev), R.phi_idx, R.dphi_idx, R.cV, R.cK, R.pnrm,
                R.spos, R.schg, (float4 *)nullptr, 0, R.pphi, R.pdphi, R.pq, R.out, (double *)nullptr);
         // chunks of Gauss points on grid.y: at most 65535 of them
         const long en_chunks = cdiv(R.npts, EN_CHUNK);
