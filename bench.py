@@ -457,8 +457,20 @@ def main():
     ap.add_argument("--precision", default="mixed", choices=["fp64", "mixed"])
     ap.add_argument("--seconds", type=float, default=0.0, help="reference arm: CPU seconds per step (default 60 / steps)")
     ap.add_argument("--sweep", action="store_true", help="one JSON line per configuration and precision (rank 0, one GPU)")
+    ap.add_argument("--probe-mma", action="store_true", help="tensor-core M2P probe (pygbe_mma_probe), P = 6 and 8; one JSON line")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.probe_mma:
+        import paper_1309_4018_b200 as pg
+        res = {}
+        for P in (6, 8):
+            r = pg.mma_probe(P)
+            base = r["cuda_core_k_m2p_single2"]["ms"]
+            for v in r.values():
+                v["ns_per_group_cell"] = 1e6 * v["ms"] / v["pairs"]
+                v["time_vs_cuda_core"] = v["ms"] / base
+            res["P=%d" % P] = r
+        print(json.dumps({"probe": "m2p_mma", "data": "synthetic far field: 8192 groups x 32 cells, Yukawa kappa = 0.125, single set", **res}))
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -243,6 +243,15 @@ const char *pygbe_last_error(void);
  * recurrence-like instruction mix of M2P / P2P; FMA = 2 flops, MUL = 1).  out4: HOST, 4 doubles. */
 int pygbe_alu_peaks(int32_t device, double *out4);
 
+/* The north star's tensor-core question, measured (csrc/mma_probe.cuh; not on the product path): per (64-target
+ * group, cell) the regrouped M2P is the product [64 x Nc] * [Nc x (P+1)] with a target-specific left operand.  On
+ * synthetic far-field data (8192 groups x 32 cells, Yukawa, single moment set) it times and checks against fp64
+ * direct sums four variants v = 0..3: the production CUDA-core kernel; only the write of the monomial tile to shared
+ * memory that any tensor-core form needs first; tile + TF32 tensor-core contraction (mma.sync m16n8k8) + radial part
+ * in one pass; the same with the 3 x TF32 split.  out12[3 v] = ms per launch, out12[3 v + 1] = rel-L2 error (NaN for
+ * the tile-only variant), out12[3 v + 2] = (group, cell) pairs per launch.  P = 6 or 8.  out12: HOST.  Synchronous. */
+int pygbe_mma_probe(int32_t device, int32_t P, double *out12);
+
 /* Library / build identification, e.g. "pygbe-b200 0.3 sm_100a". */
 const char *pygbe_version(void);
 

@@ -319,5 +319,16 @@ def alu_peaks(device=0):
     return dict(fp32_tflops=out[0], fp64_tflops=out[1], mufu_gops=out[2], fp32_mix_tflops=out[3])
 
 
+def mma_probe(P=8, device=0):
+    """pygbe_mma_probe: {variant: dict(ms, rel_l2, pairs)} for the CUDA-core M2P, the monomial-tile write alone and the
+    TF32 tensor-core contraction in one pass and with the 3 x TF32 split (csrc/mma_probe.cuh)."""
+    L = lib()
+    L.pygbe_mma_probe.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double)]
+    out = (C.c_double * 12)()
+    _check(L.pygbe_mma_probe(device, P, out))
+    names = ("cuda_core_k_m2p_single2", "monomial_tile_to_smem_only", "tile_plus_tf32_mma_1pass", "tile_plus_tf32_mma_3xsplit")
+    return {n: dict(ms=out[3 * i], rel_l2=out[3 * i + 1], pairs=out[3 * i + 2]) for i, n in enumerate(names)}
+
+
 def pygbe_version():
     return lib().pygbe_version().decode()

@@ -69,9 +69,9 @@ static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<do
     TRY(build_corrections(h, R, qt, nullptr));
     dbg_t("corrections");
     if (R.n_m2p_items > 0) {
-        TRY(h->mem.alloc(&R.mom, (size_t)R.ncells * 2 * h->Nc));
+        TRY(h->mem.alloc_big(&R.mom, (size_t)R.ncells * 2 * h->Nc));
         const bool f32 = h->precision == PYGBE_PRECISION_MIXED;
-        if (f32) TRY(h->mem.alloc(&R.pmomf, (size_t)R.np * 2 * h->Nc)); else TRY(h->mem.alloc(&R.pmom, (size_t)R.np * 2 * h->Nc));
+        if (f32) TRY(h->mem.alloc_big(&R.pmomf, (size_t)R.np * 2 * h->Nc)); else TRY(h->mem.alloc_big(&R.pmom, (size_t)R.np * 2 * h->Nc));
         if (R.n_p2m > 0 && !h->dry) {
             if (f32) LAUNCH(h, k_panel_moments<float>, R.n_p2m, PMOM_THREADS, 0, h->P, h->Nc, h->K, h->itab, R.p2m_cells, R.cgeo, R.crange,
                             R.spos, R.pnrm, R.pmomf);

@@ -68,7 +68,7 @@ static int build_corrections(pygbe_handle *h, Region &R, const QuadTables &qt, c
         CUDA_TRY(cudaStreamSynchronize(h->stream));
         h->mem.release_one(d_cnt);
     }
-    TRY(h->mem.alloc(&R.corr_val, R.corr_nnz));
+    TRY(h->mem.alloc_big(&R.corr_val, R.corr_nnz));
     if (!h->dry) LAUNCH(h, k_near_values, cdiv((long)R.np * 32, 128), 128, 0, R.np, qt, R.yukawa, R.kappa, R.corr_off, R.corr_col, R.gid, h->tri,
            R.tpos, R.pnrm, R.spos, R.cV, R.cK, R.corr_val);
     CUDA_TRY(cudaStreamSynchronize(h->stream));

@@ -107,6 +107,23 @@ struct DeviceArena {
         }
         if (!holes.empty() && holes.back().first + holes.back().second == top) { top = holes.back().first; holes.pop_back(); }
     }
+    bool dry = false;                           // size query: alloc_big only books the space
+    // The large arrays that no sizing step reads (panel moments, multipoles, correction values, Krylov basis): in a
+    // size query they are only booked, not allocated -- the dry run of the 1.08 M-panel complex then touches 1.5 GB
+    // instead of 8 GB.  The pointer returned in that case is a placeholder that must not be dereferenced.
+    template <class T> int alloc_big(T **p, size_t n)
+    {
+        if (!dry) return alloc(p, n);
+        if (n == 0) n = 1;
+        const size_t sz = round_up(n * sizeof(T));
+        const size_t off = place(sz);
+        void *q = (void *)(((uintptr_t)1 << 48) + off);
+        used.push_back({off, sz, q});
+        bytes += sz;
+        *p = (T *)q;
+        return PYGBE_OK;
+    }
+    static bool placeholder(const void *q) { return ((uintptr_t)q >> 48) == 1; }
     template <class T> int alloc(T **p, size_t n)
     {
         *p = nullptr;
@@ -139,7 +156,7 @@ struct DeviceArena {
         if (!q) return;
         for (size_t i = 0; i < used.size(); i++)
             if (used[i].ptr == q) {
-                if (!base) cudaFreeAsync(q, stream);
+                if (!base && !placeholder(q)) cudaFreeAsync(q, stream);
                 bytes -= used[i].size;
                 unplace(used[i].off, used[i].size);
                 used.erase(used.begin() + i);
@@ -148,7 +165,7 @@ struct DeviceArena {
     }
     void release()
     {
-        if (!base) for (const Block &b : used) cudaFreeAsync(b.ptr, stream);
+        if (!base) for (const Block &b : used) if (!placeholder(b.ptr)) cudaFreeAsync(b.ptr, stream);
         used.clear(); holes.clear();
         top = 0; bytes = 0;
     }

@@ -9,6 +9,7 @@
 #include "matvec.cuh"
 #include "solve.cuh"
 #include "microbench.cuh"
+#include "mma_probe.cuh"
 
 static thread_local char g_err[1024] = "";
 
@@ -200,4 +201,13 @@ extern "C" int pygbe_alu_peaks(int32_t device, double *out4)
 {
     if (!out4) { pygbe_set_error("alu_peaks: null pointer"); return PYGBE_EINVAL; }
     return run_alu_peaks(device, out4);
+}
+
+extern "C" int pygbe_mma_probe(int32_t device, int32_t P, double *out12)
+{
+    if (!out12) { pygbe_set_error("mma_probe: null pointer"); return PYGBE_EINVAL; }
+    if (P == 6) return run_mma_probe_p<6>(device, out12);
+    if (P == 8) return run_mma_probe_p<8>(device, out12);
+    pygbe_set_error("mma_probe: P = %d (instantiated for 6 and 8)", P);
+    return PYGBE_EINVAL;
 }

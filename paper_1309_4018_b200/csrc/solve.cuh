@@ -5,15 +5,15 @@
 
 static int ensure_host_staging(pygbe_handle *h)
 {
-    if (!h->xh) { TRY(h->mem.alloc(&h->xh, 2 * h->npan)); TRY(h->mem.alloc(&h->yh, 2 * h->npan)); }
+    if (!h->xh) { TRY(h->mem.alloc_big(&h->xh, 2 * h->npan)); TRY(h->mem.alloc_big(&h->yh, 2 * h->npan)); }
     return PYGBE_OK;
 }
 
 static int ensure_energy_scratch(pygbe_handle *h)
 {
     if (!h->dq && h->nq > 0) {
-        TRY(h->mem.alloc(&h->dq, h->nq));
-        CUDA_TRY(cudaMemcpyAsync(h->dq, h->qq.data(), h->nq * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+        TRY(h->mem.alloc_big(&h->dq, h->nq));
+        if (!h->dry) CUDA_TRY(cudaMemcpyAsync(h->dq, h->qq.data(), h->nq * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     }
     return PYGBE_OK;
 }
@@ -48,12 +48,12 @@ static int ensure_gmres(pygbe_handle *h, int m)
             h->mem.release_one(q);
     }
     G.m = m; G.n = n;
-    TRY(h->mem.alloc(&G.V, (size_t)(m + 1) * n));
+    TRY(h->mem.alloc_big(&G.V, (size_t)(m + 1) * n));
     TRY(h->mem.alloc(&G.H, (size_t)(m + 1) * m));
     TRY(h->mem.alloc(&G.h1, m + 2)); TRY(h->mem.alloc(&G.h2, m + 2)); TRY(h->mem.alloc(&G.cs, m + 1));
     TRY(h->mem.alloc(&G.sn, m + 1)); TRY(h->mem.alloc(&G.g, m + 2)); TRY(h->mem.alloc(&G.yk, m + 1));
     if (!G.w) {
-        TRY(h->mem.alloc(&G.w, n)); TRY(h->mem.alloc(&G.b, n)); TRY(h->mem.alloc(&G.scal, 8)); TRY(h->mem.alloc(&G.flags, 4));
+        TRY(h->mem.alloc_big(&G.w, n)); TRY(h->mem.alloc_big(&G.b, n)); TRY(h->mem.alloc(&G.scal, 8)); TRY(h->mem.alloc(&G.flags, 4));
     }
     return PYGBE_OK;
 }
