@@ -124,6 +124,25 @@ def launch_flops(rec, P, kappa):
     return 0
 
 
+def profiled_traffic(config, precision, kernel, region):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on `region`, from the newest
+    profiles/*_traffic.json (written from an `ncu --set full` capture of this command; the file names the capture and
+    the commit it was taken at).  None if there is no record for this configuration: the run itself measures no DRAM
+    counters."""
+    import glob
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.json")), reverse=True):
+        try:
+            rec = json.load(open(path))
+        except Exception:
+            continue
+        if rec.get("config") != config or rec.get("precision") != precision:
+            continue
+        for k in rec.get("kernels", []):
+            if k["kernel"] == kernel and k["region"] == region:
+                return k["dram_bytes"], "%s (%s)" % (os.path.basename(path), rec.get("source", ""))
+    return None, None
+
+
 def clocks_sampler(stop, out):
     q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
     while not stop.is_set():
@@ -376,13 +395,15 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full, bri
                 gbs = r["bytes"] / (per_ms * 1e-3) / 1e9 if per_ms > 0 else 0.0
                 passes.append({**base, "bytes_per_launch": r["bytes"], "gbs": gbs, "frac_of_hbm_peak": gbs / hbm_peak})
         dom = max(kernels, key=lambda k: k["ms_per_launch"])
+        traffic, traffic_source = profiled_traffic(args.config, precision_name, dom["kernel"].replace("<P", "<%d" % kw["P"]), dom["region"])
         roofline = {"bound": "alu", "kernel": "%s, region %d%s, 1 launch/matvec" % (
                         dom["kernel"].replace("<P", "<%d" % kw["P"]), dom["region"],
                         (" + twin %d" % dom["twin_region"]) if dom["twin_region"] >= 0 else ""),
                     "achieved": dom["tflops"], "peak": nominal[dt], "unit": "TFLOP/s", "frac": dom["frac"],
                     "peak_kind": "derived: 148 SM x %d lanes x 2 x %.0f MHz (DESIGN.md 7); FMA micro-benchmark in this run: %.1f TFLOP/s"
                                  % (64 if dt == "f64" else 128, sm_max, peaks["fp64_tflops" if dt == "f64" else "fp32_tflops"]),
-                    "traffic": None, "ms_per_launch": dom["ms_per_launch"], "flops_per_launch": dom["flops_per_launch"],
+                    "traffic": traffic, "traffic_source": traffic_source,
+                    "ms_per_launch": dom["ms_per_launch"], "flops_per_launch": dom["flops_per_launch"],
                     "units_per_launch": dom["units_per_launch"],
                     "flop_model": "DESIGN.md 7 'Flop model' (bench.py launch_flops)", "stage_ms": stage_ms,
                     "alu_peaks_measured": peaks, "hbm_peak_gbs": hbm_peak}
