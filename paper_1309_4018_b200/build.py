@@ -16,7 +16,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpygbe.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+         "-Xcompiler", "-fPIC", "-Xcompiler", "-fopenmp", "-Xptxas", "-v"]      # OpenMP: host loops of create only
 FLAGS += os.environ.get("PYGBE_CFLAGS", "").split()      # e.g. -DPYGBE_TG=64 for tuning experiments
 PMAX = 12
 
@@ -66,7 +66,7 @@ def build(force=False, verbose=False):
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         objs = [o for o, _ in ex.map(_compile, jobs)]
     if (not os.path.exists(LIB)) or os.path.getmtime(LIB) < max(os.path.getmtime(o) for o in objs):
-        cmd = [NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs
+        cmd = [NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-Xcompiler", "-fopenmp", "-o", LIB] + objs
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("link failed: %s\n%s" % (" ".join(cmd), r.stderr[-4000:]))

@@ -162,35 +162,45 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
         h->mem.release_one(q);
 
     dbg_t("  anchors, groups, traversal");
-    // ---- P2P lists: leaves -> panel ranges sorted by position; adjacent ranges with the same anchor merge
-    std::vector<int4> prng;               // merged ranges, CSR by group
-    prng.reserve(pleaf.size());
-    std::vector<int> poff2(R.ng + 1, 0);
-    long total_src_panels = 0;
-    R.p2p_pairs = 0;
-    std::vector<int4> tmp;
-    for (int g = 0; g < R.ng; g++) {
-        tmp.clear();
-        for (int r = poff[g]; r < poff[g + 1]; r++) {
-            int c = pleaf[r];
-            tmp.push_back(make_int4(crange_h[c].x, crange_h[c].y, anchor_of[c], 0));
+    // ---- P2P lists: leaves -> panel ranges sorted by position; adjacent ranges with the same anchor merge.
+    // Host work over ~17 k groups x ~30 leaves at 1 M panels: every group is independent, so the loops run in
+    // parallel (OpenMP) into per-group slots and are compacted by prefix sums; the result does not depend on the
+    // number of threads.
+    const int ng = R.ng;
+    const bool par = R.np > 20000;
+    std::vector<int4> prng_raw((size_t)poff[ng]);       // merged ranges of group g at [poff[g], poff[g] + rcnt[g])
+    std::vector<int> rcnt(ng, 0);
+    long total_src_panels = 0, p2p_pairs = 0, m2p_evals = 0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : total_src_panels, p2p_pairs, m2p_evals) if (par)
+    for (int g = 0; g < ng; g++) {
+        int4 *dst = prng_raw.data() + poff[g];
+        const int nl = poff[g + 1] - poff[g];
+        for (int r = 0; r < nl; r++) {
+            const int c = pleaf[poff[g] + r];
+            dst[r] = make_int4(crange_h[c].x, crange_h[c].y, anchor_of[c], 0);
         }
         // the traversal emits a group's leaves in Morton order, i.e. by ascending panel range: sort only if not
         auto by_pos = [](const int4 &a, const int4 &b) { return a.x < b.x; };
-        if (!std::is_sorted(tmp.begin(), tmp.end(), by_pos)) std::sort(tmp.begin(), tmp.end(), by_pos);
-        size_t start = prng.size();
-        for (const int4 &e : tmp) {
-            if (prng.size() > start && prng.back().y == e.x && prng.back().z == e.z) prng.back().y = e.y;
-            else prng.push_back(e);
+        if (!std::is_sorted(dst, dst + nl, by_pos)) std::sort(dst, dst + nl, by_pos);
+        int n = 0;
+        for (int r = 0; r < nl; r++) {
+            if (n > 0 && dst[n - 1].y == dst[r].x && dst[n - 1].z == dst[r].z) dst[n - 1].y = dst[r].y;
+            else dst[n++] = dst[r];
         }
-        poff2[g + 1] = (int)prng.size();
-        long ntg = std::min(PYGBE_TG, R.np - g * PYGBE_TG), src = 0;
-        for (size_t r = start; r < prng.size(); r++) src += prng[r].y - prng[r].x;
+        rcnt[g] = n;
+        const long ntg = std::min(PYGBE_TG, R.np - g * PYGBE_TG);
+        long src = 0;
+        for (int r = 0; r < n; r++) src += dst[r].y - dst[r].x;
         total_src_panels += src;
-        R.p2p_pairs += ntg * src * K;
+        p2p_pairs += ntg * src * K;
+        m2p_evals += ntg * mcnt[g];
     }
-    R.m2p_evals = 0;
-    for (int g = 0; g < R.ng; g++) R.m2p_evals += (long)std::min(PYGBE_TG, R.np - g * PYGBE_TG) * mcnt[g];
+    R.p2p_pairs = p2p_pairs; R.m2p_evals = m2p_evals;
+    std::vector<int> poff2(ng + 1, 0);
+    for (int g = 0; g < ng; g++) poff2[g + 1] = poff2[g] + rcnt[g];
+    std::vector<int4> prng((size_t)poff2[ng]);           // merged ranges, CSR by group
+#pragma omp parallel for schedule(static) if (par)
+    for (int g = 0; g < ng; g++) std::copy(prng_raw.begin() + poff[g], prng_raw.begin() + poff[g] + rcnt[g], prng.begin() + poff2[g]);
     TRY(upload(h, &R.p2p_off, poff2)); TRY(upload(h, &R.p2p_rng, prng));
 
     dbg_t("  P2P ranges (host)");
@@ -198,8 +208,8 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     const long want_items = 148L * 16;
     // M2P CTAs keep only 8-20 warps per SM resident (72-127 registers): finer items even out the tail (config 1:
     // 4 cells per item 0.057 ms, 8 cells 0.060, 16 cells 0.068)
-    int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[R.ng] / (6 * want_items)));
-    if (R.lap) m2p_item = std::max(m2p_item, 12);            // k_m2p_lap stages 12 cells at a time
+    int m2p_item = (int)std::min(64L, std::max(4L, (long)moff[ng] / (6 * want_items)));
+    if (R.lap) m2p_item = std::max(m2p_item, 12);            // k_m2p_lap stages up to 12 cells at a time
     m2p_item = (m2p_item + 3) / 4 * 4;
     if (const char *e = tune_env("PYGBE_M2P_ITEM")) m2p_item = std::max(1, atoi(e));                 // tuning
     // P2P tiles gather up to P2P_TILE source points from several panel ranges of one anchor cell: a group's near
@@ -209,55 +219,75 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     // tile holds panels of the group's own targets, the only place where a pair at zero distance can occur
     // (reading A5).
     const int tile_panels = std::max(1, P2P_TILE / K);
-    std::vector<int4> sub, pitems, mitems;
-    std::vector<int> gtile(R.ng + 1, 0);                           // first tile of each group
-    std::vector<int2> segs;
-    sub.reserve(total_src_panels / tile_panels + prng.size()); segs.reserve(total_src_panels / tile_panels + 2 * prng.size());
-    mitems.reserve((size_t)moff[R.ng] / m2p_item + R.ng);
-    std::vector<int4> grng;
-    for (int g = 0; g < R.ng; g++) {
-        grng.assign(prng.begin() + poff2[g], prng.begin() + poff2[g + 1]);
-        std::stable_sort(grng.begin(), grng.end(), [](const int4 &a, const int4 &b) { return a.z < b.z; });
-        const int own_lo = g * PYGBE_TG, own_hi = std::min(R.np, own_lo + PYGBE_TG);
-        const size_t tile0 = sub.size();
-        long src = 0;
-        int fill = 0;                                              // panels in the open tile (sub.back())
-        for (size_t r = 0; r < grng.size(); r++) {
-            if (r > 0 && grng[r].z != grng[r - 1].z) fill = 0;     // another anchor: close the tile
-            int a = grng[r].x;
-            while (a < grng[r].y) {
-                if (fill == 0 || fill == tile_panels) {
-                    sub.push_back(make_int4((int)segs.size(), (int)segs.size(), grng[r].z, 0));
-                    fill = 0;
+    // pass 1 (parallel): tiles and segments of every group with group-local segment indices
+    std::vector<std::vector<int4>> gsub(ng);
+    std::vector<std::vector<int2>> gseg(ng);
+#pragma omp parallel if (par)
+    {
+        std::vector<int4> grng;
+#pragma omp for schedule(dynamic, 64)
+        for (int g = 0; g < ng; g++) {
+            grng.assign(prng.begin() + poff2[g], prng.begin() + poff2[g + 1]);
+            std::stable_sort(grng.begin(), grng.end(), [](const int4 &a, const int4 &b) { return a.z < b.z; });
+            const int own_lo = g * PYGBE_TG, own_hi = std::min(R.np, own_lo + PYGBE_TG);
+            std::vector<int4> &sub = gsub[g];
+            std::vector<int2> &segs = gseg[g];
+            int fill = 0;                                              // panels in the open tile (sub.back())
+            for (size_t r = 0; r < grng.size(); r++) {
+                if (r > 0 && grng[r].z != grng[r - 1].z) fill = 0;     // another anchor: close the tile
+                int a = grng[r].x;
+                while (a < grng[r].y) {
+                    if (fill == 0 || fill == tile_panels) {
+                        sub.push_back(make_int4((int)segs.size(), (int)segs.size(), grng[r].z, 0));
+                        fill = 0;
+                    }
+                    const int take = std::min(grng[r].y - a, tile_panels - fill);
+                    segs.push_back(make_int2(a * K, take * K));
+                    int4 &t = sub.back();
+                    t.y = (int)segs.size();
+                    t.w += 2 * take * K;
+                    if (a < own_hi && a + take > own_lo) t.w |= 1;
+                    a += take; fill += take;
                 }
-                const int take = std::min(grng[r].y - a, tile_panels - fill);
-                segs.push_back(make_int2(a * K, take * K));
-                int4 &t = sub.back();
-                t.y = (int)segs.size();
-                t.w += 2 * take * K;
-                if (a < own_hi && a + take > own_lo) t.w |= 1;
-                a += take; fill += take; src += take;
             }
         }
-        gtile[g + 1] = (int)sub.size();
-        for (int s = moff[g]; s < moff[g + 1]; s += m2p_item)
-            mitems.push_back(make_int4(g, s, std::min(s + m2p_item, moff[g + 1]), 0));
+    }
+    std::vector<int> gtile(ng + 1, 0), gsegoff(ng + 1, 0), gmit(ng + 1, 0);   // first tile / segment / M2P item of each group
+    for (int g = 0; g < ng; g++) {
+        gtile[g + 1] = gtile[g] + (int)gsub[g].size();
+        gsegoff[g + 1] = gsegoff[g] + (int)gseg[g].size();
+        gmit[g + 1] = gmit[g] + (moff[g + 1] - moff[g] + m2p_item - 1) / m2p_item;
     }
     // items = short runs of a group's tiles.  An SM holds ~12 of these CTAs, which share its pipes, so an item of n
     // tiles lasts about n / 1100 of the whole launch at config 1 (13 k tiles): equal items of 5 tiles left a tail
     // of a fifth of the kernel, single tiles none (the double buffer then only hides the first tile's latency
     // behind other CTAs).  Large problems take longer runs to save the per-item target loads and atomics.
-    {
-        const long slots = 148L * 12;
-        int per_item = (int)std::min(8L, std::max(1L, (long)sub.size() / (slots * 24)));
-        if (const char *e = tune_env("PYGBE_P2P_ITEM_TILES")) per_item = std::max(1, atoi(e));      // tuning
-        for (int g = 0; g < R.ng; g++)
-            for (int t = gtile[g]; t < gtile[g + 1]; t += per_item) {
-                const int n = std::min(per_item, gtile[g + 1] - t);
-                int acc = 0;
-                for (int u = 0; u < n; u++) acc += (sub[t + u].w >> 1) / K;
-                pitems.push_back(make_int4(g, t, t + n, acc));
-            }
+    const long slots = 148L * 12;
+    int per_item = (int)std::min(8L, std::max(1L, (long)gtile[ng] / (slots * 24)));
+    if (const char *e = tune_env("PYGBE_P2P_ITEM_TILES")) per_item = std::max(1, atoi(e));      // tuning
+    std::vector<int> gpit(ng + 1, 0);
+    for (int g = 0; g < ng; g++) gpit[g + 1] = gpit[g] + ((int)gsub[g].size() + per_item - 1) / per_item;
+    // pass 2 (parallel): concatenate with global indices
+    std::vector<int4> sub((size_t)gtile[ng]), pitems((size_t)gpit[ng]), mitems((size_t)gmit[ng]);
+    std::vector<int2> segs((size_t)gsegoff[ng]);
+#pragma omp parallel for schedule(static) if (par)
+    for (int g = 0; g < ng; g++) {
+        const int nt = (int)gsub[g].size();
+        for (int t = 0; t < nt; t++) {
+            int4 v = gsub[g][t];
+            v.x += gsegoff[g]; v.y += gsegoff[g];
+            sub[gtile[g] + t] = v;
+        }
+        std::copy(gseg[g].begin(), gseg[g].end(), segs.begin() + gsegoff[g]);
+        int at = gpit[g];
+        for (int t = 0; t < nt; t += per_item) {
+            const int n = std::min(per_item, nt - t);
+            int acc = 0;
+            for (int u = 0; u < n; u++) acc += (gsub[g][t + u].w >> 1) / K;
+            pitems[at++] = make_int4(g, gtile[g] + t, gtile[g] + t + n, acc);
+        }
+        at = gmit[g];
+        for (int q = moff[g]; q < moff[g + 1]; q += m2p_item) mitems[at++] = make_int4(g, q, std::min(q + m2p_item, moff[g + 1]), 0);
     }
     if (tune_env("PYGBE_DEBUG")) {
         long pts = 0, selft = 0; int hist[9] = {0};
@@ -266,13 +296,6 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
                 R.ng, prng.size(), pitems.size(), sub.size(), (double)pts / (sub.size() * (double)P2P_TILE), selft);
         for (int i = 0; i < 9; i++) fprintf(stderr, " %d", hist[i]);
         fprintf(stderr, "\n");
-        int tmin = 1 << 30, tmax = 0, over15 = 0;
-        const double tavg = (double)sub.size() / std::max(1, R.ng);
-        for (int g = 0; g < R.ng; g++) {
-            const int nt = gtile[g + 1] - gtile[g];
-            tmin = std::min(tmin, nt); tmax = std::max(tmax, nt); over15 += nt > 1.5 * tavg;
-        }
-        fprintf(stderr, "[pygbe] tiles per group: min %d avg %.1f max %d, %d of %d groups above 1.5 x avg\n", tmin, tavg, tmax, over15, R.ng);
     }
     dbg_t("  tiles + items (host)");
     R.n_p2p_items = (int)pitems.size(); R.n_m2p_items = (int)mitems.size();

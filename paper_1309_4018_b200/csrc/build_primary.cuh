@@ -14,16 +14,20 @@ static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<do
     // root cube around the centroids; longest panel (for the near-field guard of the traversal)
     double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
     double Lmax = 0.0;
-    for (int p = 0; p < R.np; p++) {
-        const double *t = tri_host.data() + 9 * (size_t)b.gid[p];
-        double ux = t[3] - t[0], uy = t[4] - t[1], uz = t[5] - t[2];
-        double vx = t[6] - t[0], vy = t[7] - t[1], vz = t[8] - t[2];
-        double cx = uy * vz - uz * vy, cy = uz * vx - ux * vz, cz = ux * vy - uy * vx;
-        Lmax = std::max(Lmax, std::sqrt(std::sqrt(cx * cx + cy * cy + cz * cz)));   // sqrt(2A), 2A = |cross|
-        for (int a = 0; a < 3; a++) {
-            double c = (t[a] + t[3 + a] + t[6 + a]) / 3.0;
-            lo[a] = std::min(lo[a], c); hi[a] = std::max(hi[a], c);
+    {
+        double l0 = 1e300, l1 = 1e300, l2 = 1e300, h0 = -1e300, h1 = -1e300, h2 = -1e300;      // min / max are order-independent
+#pragma omp parallel for schedule(static) reduction(min : l0, l1, l2) reduction(max : h0, h1, h2, Lmax) if (R.np > 20000)
+        for (int p = 0; p < R.np; p++) {
+            const double *t = tri_host.data() + 9 * (size_t)b.gid[p];
+            double ux = t[3] - t[0], uy = t[4] - t[1], uz = t[5] - t[2];
+            double vx = t[6] - t[0], vy = t[7] - t[1], vz = t[8] - t[2];
+            double cx = uy * vz - uz * vy, cy = uz * vx - ux * vz, cz = ux * vy - uy * vx;
+            Lmax = std::max(Lmax, std::sqrt(std::sqrt(cx * cx + cy * cy + cz * cz)));   // sqrt(2A), 2A = |cross|
+            const double c0 = (t[0] + t[3] + t[6]) / 3.0, c1 = (t[1] + t[4] + t[7]) / 3.0, c2 = (t[2] + t[5] + t[8]) / 3.0;
+            l0 = std::min(l0, c0); l1 = std::min(l1, c1); l2 = std::min(l2, c2);
+            h0 = std::max(h0, c0); h1 = std::max(h1, c1); h2 = std::max(h2, c2);
         }
+        lo[0] = l0; lo[1] = l1; lo[2] = l2; hi[0] = h0; hi[1] = h1; hi[2] = h2;
     }
     R.Lmax = Lmax;
     const double edge = std::max({hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2]}) * (1.0 + 1e-6) + 1e-9;

@@ -24,7 +24,8 @@ static void collect_boundary(const pygbe_handle *h, int id, Boundary &b)
     size_t total = 0;
     for (int s = 0; s < h->nsurf; s++)
         if (h->rin[s] == id || h->rout[s] == id) total += (size_t)h->surf_count[s];
-    b.gid.reserve(total); b.phi.reserve(total); b.dphi.reserve(total); b.row.reserve(total); b.cV.reserve(total); b.cK.reserve(total);
+    b.gid.resize(total); b.phi.resize(total); b.dphi.resize(total); b.row.resize(total); b.cV.resize(total); b.cK.resize(total);
+    size_t at = 0;
     for (int s = 0; s < h->nsurf; s++) {
         double sigma, c;
         int half;
@@ -32,15 +33,17 @@ static void collect_boundary(const pygbe_handle *h, int id, Boundary &b)
         else if (h->rout[s] == id) { sigma = -1.0; c = h->eps[h->rin[s]] / h->eps[h->rout[s]]; half = 1; }
         else continue;
         b.surfaces.push_back(s);
-        long o = h->surf_first[s], N = h->surf_count[s];
+        const long o = h->surf_first[s], N = h->surf_count[s];
+#pragma omp parallel for schedule(static) if (N > 20000)
         for (long j = 0; j < N; j++) {
-            b.gid.push_back((int)(o + j));
-            b.phi.push_back((int)(2 * o + j));
-            b.dphi.push_back((int)(2 * o + N + j));
-            b.row.push_back((int)(2 * o + half * N + j));
-            b.cV.push_back(sigma * c);
-            b.cK.push_back(sigma);
+            b.gid[at + j] = (int)(o + j);
+            b.phi[at + j] = (int)(2 * o + j);
+            b.dphi[at + j] = (int)(2 * o + N + j);
+            b.row[at + j] = (int)(2 * o + half * N + j);
+            b.cV[at + j] = sigma * c;
+            b.cK[at + j] = sigma;
         }
+        at += (size_t)N;
     }
 }
 
