@@ -411,6 +411,10 @@ def measure(args, precision_name, pg, torch, dist, world, rank, local, full, bri
             # context, not the denominator: what the FP32 pipe delivers on a register-resident FMUL + 3-register
             # FFMA mix (pygbe_alu_peaks out[3]), the practical ceiling of a mixed FMUL / FFMA stream
             roofline["frac_of_mix_ceiling"] = dom["tflops"] / peaks["fp32_mix_tflops"]
+        if dt == "f32" and "lap" in dom["kernel"] and peaks.get("fp32_horner_tflops"):
+            # what the bare Horner stream of this kernel (packed FFMA2, broadcast coefficient from shared memory) reaches
+            # on this machine, measured in this run (pygbe_alu_peaks out[4]): the ceiling of the kernel's pattern
+            roofline["frac_of_horner_ceiling"] = dom["tflops"] / peaks["fp32_horner_tflops"]
         # ---- time-to-solution (second half of the metric): create + rhs + GMRES + energy, host buffers.  The first
         # solve of a handle is reported apart on the small configs (warm-up of the cooperative launch); the large
         # ones run one solve

@@ -238,10 +238,12 @@ int pygbe_launch_times(pygbe_handle *h, pygbe_launch_info *out, int32_t max_out,
 const char *pygbe_last_error(void);
 
 /* ALU roofline denominators measured on `device` with dependent-FMA / MUFU micro-kernels (synchronous,
- * ~80 ms): out4[0] = fp32 FMA TFLOP/s, out4[1] = fp64 FMA TFLOP/s, out4[2] = MUFU.RSQ Gop/s, out4[3] = TFLOP/s
- * of an fp32 FMUL + three-register FFMA mix over 24 live registers (the practical ceiling of the
- * recurrence-like instruction mix of M2P / P2P; FMA = 2 flops, MUL = 1).  out4: HOST, 4 doubles. */
-int pygbe_alu_peaks(int32_t device, double *out4);
+ * ~100 ms): out5[0] = fp32 FMA TFLOP/s, out5[1] = fp64 FMA TFLOP/s, out5[2] = MUFU.RSQ Gop/s, out5[3] = TFLOP/s
+ * of an fp32 FMUL + three-register FFMA mix over 24 live registers (the practical ceiling of the instruction mix of the
+ * regrouped M2P / P2P; FMA = 2 flops, MUL = 1), out5[4] = TFLOP/s of the bare Horner stream of the Laplace-form M2P
+ * (packed FFMA2 with a broadcast coefficient from shared memory, P = 8: the ceiling of k_m2p_lap's pattern).
+ * out5: HOST, 5 doubles. */
+int pygbe_alu_peaks(int32_t device, double *out5);
 
 /* The north star's tensor-core question, measured (csrc/mma_probe.cuh; not on the product path): per (64-target
  * group, cell) the regrouped M2P is the product [64 x Nc] * [Nc x (P+1)] with a target-specific left operand.  On

@@ -311,12 +311,12 @@ def _workspace_size_of(p, gmres_restart, **kw):
 
 
 def alu_peaks(device=0):
-    """Measured ALU peaks of the device: dict(fp32_tflops, fp64_tflops, mufu_gops, fp32_mix_tflops)."""
+    """Measured ALU peaks of the device: dict(fp32_tflops, fp64_tflops, mufu_gops, fp32_mix_tflops, fp32_horner_tflops)."""
     L = lib()
     L.pygbe_alu_peaks.argtypes = [C.c_int32, C.POINTER(C.c_double)]
-    out = (C.c_double * 4)()
+    out = (C.c_double * 5)()
     _check(L.pygbe_alu_peaks(device, out))
-    return dict(fp32_tflops=out[0], fp64_tflops=out[1], mufu_gops=out[2], fp32_mix_tflops=out[3])
+    return dict(fp32_tflops=out[0], fp64_tflops=out[1], mufu_gops=out[2], fp32_mix_tflops=out[3], fp32_horner_tflops=out[4])
 
 
 def mma_probe(P=8, device=0):

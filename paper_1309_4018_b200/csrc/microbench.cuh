@@ -3,6 +3,7 @@
 // Dependent FMA chains, 8 per thread, enough warps to fill every SM; one MUFU.RSQ chain set for the SFU.
 #pragma once
 #include "common.cuh"
+#include "m2p.cuh"
 
 template <typename T>
 __global__ void __launch_bounds__(256) k_fma_peak(int iters, T a, T b, T *out)
@@ -52,6 +53,30 @@ __global__ void __launch_bounds__(128) k_mix_peak(int iters, float *out)
     if (s == -12345.f) out[0] = s;
 }
 
+// The instruction stream of the Laplace-form M2P with nothing around it: lap_poly<8, float> (164 Horner steps on four
+// targets = 328 FFMA2 with a scalar coefficient operand read from shared memory by broadcast LDS.128) on register-
+// resident arguments, no staging, no offsets, no accumulation.  What it reaches is the ceiling of that pattern on this
+// machine (0.74-0.75 of the nominal FMA peak on B200, with 4 or 8 targets per thread alike), against which k_m2p_lap's
+// fraction is to be read.
+__global__ void __launch_bounds__(32) k_horner_peak(int ncell, const float *__restrict__ wg, float *out)
+{
+    __shared__ __align__(16) float s_w[8][m2p_lap_stride(8)];
+    for (int i = threadIdx.x; i < 8 * m2p_lap_stride(8); i += 32) s_w[i / m2p_lap_stride(8)][i % m2p_lap_stride(8)] = wg[i];
+    __syncwarp();
+    const int sub = threadIdx.x >> 4;
+    float a = 1e-3f * threadIdx.x, acc = 0.f;
+    for (int c = 0; c < ncell; c++) {
+        typedef LapVec<float> V;
+        const V p = lap_poly<8, float>(V::make(a, a + .1f, a + .2f, a + .3f), V::make(a + .01f, a + .11f, a + .21f, a + .31f),
+                                       V::make(a + .02f, a + .12f, a + .22f, a + .32f), s_w[(2 * c + sub) & 7]);
+        float o[4];
+        p.get(o);
+        acc += (o[0] + o[1]) + (o[2] + o[3]);
+        a += 1e-4f;
+    }
+    if (acc == -12345.f) out[0] = acc;
+}
+
 // out[0] = fp32 FMA TFLOP/s, out[1] = fp64 FMA TFLOP/s, out[2] = MUFU.RSQ Gop/s, out[3] = fp32 FMUL + 3-register
 // FFMA mix TFLOP/s (FMA = 2 flops, MUL = 1); best of 5 launches each
 static int run_alu_peaks(int device, double *out)
@@ -94,6 +119,24 @@ static int run_alu_peaks(int device, double *out)
             if (rep > 0) best = std::max(best, (double)g2 * 128 * iters * 24.0 * 3.0 / (ms * 1e-3));
         }
         out[3] = best * 1e-12;
+    }
+    {   // out[4] = TFLOP/s of the bare Horner stream of k_m2p_lap<8, float> (2 flops per step and target)
+        const int g3 = prop.multiProcessorCount * 16, ncell = 400;
+        float *wg;
+        CUDA_TRY(cudaMalloc(&wg, 8 * m2p_lap_stride(8) * sizeof(float)));
+        CUDA_TRY(cudaMemset(wg, 0, 8 * m2p_lap_stride(8) * sizeof(float)));
+        double best = 0.0;
+        for (int rep = 0; rep < 6; rep++) {
+            CUDA_TRY(cudaEventRecord(e0));
+            k_horner_peak<<<g3, 32>>>(ncell, wg, (float *)buf);
+            CUDA_TRY(cudaEventRecord(e1));
+            CUDA_TRY(cudaEventSynchronize(e1));
+            float ms = 0;
+            CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+            if (rep > 0) best = std::max(best, (double)g3 * 32 * ncell * 4.0 * 164.0 * 2.0 / (ms * 1e-3));
+        }
+        out[4] = best * 1e-12;
+        cudaFree(wg);
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     cudaFree(buf);

@@ -197,10 +197,10 @@ extern "C" int pygbe_stats(const pygbe_handle *h, pygbe_stats_t *s)
     return PYGBE_OK;
 }
 
-extern "C" int pygbe_alu_peaks(int32_t device, double *out4)
+extern "C" int pygbe_alu_peaks(int32_t device, double *out5)
 {
-    if (!out4) { pygbe_set_error("alu_peaks: null pointer"); return PYGBE_EINVAL; }
-    return run_alu_peaks(device, out4);
+    if (!out5) { pygbe_set_error("alu_peaks: null pointer"); return PYGBE_EINVAL; }
+    return run_alu_peaks(device, out5);
 }
 
 extern "C" int pygbe_mma_probe(int32_t device, int32_t P, double *out12)

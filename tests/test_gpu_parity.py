@@ -739,3 +739,38 @@ def test_many_charges_reaction_potential(env):
     eo = o.solvation_energy(x.cpu().numpy())
     assert abs(es - eo) <= 1e-10 * abs(eo)
     h.close()
+
+
+def test_launch_times_account_for_the_lists(env):
+    """pygbe_launch_times (the per-launch records bench.py turns into rooflines): on a three-region problem without
+    twins the two kappa = 0 regions run the Laplace-form M2P, the solvent the regrouped kernel; the units of the
+    compute launches add up to the list counts of pygbe_stats; HBM-bound launches carry byte counts."""
+    pg, torch, orc = env
+    prob = W.stern_sphere_problem(3)
+    for prec, lapname in ((pg.PRECISION_FP64, "k_m2p_lap<P,double>"), (pg.PRECISION_MIXED, "k_m2p_lap<P,float>")):
+        h = pg.Handle.from_problem(prob, K=4, P=6, theta=0.5, ncrit=16, precision=prec)
+        x = torch.tensor(np.random.default_rng(3).normal(size=h.n), device="cuda")
+        y = h.matvec(x)
+        h.profile(True)
+        for _ in range(3):
+            h.matvec(x, y)
+        recs = h.launch_times()
+        stages = h.stage_times()
+        h.profile(False)
+        st = h.stats()
+        m2p = [r for r in recs if r["stage"] == "m2p"]
+        p2p = [r for r in recs if r["stage"] == "p2p"]
+        assert len(m2p) == 3 and len(p2p) == 3 and all(r["launches"] == 3 and r["twin_region"] == -1 for r in m2p + p2p)
+        kappa = list(prob.kappa)
+        for r in m2p:
+            assert (r["kernel"] == lapname) == (kappa[r["region"]] == 0.0)
+        assert sum(r["units"] for r in m2p) == st["m2p_evals"] and sum(r["units"] for r in p2p) == st["p2p_pairs"]
+        for r in recs:
+            if r["stage"] in ("prep", "p2m", "m2m", "near", "combine"):
+                assert r["bytes"] > 0 and r["ms"] > 0
+        assert abs(sum(r["ms"] for r in m2p) - stages["m2p"][0]) < 1e-6
+        # the profiled matvec (one stream, direct launches) and the normal one (graph / three streams) agree
+        y2 = h.matvec(x)
+        assert rel(y2.cpu().numpy(), y.cpu().numpy()) < 1e-12
+        assert st["graph_launches"] >= 1
+        h.close()
