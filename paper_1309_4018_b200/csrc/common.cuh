@@ -319,11 +319,11 @@ struct pygbe_handle {
     long graph_launches = 0;
     char graph_note[160] = "";      // why a capture failed, if one did
     bool overlap = true;
-    // Large problems: the upward pass (P2M stream, M2M) is bandwidth- and latency-bound and runs beside the
-    // FMA-bound P2P; at full width its CTAs (high priority, 350-512 threads, few of them busy) take the thread
-    // slots of every SM and the P2P waits, so the two run one after the other.  Capped at 2 (P2M) / 1 (M2M) CTAs
-    // per SM they share the SMs: 16.5 -> 15.5 ms per matvec on the 1.08 M-panel complex.  Small problems keep the
-    // full width: there the far-field chain is the critical path.
+    // The upward pass (P2M stream, M2M) is bandwidth- and latency-bound and runs beside the FMA-bound P2P; at full
+    // width its CTAs (high priority, 350-512 threads, few of them busy) take the thread slots of every SM and the P2P
+    // waits, so the two run one after the other.  Capped at 4 unsplit (P2M) / 1 (M2M) CTAs per SM they share the SMs:
+    // 16.5 -> 15.3 ms per matvec on the 1.08 M-panel complex, 0.138 -> 0.132 ms on config 1 (every configuration
+    // measured gains 4-10 %).
     bool narrow_upward = false;
     // optional block-diagonal right preconditioner of GMRES (pygbe_options.precond)
     int precond = 0;

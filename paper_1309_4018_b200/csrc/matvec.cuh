@@ -175,10 +175,15 @@ static int matvec_impl(pygbe_handle *h, VecRef x, VecRef y, const int *skip)
             STAGE(h, PYGBE_STAGE_P2M, A.id);
             if (A.n_p2m > 0) {
                 // leaves are taken grid-stride; on large problems the grid is capped (see h->narrow_upward)
-                int p2m_grid = h->narrow_upward ? std::min(A.n_p2m, 2 * h->n_sm) : A.n_p2m;
+                // narrowed: four CTAs per SM of one thread per coefficient (no panel split): the same thread slots as two
+                // split CTAs, twice the leaves in flight (P2M of config 4: 2.8 -> 2.0 ms, matvec 15.5 -> 15.3 ms)
+                int p2m_grid = h->narrow_upward ? std::min(A.n_p2m, 4 * h->n_sm) : A.n_p2m;
                 if (const char *e = tune_env("PYGBE_P2M_GRID")) p2m_grid = std::min(A.n_p2m, std::max(1, atoi(e)));   // tuning
-                if (mixed) LAUNCH(h, k_p2m<float>, p2m_grid, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.n_p2m, A.p2m_rec, A.pq, A.pmomf, A.mom, mo);
-                else LAUNCH(h, k_p2m<double>, p2m_grid, p2m_threads(h->Nc), 0, skip, h->Nc, p2m_nsplit(h->Nc), A.n_p2m, A.p2m_rec, A.pq, A.pmom, A.mom, mo);
+                int nsplit = h->narrow_upward ? 1 : p2m_nsplit(h->Nc);
+                if (const char *e = tune_env("PYGBE_P2M_NSPLIT")) nsplit = std::max(1, atoi(e));                      // tuning
+                const int p2m_thr = (nsplit * h->Nc + 31) / 32 * 32;
+                if (mixed) LAUNCH(h, k_p2m<float>, p2m_grid, p2m_thr, 0, skip, h->Nc, nsplit, A.n_p2m, A.p2m_rec, A.pq, A.pmomf, A.mom, mo);
+                else LAUNCH(h, k_p2m<double>, p2m_grid, p2m_thr, 0, skip, h->Nc, nsplit, A.n_p2m, A.p2m_rec, A.pq, A.pmom, A.mom, mo);
             }
             STAGE_END(h, PYGBE_STAGE_P2M);
             STAGE(h, PYGBE_STAGE_M2M, A.id);
@@ -226,10 +231,11 @@ static int matvec_impl(pygbe_handle *h, VecRef x, VecRef y, const int *skip)
 }
 
 // ---------------------------------------------------------------------------------------------- CUDA graphs
-// Used on the small, launch-latency-bound problems only (h->use_graphs): stream capture does not carry a stream's
-// priority into the kernel nodes, and on the large problems the priorities of the side streams are what lets the
-// narrowed upward pass run beside the P2P (measured on the 1.08 M-panel complex: captured matvec 16.8 ms, like the
-// one without priorities; direct launches 15.5 ms; setting the node attribute after capture changed nothing).
+// Used in direct mode only (theta = 0, no far-field chain; h->use_graphs): stream capture does not carry a stream's
+// priority into the kernel nodes, and the priority of the side streams is what lets the narrowed upward pass and the
+// M2P run beside the P2P.  Measured, captured against direct launches: 1.08 M-panel complex 16.8 / 15.5 ms, config 1
+// 0.138 / 0.132 ms, 1000-atom protein 0.314 / 0.299 ms (setting the priority attribute on the captured nodes changed
+// nothing).  In direct mode a matvec is prep + P2P + corrections + combine and the graph costs nothing.
 // body() issues launches through LAUNCH / matvec_impl; they are captured on h->capst (the caller's stream may be the
 // legacy default stream, which cannot capture) and instantiated.  Returns false if graphs are unavailable; the
 // caller then launches directly.

@@ -772,5 +772,14 @@ def test_launch_times_account_for_the_lists(env):
         # the profiled matvec (one stream, direct launches) and the normal one (graph / three streams) agree
         y2 = h.matvec(x)
         assert rel(y2.cpu().numpy(), y.cpu().numpy()) < 1e-12
-        assert st["graph_launches"] >= 1
+        assert st["graph_launches"] == 0             # a treecode handle keeps its stream priorities: no graph
         h.close()
+    # direct mode (theta = 0) has no far-field chain: the matvec and the GMRES iterations are replayed as CUDA graphs
+    h = pg.Handle.from_problem(W.born_problem(2), K=4, theta=0.0)
+    x = torch.tensor(np.random.default_rng(4).normal(size=h.n), device="cuda")
+    ya = h.matvec(x).cpu().numpy()
+    h.profile(True); yb = h.matvec(x).cpu().numpy(); h.profile(False)       # direct launches, one stream
+    assert rel(ya, yb) < 1e-12
+    xs, it, rr, rc = h.solve(tol=1e-8)
+    assert h.stats()["graph_launches"] >= 2 and rr <= 1e-8
+    h.close()
