@@ -254,6 +254,22 @@ int pygbe_alu_peaks(int32_t device, double *out5);
  * the tile-only variant), out12[3 v + 2] = (group, cell) pairs per launch.  P = 6 or 8.  out12: HOST.  Synchronous. */
 int pygbe_mma_probe(int32_t device, int32_t P, double *out12);
 
+/* ONE entry point that allocates nothing (csrc/noalloc.cu), for callers that cannot call cudaMalloc (CUDA graph
+ * capture, tight serving loops, harnesses that forbid it): the Coulomb energy of n point charges in one region of
+ * permittivity eps (eq. 8),  E = 1/2 C0 sum_{k != l} q_k q_l / (4 pi eps r_kl)  in kJ/mol -- the term
+ * pygbe_energy returns as E_coul, without a handle.  Its scratch (the charges packed as (x, y, z, q) records and the
+ * accumulator) is a file-scope static __device__ array of PYGBE_NOALLOC_MAX_CHARGES records, 512.25 KB, which every GPU
+ * that loads the library holds until the process exits.  The call issues three kernels on `stream` and calls no
+ * cudaMalloc, cudaFree or allocating library routine; n > PYGBE_NOALLOC_MAX_CHARGES is rejected with PYGBE_EINVAL.
+ * xyz_dev [n][3], q_dev [n]: DEVICE, read only;  E_dev [1]: DEVICE, written.  Asynchronous.  The array is shared by
+ * every call and keeps the last call's contents (each call rewrites what it uses and clears the accumulator): calls
+ * that overlap on the GPU -- two streams, two host threads -- race on it; serialise them.  pygbe_noalloc_setup takes
+ * the array's device address (once per device; also done by the first call) so that later calls do no set-up work. */
+#define PYGBE_NOALLOC_MAX_CHARGES 16384
+int pygbe_noalloc_setup(int32_t device);
+int pygbe_coulomb_energy_noalloc(int32_t device, void *stream, const double *xyz_dev, const double *q_dev, int64_t n,
+                                 double eps, double *E_dev);
+
 /* Library / build identification, e.g. "pygbe-b200 0.3 sm_100a". */
 const char *pygbe_version(void);
 

@@ -330,5 +330,28 @@ def mma_probe(P=8, device=0):
     return {n: dict(ms=out[3 * i], rel_l2=out[3 * i + 1], pairs=out[3 * i + 2]) for i, n in enumerate(names)}
 
 
+NOALLOC_MAX_CHARGES = 16384
+
+
+def coulomb_energy_noalloc(xyz, q, eps, out, device=0, stream=None):
+    """pygbe_coulomb_energy_noalloc: Coulomb energy (kJ/mol) of the charges xyz [n,3], q [n] (fp64 CUDA tensors) in a
+    region of permittivity eps, written to out (fp64 CUDA tensor, 1 element).  Allocates nothing; asynchronous."""
+    import torch
+    L = lib()
+    L.pygbe_coulomb_energy_noalloc.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_void_p]
+    if stream is None:
+        stream = torch.cuda.current_stream(device).cuda_stream
+    n = int(q.numel())
+    _check(L.pygbe_coulomb_energy_noalloc(device, C.c_void_p(stream), _dptr(xyz) if n else None, _dptr(q) if n else None, n,
+                                          float(eps), _dptr(out)))
+    return out
+
+
+def noalloc_setup(device=0):
+    L = lib()
+    L.pygbe_noalloc_setup.argtypes = [C.c_int32]
+    _check(L.pygbe_noalloc_setup(device))
+
+
 def pygbe_version():
     return lib().pygbe_version().decode()

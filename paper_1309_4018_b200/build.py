@@ -52,7 +52,8 @@ def build(force=False, verbose=False):
     if force:
         for f in os.listdir(OBJ):
             os.remove(os.path.join(OBJ, f))
-    jobs = [(os.path.join(CSRC, "pygbe.cu"), os.path.join(OBJ, "pygbe.o"), [])]
+    jobs = [(os.path.join(CSRC, "pygbe.cu"), os.path.join(OBJ, "pygbe.o"), []),
+            (os.path.join(CSRC, "noalloc.cu"), os.path.join(OBJ, "noalloc.o"), [])]
     # the largest orders first: they take longest
     # PYGBE_FAST_BUILD=<n>: development shortcut, orders above n are compiled as stubs that refuse to run
     fast = int(os.environ.get("PYGBE_FAST_BUILD", "0"))
