@@ -160,7 +160,8 @@ static int matvec_impl(pygbe_handle *h, VecRef x, VecRef y, const int *skip)
     }
     if (fork) cudaEventRecord(h->ev_join2, h->side2);
 
-    // far field: upward passes of all trees, then their M2P
+    // far field: upward passes of all trees, then their M2P (starting a tree's M2P on another stream as soon as its own
+    // upward pass is done was slower: the contention delays the later trees' upward passes)
     h->stream = fork ? h->side : main_st;
     if (any_far) {
         for (auto &w : work) {
