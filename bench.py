@@ -75,19 +75,19 @@ def make_problem(name):
 
 # ------------------------------------------------------------------------------------------ flop model
 def m2p_nw(P):
-    """W_{m,e} per moment set of the regrouped Taylor series (m2p.cuh): 130 at P = 6, 295 at P = 8."""
-    return sum((t + 1) * (t + 2) // 2 * ((P - t) // 2 + 1) for t in range(P + 1))
+    """W_{m,e} per moment set of the regrouped Taylor series on harmonically reduced moments (m2p.cuh, tables.cuh):
+    84 at P = 6, 165 at P = 8 (unreduced: 130, 295)."""
+    return sum((2 * t + 1) * ((P - t) // 2 + 1) for t in range(P + 1))
 
 
 def m2p_flops(P, yukawa):
     """Algorithmic flops of one (target, cell) Taylor evaluation as the regrouped kernels do it (m2p.cuh;
-    multiply-add = 2, rsqrt = exp = 1): offset and radius, the Nc - 1 monomials d^e, one FMA per W_{m,e} for every
-    region in `yukawa` (a tuple of booleans: one entry, or two for twin regions evaluated in one pass), and per
+    multiply-add = 2, rsqrt = exp = 1): offset and radius, the (P+1)^2 - 1 monomials d^e with ez <= 1, one FMA per W_{m,e}
+    for every region in `yukawa` (a tuple of booleans: one entry, or two for twin regions evaluated in one pass), and per
     region the P + 1 radial derivatives F^(m) and their dot product with Q_m.  DESIGN.md 'Flop model'."""
     if isinstance(yukawa, bool):
         yukawa = (yukawa,)
-    nc = (P + 1) * (P + 2) * (P + 3) // 6
-    f = 3 + 5 + 3 + (nc - 1)                           # d ; r^2 ; 1/r, 1/r^2, r ; monomials
+    f = 3 + 5 + 3 + ((P + 1) * (P + 1) - 1)            # d ; r^2 ; 1/r, 1/r^2, r ; monomials
     for yk in yukawa:
         f += 2 * m2p_nw(P)                             # Q_m += W d^e
         f += (2 if yk else 0) + 1 + 5                  # [kappa r, exp] ; F0 ; F1

@@ -107,7 +107,8 @@ static int build_tree_and_lists(pygbe_handle *h, Region &R)
     // evaluation costs Nc - 1 + NW FMA-pipe instructions per region, a P2P pair ~14 per region, and the sweep of
     // profiles/r2a_regrouped_path.md puts the optimum at ~16 points for P = 6 (344 instructions) in both precisions
     // (the Laplace form costs Nc - 1 FMAs)
-    int small_leaf = (int)(16.0 * (R.lap ? (double)h->Nc : h->Nc + 2.0 * h->NW) / 344.0 / K);
+    // (regrouped form on reduced moments: (P+1)^2 monomials + NW FMAs per region)
+    int small_leaf = (int)(16.0 * (R.lap ? (double)h->Nc : (h->P + 1.0) * (h->P + 1.0) + 2.0 * h->NW) / 344.0 / K);
     if (const char *e = tune_env("PYGBE_SMALL_LEAF")) small_leaf = atoi(e);                     // tuning
     const int exact_mac = h->group_mac == 0 ? 1 : 0;             // 1 = group MAC on the group's own points
     LAUNCH(h, k_traverse, cdiv(R.ng, TRAV_WARPS), TRAV_WARPS * 32, 0, R.ng, R.tpos, R.np, exact_mac, R.ggeo, R.cgeo, R.crange, R.cchild,

@@ -234,6 +234,7 @@ struct Region {
     long p2p_pairs = 0, m2p_evals = 0;
     // multipoles ------------------------------------------------------------------------------------
     double *mom = nullptr;          // [ncells][2][Nc]: MV, MK (farfield.cuh), shared by twin regions
+    const int *wt_off = nullptr; const short *wt_k = nullptr; const double *wt_c = nullptr;   // the W table of this region's kappa (handle-owned)
     bool lap = false;               // tree owner, kappa = 0, no twin: wc holds the Nc coefficients C'_f of k_m2p_lap instead
     long p2m_panels = 0, m2m_children = 0;   // panels streamed by one P2M launch, child cells read by one M2M launch
     void *wc = nullptr;             // tree owner: [ncells][m2p_stride(P, twin)] regrouped multipoles W_{m,e} of this region and,
@@ -303,7 +304,8 @@ struct pygbe_handle {
     double *phi_reac = nullptr;     // [nq]
     struct IndexTables *itab = nullptr;   // device copy of the multi-index tables
     int NW = 0;                           // W_{m,e} per moment set (m2p_nw(P)) and the table that forms them (tables.cuh)
-    int *wt_off = nullptr; short *wt_k = nullptr; double *wt_c = nullptr;
+    struct WDev { double kappa; int *off; short *k; double *c; };
+    std::vector<WDev> wtabs;              // one reduced W table per distinct kappa among the regions (tables.cuh)
     int *lt_off = nullptr; short *lt_k = nullptr, *lt_deg = nullptr; double *lt_c = nullptr;   // Laplace form (build_lap_table), Nc entries
     cudaStream_t side = nullptr;    // far-field chain (P2M, M2M, M2P) runs here, concurrently with P2P
     cudaStream_t side2 = nullptr;   // near-field correction SpMV runs here

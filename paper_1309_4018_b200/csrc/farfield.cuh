@@ -25,7 +25,8 @@ struct MomOut {
     void *wc;
     double caA, cbA, caB, cbB;
     int fp32, stride, twin, NW;
-    const int *wt_off; const short *wt_k; const double *wt_c;
+    const int *wt_off; const short *wt_k; const double *wt_c;      // table of the tree owner's kappa (tables.cuh)
+    const int *wtB_off; const short *wtB_k; const double *wtB_c;   // table of the twin's kappa (the reduction depends on kappa)
     const short *wt_deg;            // Laplace form: degree of entry p; nullptr otherwise
     const double4 *cgeo;            // cell geometry (edge length in .w)
 };
@@ -40,7 +41,16 @@ __device__ __forceinline__ void wc_store(const MomOut &o, long cell, const doubl
             const double c = o.wt_c[i];
             wv += c * mv[k]; wk += c * mk[k];
         }
-        double a = o.caA * wv + o.cbA * wk, b = o.caB * wv + o.cbB * wk;
+        double a = o.caA * wv + o.cbA * wk, b = 0.0;
+        if (o.twin) {
+            double bv = 0.0, bk = 0.0;
+            for (int i = o.wtB_off[p]; i < o.wtB_off[p + 1]; i++) {
+                const int k = o.wtB_k[i];
+                const double c = o.wtB_c[i];
+                bv += c * mv[k]; bk += c * mk[k];
+            }
+            b = o.caB * bv + o.cbB * bk;
+        }
         if (o.wt_deg) {                                            // C'_f = C_f / edge^|f|
             double s = 1.0;
             for (int d = o.wt_deg[p]; d > 0; d--) s *= inv_edge;

@@ -28,12 +28,14 @@
 #define PYGBE_TG_M2P PYGBE_TG
 
 // number of W_{m,e} per moment set, in the order the kernel consumes them (ex, ey, ez ascending, then J)
+// (harmonically reduced moments, tables.cuh: ez <= 1, i.e. 2 t + 1 monomials of degree t)
 static inline __host__ __device__ constexpr int m2p_nw(int P)
 {
     int n = 0;
-    for (int t = 0; t <= P; t++) n += (t + 1) * (t + 2) / 2 * ((P - t) / 2 + 1);
+    for (int t = 0; t <= P; t++) n += (2 * t + 1) * ((P - t) / 2 + 1);
     return n;
 }
+#define M2P_EZ(P, ex, ey) ((P) - (ex) - (ey) < 1 ? (P) - (ex) - (ey) : 1)      // last ez of the reduced index set
 // Row stride of wc[cell][stride] (elements of T): the W of the tree owner and, interleaved, of its twin,
 // padded to a multiple of 4 so that every row starts on a 16-byte boundary and moves with 16-byte cp.async.
 static inline __host__ __device__ constexpr int m2p_stride(int P, bool twin) { return (m2p_nw(P) * (twin ? 2 : 1) + 3) / 4 * 4; }
@@ -82,7 +84,7 @@ __device__ __forceinline__ void m2p_q(T dx, T dy, T dz, const T *__restrict__ w,
         for (int ey = 0; ey <= P - ex; ey++) {
             T mono = pxy;
 #pragma unroll
-            for (int ez = 0; ez <= P - ex - ey; ez++) {
+            for (int ez = 0; ez <= M2P_EZ(P, ex, ey); ez++) {
                 const int t = ex + ey + ez;
 #pragma unroll
                 for (int J = 0; J <= (P - t) / 2; J++) {
@@ -142,7 +144,7 @@ __device__ __forceinline__ f2_t m2p_twin_packed(float dx, float dy, float dz, co
         for (int ey = 0; ey <= P - ex; ey++) {
             float mono = pxy;
 #pragma unroll
-            for (int ez = 0; ez <= P - ex - ey; ez++) {
+            for (int ez = 0; ez <= M2P_EZ(P, ex, ey); ez++) {
                 const int t = ex + ey + ez;
                 const f2_t m2 = f2_pack(mono, mono);
 #pragma unroll
@@ -269,7 +271,7 @@ __device__ __forceinline__ void m2p_twin_packed2(f2_t dx, f2_t dy, f2_t dz, cons
         for (int ey = 0; ey <= P - ex; ey++) {
             f2_t mono = pxy;
 #pragma unroll
-            for (int ez = 0; ez <= P - ex - ey; ez++) {
+            for (int ez = 0; ez <= M2P_EZ(P, ex, ey); ez++) {
                 const int t = ex + ey + ez;
                 float ma, mb;
                 f2_unpack(mono, ma, mb);
@@ -441,7 +443,7 @@ k_m2p_single2(const int *__restrict__ skip, const int4 *__restrict__ items, cons
                 for (int ey = 0; ey <= P - ex; ey++) {
                     f2_t mono = pxy;
 #pragma unroll
-                    for (int ez = 0; ez <= P - ex - ey; ez++) {
+                    for (int ez = 0; ez <= M2P_EZ(P, ex, ey); ez++) {
                         const int t = ex + ey + ez;
 #pragma unroll
                         for (int J = 0; J <= (P - t) / 2; J++) {
@@ -507,7 +509,7 @@ __device__ __forceinline__ void m2p_q2(double dx0, double dy0, double dz0, doubl
         for (int ey = 0; ey <= P - ex; ey++) {
             double m0 = pxy0, m1 = pxy1;
 #pragma unroll
-            for (int ez = 0; ez <= P - ex - ey; ez++) {
+            for (int ez = 0; ez <= M2P_EZ(P, ex, ey); ez++) {
                 const int t = ex + ey + ez;
 #pragma unroll
                 for (int J = 0; J <= (P - t) / 2; J++) {

@@ -172,7 +172,9 @@ static int matvec_impl(pygbe_handle *h, VecRef x, VecRef y, const int *skip)
             mo.wc = A.wc; mo.caA = 1.0; mo.cbA = -1.0; mo.caB = A.twin_rV; mo.cbB = 1.0;
             mo.fp32 = mixed ? 1 : 0; mo.twin = B ? 1 : 0; mo.stride = m2p_row_elems(h->P, A); mo.cgeo = A.cgeo;
             if (A.lap) { mo.NW = h->Nc; mo.wt_off = h->lt_off; mo.wt_k = h->lt_k; mo.wt_c = h->lt_c; mo.wt_deg = h->lt_deg; }
-            else { mo.NW = h->NW; mo.wt_off = h->wt_off; mo.wt_k = h->wt_k; mo.wt_c = h->wt_c; mo.wt_deg = nullptr; }
+            else { mo.NW = h->NW; mo.wt_off = A.wt_off; mo.wt_k = A.wt_k; mo.wt_c = A.wt_c; mo.wt_deg = nullptr; }
+            const Region &T = B ? *B : A;
+            mo.wtB_off = T.wt_off; mo.wtB_k = T.wt_k; mo.wtB_c = T.wt_c;
             STAGE(h, PYGBE_STAGE_P2M, A.id);
             if (A.n_p2m > 0) {
                 // leaves are taken grid-stride; on large problems the grid is capped (see h->narrow_upward)

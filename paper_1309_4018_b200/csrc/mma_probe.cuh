@@ -1,13 +1,14 @@
 // mma_probe.cuh -- the tensor-core question of the north star, answered with numbers (SURVEY 8(d) "Tensor cores",
 // 8(f) item 3): "tensor cores are used only if a batched M2P stage is shown to be a dense contraction".
 //
-// In the regrouped form of the series (m2p.cuh) the 64 targets of a group multiply their monomial rows d^e by the
-// SAME per-cell coefficients: per (group, cell) that is the product  Q[64 x (P+1)] = A[64 x Nc] * B[Nc x (P+1)],
-// A[t][e] = d_t^e (target-specific, recomputed for every cell), B[e][m] = W_{m,e} (20 % dense), followed by
+// In the regrouped form of the series (m2p.cuh; harmonically reduced moments, Ne = (P+1)^2 monomials with ez <= 1) the
+// 64 targets of a group multiply their monomial rows d^e by the SAME per-cell coefficients: per (group, cell) that is
+// the product  Q[64 x (P+1)] = A[64 x Ne] * B[Ne x (P+1)],
+// A[t][e] = d_t^e (target-specific, recomputed for every cell), B[e][m] = W_{m,e} (23 % dense), followed by
 // sum_m F^(m)(r_t) Q[t][m].  This file measures, on synthetic far-field data shaped like the M2P lists of the Yukawa
 // region of config 4 (P = 8, single moment set, 64-target groups, cells of 2-8 A at 1.1-3 times the MAC distance),
 //   cuda   the production kernel k_m2p_single2<P> (packed fp32 FMAs, coefficients broadcast from shared memory),
-//   tile   only what ANY tensor-core formulation has to do first: put the 64 x Nc monomial tile of every (group,
+//   tile   only what ANY tensor-core formulation has to do first: put the 64 x Ne monomial tile of every (group,
 //          cell) into shared memory (tcgen05.mma and mma.sync both read A from shared memory / TMEM, and the
 //          monomials are per target and per cell, so the tile cannot be reused or loaded by TMA),
 //   mma1   tile + the contraction on the tensor cores in one TF32 pass + the radial combination,
@@ -38,7 +39,7 @@ __device__ __forceinline__ void mma_tf32(float (&d)[4], const float (&a)[4], con
 }
 
 template <int P> struct MmaShape {
-    static constexpr int NC = (P + 1) * (P + 2) * (P + 3) / 6;
+    static constexpr int NC = (P + 1) * (P + 1);           // monomials d^e of the reduced index set (ez <= 1)
     static constexpr int KP = (NC + 7) / 8 * 8;            // K padded to the MMA's k = 8
     static constexpr int NP = (P + 1 + 7) / 8 * 8;         // N padded to n = 8 tiles
     static constexpr int AS = KP + 1;                      // row stride of the A tile (odd: conflict-free row writes)
@@ -63,7 +64,7 @@ __device__ __forceinline__ void mp_build_tile(float dx0, float dy0, float dz0, f
         for (int ey = 0; ey <= P - ex; ey++) {
             float m0 = pxy0, m1 = pxy1;
 #pragma unroll
-            for (int ez = 0; ez <= P - ex - ey; ez++) {
+            for (int ez = 0; ez <= M2P_EZ(P, ex, ey); ez++) {
                 const float h0 = to_tf32(m0), h1 = to_tf32(m1);
                 r0[idx] = h0; r1[idx] = h1;
                 if (SPLIT) { l0[idx] = to_tf32(m0 - h0); l1[idx] = to_tf32(m1 - h1); }
@@ -225,11 +226,12 @@ template <int P> static int run_mma_probe_p(int device, double *out)
     IndexTables *it = new IndexTables;
     fill_index_tables(it);
     WTable wt;
-    build_w_table(P, *it, &wt);
+    build_w_table(P, kappa, *it, &wt);
     const int NW = (int)wt.off.size() - 1, stride = m2p_stride(P, false);
     std::vector<float> wc((size_t)NCELL * stride, 0.f), Bhi((size_t)NCELL * S::NP * S::KP, 0.f), Blo(Bhi.size(), 0.f);
     auto tf32 = [](float x) { unsigned u; memcpy(&u, &x, 4); u += 0x1000u; u &= 0xffffe000u; float y; memcpy(&y, &u, 4); return y; };   // round to nearest (ties away), 10-bit mantissa
-    std::vector<double> M(S::NC);
+    const int NCF = nc_of(P);                              // full set of Cartesian moments, the input of the table
+    std::vector<double> M(NCF);
     for (int c = 0; c < NCELL; c++) {
         const double edge = 2.0 * (1 << (c % 3));
         double d[3]; unit(d);
@@ -239,14 +241,14 @@ template <int P> static int run_mma_probe_p(int device, double *out)
         for (int k = 0; k < NQ; k++) {
             const double x = edge * (U(rng) - 0.5), y = edge * (U(rng) - 0.5), z = edge * (U(rng) - 0.5), q = N01(rng);
             qpos[(size_t)c * NQ + k] = make_double4(cgeo[c].x + x, cgeo[c].y + y, cgeo[c].z + z, q);
-            for (int i = 0; i < S::NC; i++)
+            for (int i = 0; i < NCF; i++)
                 M[i] += q * std::pow(x, it->kxyz[i][0]) * std::pow(y, it->kxyz[i][1]) * std::pow(z, it->kxyz[i][2]);
         }
         // W stream (m2p.cuh order) and the same numbers as the dense tile B[m][e]
         int p = 0, e = 0;
         for (int ex = 0; ex <= P; ex++)
             for (int ey = 0; ey <= P - ex; ey++)
-                for (int ez = 0; ez <= P - ex - ey; ez++, e++)
+                for (int ez = 0; ez <= M2P_EZ(P, ex, ey); ez++, e++)
                     for (int J = 0; J <= (P - ex - ey - ez) / 2; J++, p++) {
                         double w = 0.0;
                         for (int i = wt.off[p]; i < wt.off[p + 1]; i++) w += wt.c[i] * M[wt.k[i]];

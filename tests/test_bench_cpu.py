@@ -20,15 +20,17 @@ def _free_port():
 
 def test_whole_job_value_and_flop_model():
     assert bench.whole_job_value(4, 1000, 10, 2.0) == 20000.0
-    # regrouped Taylor series (m2p.cuh): W_{m,e} counts, more terms with order, Yukawa = Laplace + exp
-    assert bench.m2p_nw(6) == 130 and bench.m2p_nw(8) == 295 and bench.m2p_nw(0) == 1
+    # regrouped Taylor series on harmonically reduced moments (m2p.cuh, tables.cuh): W_{m,e} counts, more terms with
+    # order, Yukawa = Laplace + exp
+    assert bench.m2p_nw(6) == 84 and bench.m2p_nw(8) == 165 and bench.m2p_nw(0) == 1
     f = [bench.m2p_flops(P, False) for P in (1, 2, 6, 8)]
     assert all(b > a for a, b in zip(f, f[1:]))
     assert bench.m2p_flops(6, True) == bench.m2p_flops(6, False) + 2
-    # cross-check against the SASS of k_m2p<6, twin, float> per (target, cell): 276 FFMA + 116 FMUL + 10 FADD
-    # + 3 MUFU = 681 flops; the model counts the fp64 offset subtraction and the unfused radial terms on top
-    assert bench.m2p_flops(6, False) == 394 and bench.m2p_flops(6, (False, True)) == 696
+    # P = 6: 11 + 48 monomials + 2 * 84 + 6 + 20 + 14 = 267 for one region; twin regions share offsets and monomials
+    assert bench.m2p_flops(6, False) == 267 and bench.m2p_flops(6, (False, True)) == 477
+    assert bench.m2p_flops(8, True) == 11 + 80 + 2 * 165 + 8 + 28 + 18
     assert bench.m2p_flops(6, (False, True)) < bench.m2p_flops(6, False) + bench.m2p_flops(6, True)
+    assert bench.m2p_lap_flops(8) == 344
     assert bench.P2P_FLOPS_FUSED < bench.P2P_FLOPS[False] + bench.P2P_FLOPS[True]
 
 
