@@ -10,10 +10,12 @@
 //     sum_k a^k M^k = sum_{m=0..P} F^(m)(s) Q_m,     Q_m = sum_{e : |e| <= m, 2m - |e| <= P} W_{m,e} d^e,
 //     W_{m,e} = (-1)^|e| / e!  sum_{|j| = m - |e|}  M^(e + 2j) / (2^|j| j!)
 // where the W depend on the cell only: they are formed when the cell's multipoles are (P2M / M2M epilogue,
-// farfield.cuh, from a table built at create) and replace the multipoles as the M2P's input.  Per (target,
-// cell) the work is then Nc - 1 multiplies for the monomials and one FMA per W -- 130 per moment set at P = 6,
-// 295 at P = 8 -- instead of a recurrence of 6 (Laplace) to 12 (Yukawa) instructions per coefficient, and it
-// is independent of the kernel: Laplace and Yukawa differ only in the P + 1 numbers F^(m)(s),
+// farfield.cuh, from a table built at create) and replace the multipoles as the M2P's input.  The M here are the
+// HARMONICALLY REDUCED moments of tables.cuh ((laplace - kappa^2) G = 0 folds every moment with kz >= 2 into lower
+// ones, exactly), so only e with ez <= 1 occur.  Per (target, cell) the work is then (P+1)^2 - 1 multiplies for the
+// monomials and one FMA per W -- 84 per moment set at P = 6, 165 at P = 8 (unreduced: Nc - 1 and 130 / 295) -- instead
+// of a recurrence of 6 (Laplace) to 12 (Yukawa) instructions per coefficient, and its form is
+// independent of the kernel: Laplace and Yukawa differ only in the table and in the P + 1 numbers F^(m)(s),
 //     F^(0) = exp(-kappa r) / r,   F^(1) = -exp(-kappa r) (kappa r + 1) / r^3,
 //     F^(m+1) = -[ (2m + 1) F^(m) - kappa^2 F^(m-1) ] / r^2        (kappa = 0: Laplace),
 // so the two regions on either side of a surface set ("twins") are evaluated in one pass.
