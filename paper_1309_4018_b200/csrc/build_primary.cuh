@@ -45,15 +45,12 @@ static int build_region_primary(pygbe_handle *h, Region &R, const std::vector<do
     TRY(h->mem.alloc(&d_keys_u, R.np)); TRY(h->mem.alloc(&R.keys, R.np));
     LAUNCH(h, k_region_keys, cdiv(R.np, 256), 256, 0, h->gcen, d_gid_u, R.np, R.root_c[0] - 0.5 * edge,
            R.root_c[1] - 0.5 * edge, R.root_c[2] - 0.5 * edge, 2097152.0 / edge, d_keys_u, d_iota);
-    {
-        size_t tmp_bytes = 0;
-        cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, d_keys_u, R.keys, d_iota, R.perm, R.np, 0, 63, h->stream);
-        char *tmp;
-        TRY(h->mem.alloc(&tmp, tmp_bytes));
-        CUDA_TRY(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, d_keys_u, R.keys, d_iota, R.perm, R.np, 0, 63, h->stream));
-        h->launches += 4;
+    {   // stable radix sort of (Morton key, panel) by the 63 key bits (blockops.cuh)
+        int *hist;
+        TRY(h->mem.alloc(&hist, (size_t)256 * radix_sort_ctas(R.np)));
+        TRY(radix_sort_pairs(d_keys_u, d_iota, R.keys, R.perm, R.np, 63, hist, h->stream, &h->launches));
         CUDA_TRY(cudaStreamSynchronize(h->stream));
-        h->mem.release_one(tmp);
+        h->mem.release_one(hist);
     }
     TRY(h->mem.alloc(&R.gid, R.np)); TRY(h->mem.alloc(&R.phi_idx, R.np)); TRY(h->mem.alloc(&R.dphi_idx, R.np));
     TRY(h->mem.alloc(&R.row_idx, R.np)); TRY(h->mem.alloc(&R.cV, R.np)); TRY(h->mem.alloc(&R.cK, R.np));

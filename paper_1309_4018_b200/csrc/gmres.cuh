@@ -11,7 +11,7 @@
 #include "common.cuh"
 #include "tables.cuh"
 #include "nearfield.cuh"
-#include <cub/cub.cuh>
+#include "blockops.cuh"
 
 #define GM_THREADS 256
 #define GM_ROWS_PER_CTA 2048
@@ -23,12 +23,10 @@ k_gm_residual(const int *__restrict__ flags, long n, const double *__restrict__ 
               int use_w, double *__restrict__ r, double *__restrict__ scal)
 {
     if (flags[0]) return;
-    typedef cub::BlockReduce<double, GM_THREADS> Red;
-    __shared__ typename Red::TempStorage tmp;
     long i = (long)blockIdx.x * GM_THREADS + threadIdx.x;
     double v = 0.0;
     if (i < n) { v = b[i] - (use_w ? w[i] : 0.0); r[i] = v; }
-    double s = Red(tmp).Sum(v * v);
+    double s = block_sum<GM_THREADS>(v * v);
     if (threadIdx.x == 0) atomicAdd(scal + 3, s);
 }
 
@@ -140,8 +138,6 @@ k_gm_arnoldi(int *flags, double *V, long n, int m, double *w, double *h1, double
     // the step number is the count of columns built so far; it is read here by every CTA and rewritten only after
     // the last grid-wide barrier, so one captured launch serves every step
     const int j = flags[1];
-    typedef cub::BlockReduce<double, GM_THREADS> Red;
-    __shared__ typename Red::TempStorage tmp;
     const int nvec = j + 1;
     const long per = (n + gridDim.x - 1) / gridDim.x;
     const long lo = (long)blockIdx.x * per, hi = min(n, lo + per);
@@ -204,7 +200,7 @@ k_gm_arnoldi(int *flags, double *V, long n, int m, double *w, double *h1, double
     // phase 3
     {
         const double part = slice_update(h2, true);
-        const double s = Red(tmp).Sum(part);
+        const double s = block_sum<GM_THREADS>(part);
         if (threadIdx.x == 0) atomicAdd(nrm2, s);
     }
     grid.sync();

@@ -3,7 +3,7 @@
 #pragma once
 #include "common.cuh"
 #include "tables.cuh"
-#include <cub/cub.cuh>
+#include "blockops.cuh"
 
 // One (target, Gauss point) interaction with the region's kernel, both layers at once (eq. 2 / 9,
 // PAPER.md:55-58, :98):   mV G(r) - mK . grad_y G,   G = exp(-kappa r)/r   (1/(4 pi) is in the weights),
@@ -286,8 +286,6 @@ k_reaction(int npts, const double4 *__restrict__ spos, const double4 *__restrict
            const double4 *__restrict__ qpos, const int *__restrict__ qid, double kappa,
            double *__restrict__ phi_reac)
 {
-    typedef cub::BlockReduce<double, EN_THREADS> Red;
-    __shared__ typename Red::TempStorage tmp;
     int k = blockIdx.x;
     double4 X = qpos[k];
     long lo = (long)blockIdx.y * EN_CHUNK, hi = min((long)npts, lo + EN_CHUNK);
@@ -296,7 +294,7 @@ k_reaction(int npts, const double4 *__restrict__ spos, const double4 *__restrict
         double4 a = spos[i], c = schg[i];
         acc += pair_f64<YUKAWA>(X.x - a.x, X.y - a.y, X.z - a.z, c.x, c.y, c.z, c.w, kappa);
     }
-    double s = Red(tmp).Sum(acc);
+    double s = block_sum<EN_THREADS>(acc);
     if (threadIdx.x == 0) atomicAdd(phi_reac + qid[k], s);
 }
 
@@ -304,19 +302,15 @@ k_reaction(int npts, const double4 *__restrict__ spos, const double4 *__restrict
 __global__ void __launch_bounds__(256) k_dot_q(int nq, const double *__restrict__ q,
                                                const double *__restrict__ phi, double *__restrict__ out)
 {
-    typedef cub::BlockReduce<double, 256> Red;
-    __shared__ typename Red::TempStorage tmp;
     double acc = 0.0;
     for (int i = threadIdx.x; i < nq; i += 256) acc += q[i] * phi[i];
-    double s = Red(tmp).Sum(acc);
+    double s = block_sum<256>(acc);
     if (threadIdx.x == 0) out[0] = s;
 }
 
 // Coulomb energy sum over pairs inside one region (eq. 8): sum_{k != l} q_k q_l / r_kl.
 __global__ void __launch_bounds__(128) k_coulomb(int nq, const double4 *__restrict__ qpos, double *__restrict__ out)
 {
-    typedef cub::BlockReduce<double, 128> Red;
-    __shared__ typename Red::TempStorage tmp;
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     double acc = 0.0;
     if (k < nq) {
@@ -327,6 +321,6 @@ __global__ void __launch_bounds__(128) k_coulomb(int nq, const double4 *__restri
         }
         acc *= X.w;
     }
-    double s = Red(tmp).Sum(acc);
+    double s = block_sum<128>(acc);
     if (threadIdx.x == 0) atomicAdd(out, s);
 }

@@ -3,7 +3,7 @@
 #pragma once
 #include "common.cuh"
 #include "tables.cuh"
-#include <cub/cub.cuh>
+#include "blockops.cuh"
 
 // ------------------------------------------------------------------------------------------ geometry
 // flat triangles, collocation at the panel centre.  flags[0] is raised for a
@@ -100,8 +100,6 @@ k_split_level(const unsigned long long *__restrict__ keys, int level, int lvl_be
               int maxcells, double4 *cgeo, int2 *crange, int2 *cchild, int *cparent,
               unsigned long long *ckey, int *ncells_io)
 {
-    typedef cub::BlockScan<int, SPLIT_THREADS> Scan;
-    __shared__ typename Scan::TempStorage tmp;
     __shared__ int s_base;
     if (threadIdx.x == 0) s_base = *ncells_io;
     __syncthreads();
@@ -128,7 +126,7 @@ k_split_level(const unsigned long long *__restrict__ keys, int level, int lvl_be
             }
         }
         int off, total;
-        Scan(tmp).ExclusiveSum(nchild, off, total);
+        block_exclusive_sum<SPLIT_THREADS>(nchild, off, total);
         int base = s_base;
         __syncthreads();
         if (nchild > 0) {
@@ -165,8 +163,6 @@ k_split_level(const unsigned long long *__restrict__ keys, int level, int lvl_be
 __global__ void __launch_bounds__(PYGBE_TG)
 k_group_geometry(const double4 *__restrict__ tpos, int np, double4 *__restrict__ ggeo)
 {
-    typedef cub::BlockReduce<double, PYGBE_TG> Red;
-    __shared__ typename Red::TempStorage tmp;
     __shared__ double s_c[3];
     int g = blockIdx.x;
     int t = g * PYGBE_TG + threadIdx.x;
@@ -176,16 +172,16 @@ k_group_geometry(const double4 *__restrict__ tpos, int np, double4 *__restrict__
     double mn[3], mx[3];
     double v[3] = {x.x, x.y, x.z};
     for (int a = 0; a < 3; a++) {
-        mn[a] = Red(tmp).Reduce(ok ? v[a] : big, cub::Min());
+        mn[a] = block_reduce<PYGBE_TG>(ok ? v[a] : big, OpMin());
         __syncthreads();
-        mx[a] = Red(tmp).Reduce(ok ? v[a] : -big, cub::Max());
+        mx[a] = block_reduce<PYGBE_TG>(ok ? v[a] : -big, OpMax());
         __syncthreads();
         if (threadIdx.x == 0) s_c[a] = 0.5 * (mn[a] + mx[a]);
     }
     __syncthreads();
     double dx = x.x - s_c[0], dy = x.y - s_c[1], dz = x.z - s_c[2];
     double r = ok ? sqrt(dx * dx + dy * dy + dz * dz) : 0.0;
-    double rmax = Red(tmp).Reduce(r, cub::Max());
+    double rmax = block_reduce<PYGBE_TG>(r, OpMax());
     if (threadIdx.x == 0) {
         ggeo[2 * g] = make_double4(s_c[0], s_c[1], s_c[2], rmax);
         ggeo[2 * g + 1] = make_double4(0.5 * (mx[0] - mn[0]), 0.5 * (mx[1] - mn[1]), 0.5 * (mx[2] - mn[2]), 0.0);

@@ -145,3 +145,13 @@ def test_no_environment_knobs_in_the_product_build():
             if re.search(r"\bgetenv\s*\(", line) and not line.strip().startswith("//"):
                 hits.append((f, i))
     assert hits == [("common.cuh", hits[0][1])] and len(hits) == 1
+
+
+def test_no_library_kernels_in_the_product():
+    """North star: hand-written kernels, a GMRES "built on its own reduction kernels": no CUB / Thrust / cuBLAS include
+    anywhere in the library's sources (the Morton sort and the block reductions are csrc/blockops.cuh)."""
+    csrc = os.path.join(ROOT, "paper_1309_4018_b200", "csrc")
+    for f in sorted(os.listdir(csrc)):
+        text = open(os.path.join(csrc, f)).read()
+        for lib in ("cub/", "thrust/", "cublas", "cusparse", "cusolver"):
+            assert not re.search(r"#include\s*[<\"]" + lib, text), (f, lib)
