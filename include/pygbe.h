@@ -270,6 +270,16 @@ int pygbe_noalloc_setup(int32_t device);
 int pygbe_coulomb_energy_noalloc(int32_t device, void *stream, const double *xyz_dev, const double *q_dev, int64_t n,
                                  double eps, double *E_dev);
 
+/* Host-only (no GPU needed): the sparse coefficient tables that the P2M / M2M epilogue applies to a cell's Cartesian
+ * moments (canonical order: total order n, then kx descending, then ky descending) to form the M2P's input.
+ *   which = 0  regrouped form on harmonically reduced moments for the kernel exp(-kappa r)/r: entry p of the
+ *              stream -- ex, ey ascending, ez in {0, 1}, |e| <= P, then J = 0 .. (P - |e|)/2 -- is W_{m = |e| + J, e};
+ *   which = 1  Laplace form: entry p -- fx, fy, fz descending, |f| <= P -- is C_f, the coefficient of (d / r^2)^f; deg[p] = |f|.
+ * Entry p = sum_{i in [off[p], off[p+1])} c[i] * M^(k[i]).  With off == NULL only the sizes are returned.
+ * off: HOST int32 [cap_entries + 1]; k: int16 [cap_nnz]; c: double [cap_nnz]; deg: int16 [cap_entries] or NULL. */
+int pygbe_host_table(int32_t which, int32_t P, double kappa, int32_t cap_entries, int32_t cap_nnz, int32_t *n_entries,
+                     int32_t *n_nnz, int32_t *off, int16_t *k, double *c, int16_t *deg);
+
 /* Library / build identification, e.g. "pygbe-b200 0.3 sm_100a". */
 const char *pygbe_version(void);
 

@@ -353,5 +353,21 @@ def noalloc_setup(device=0):
     _check(L.pygbe_noalloc_setup(device))
 
 
+def host_table(which, P, kappa=0.0):
+    """pygbe_host_table: (off, k, c, deg) of the M2P coefficient table (0: regrouped / reduced, 1: Laplace form).  No GPU."""
+    L = lib()
+    ip = C.POINTER(C.c_int32)
+    L.pygbe_host_table.argtypes = [C.c_int32, C.c_int32, C.c_double, C.c_int32, C.c_int32, ip, ip, ip, C.POINTER(C.c_int16),
+                                   C.POINTER(C.c_double), C.POINTER(C.c_int16)]
+    ne, nz = C.c_int32(), C.c_int32()
+    _check(L.pygbe_host_table(which, P, float(kappa), 0, 0, C.byref(ne), C.byref(nz), None, None, None, None))
+    off = np.zeros(ne.value + 1, dtype=np.int32); k = np.zeros(nz.value, dtype=np.int16)
+    c = np.zeros(nz.value); deg = np.zeros(ne.value, dtype=np.int16)
+    _check(L.pygbe_host_table(which, P, float(kappa), ne.value, nz.value, C.byref(ne), C.byref(nz), off.ctypes.data_as(ip),
+                              k.ctypes.data_as(C.POINTER(C.c_int16)), c.ctypes.data_as(C.POINTER(C.c_double)),
+                              deg.ctypes.data_as(C.POINTER(C.c_int16))))
+    return off, k, c, deg
+
+
 def pygbe_version():
     return lib().pygbe_version().decode()

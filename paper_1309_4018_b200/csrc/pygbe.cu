@@ -211,3 +211,22 @@ extern "C" int pygbe_mma_probe(int32_t device, int32_t P, double *out12)
     pygbe_set_error("mma_probe: P = %d (instantiated for 6 and 8)", P);
     return PYGBE_EINVAL;
 }
+
+// Host-only: the coefficient tables of the M2P (tables.cuh), for CPU-side checks of the host logic.
+extern "C" int pygbe_host_table(int32_t which, int32_t P, double kappa, int32_t cap_entries, int32_t cap_nnz, int32_t *n_entries,
+                                int32_t *n_nnz, int32_t *off, int16_t *k, double *c, int16_t *deg)
+{
+    if (P < 0 || P > PYGBE_PMAX || !n_entries || !n_nnz || (which != 0 && which != 1)) { pygbe_set_error("host_table: bad arguments"); return PYGBE_EINVAL; }
+    IndexTables *it = new IndexTables;
+    fill_index_tables(it);
+    WTable w;
+    if (which == 0) build_w_table(P, kappa, *it, &w); else build_lap_table(P, *it, &w);
+    delete it;
+    *n_entries = (int)w.off.size() - 1; *n_nnz = (int)w.k.size();
+    if (!off || !k || !c) return PYGBE_OK;                              // size query
+    if (cap_entries < *n_entries || cap_nnz < *n_nnz) { pygbe_set_error("host_table: buffers too small"); return PYGBE_EINVAL; }
+    for (size_t i = 0; i < w.off.size(); i++) off[i] = w.off[i];
+    for (size_t i = 0; i < w.k.size(); i++) { k[i] = w.k[i]; c[i] = w.c[i]; }
+    if (deg && which == 1) for (size_t i = 0; i < w.deg.size(); i++) deg[i] = w.deg[i];
+    return PYGBE_OK;
+}
