@@ -107,7 +107,8 @@ k_panel_moments(int P, int Nc, int K, const IndexTables *__restrict__ tab, const
     }
 }
 
-// One CTA per needed leaf, one work item (split s, coefficient k) per thread: split s takes every nsplit-th
+// CTAs take needed leaves grid-stride (4 CTAs per SM with nsplit = 1 in the narrowed pass, matvec.cuh; one CTA per leaf at
+// full width); one work item (split s, coefficient k) per thread: split s takes every nsplit-th
 // panel of the leaf; the partial sums meet in shared memory in a fixed order (deterministic).
 #define P2M_MAXT 512
 static inline int p2m_nsplit(int Nc) { return Nc >= 192 ? 1 : (Nc >= 96 ? 2 : (256 / Nc > 8 ? 8 : 256 / Nc)); }
@@ -166,7 +167,7 @@ k_p2m(const int *__restrict__ skip, int Nc, int nsplit, int n_leaves, const int4
 // whose multipoles are used: the ones in some M2P list and, to build those, all their descendants
 // (build_lists.cuh) -- and handed out by an atomic ticket; a parent waits for the ready flag of each internal
 // child.  A child's ticket is always smaller than its parent's, so the CTA holding it is already running: no
-// deadlock whatever the residency.  Ready flags hold the matvec number (never reset); the last CTA to leave
+// deadlock whatever the residency.  Ready flags hold the number of the upward pass (sync[2], kept on the device; never reset); the last CTA to leave
 // resets the ticket.  Children are read with ld.global.cg (written by other SMs during this launch).
 // rec[i] = (cell, first child, number of children, bit c set if child c is internal).
 // Dynamic shared memory: 8 children x 2 Nc doubles.
