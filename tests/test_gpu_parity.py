@@ -783,3 +783,43 @@ def test_launch_times_account_for_the_lists(env):
     xs, it, rr, rc = h.solve(tol=1e-8)
     assert h.stats()["graph_launches"] >= 2 and rr <= 1e-8
     h.close()
+
+
+def test_destroy_returns_the_pool_memory(env):
+    """handles created without a workspace take their memory from a pool of the library's own (never the
+    device's default pool) whose release threshold is 256 MB, so destroying handles of growing size gives the memory
+    back to the driver; two handles alive at once on different streams do not disturb each other."""
+    pg, torch, orc = env
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    used = []
+    for level in (3, 4, 5, 6):
+        h = pg.Handle.from_problem(W.kirkwood_problem(level), K=4, P=6, theta=0.5, workspace=None)
+        x = torch.tensor(np.random.default_rng(level).normal(size=h.n), device="cuda")
+        h.matvec(x)
+        xs, it, rr, rc = h.solve(tol=1e-5)
+        used.append(h.stats()["device_bytes"])
+        h.close()
+        torch.cuda.synchronize()
+    assert used[-1] > 250e6                                          # the last handle was larger than what the pool may keep
+    free1 = torch.cuda.mem_get_info()[0]
+    assert free0 - free1 < 300e6, (free0, free1, used)
+    # two handles, two streams, interleaved matvecs
+    prob = W.kirkwood_problem(3)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    h1 = pg.Handle.from_problem(prob, K=4, P=6, theta=0.5, ncrit=16, stream=s1.cuda_stream)
+    h2 = pg.Handle.from_problem(prob, K=4, P=6, theta=0.5, ncrit=16, precision=pg.PRECISION_MIXED, stream=s2.cuda_stream)
+    x = torch.tensor(np.random.default_rng(2).normal(size=h1.n), device="cuda")
+    torch.cuda.synchronize()
+    y1 = [torch.empty_like(x) for _ in range(6)]
+    y2 = [torch.empty_like(x) for _ in range(6)]
+    for a, b in zip(y1, y2):
+        h1.matvec(x, a)
+        h2.matvec(x, b)
+    torch.cuda.synchronize()
+    for a in y1[1:]:
+        assert rel(a.cpu().numpy(), y1[0].cpu().numpy()) < 1e-12
+    for b in y2[1:]:
+        assert rel(b.cpu().numpy(), y2[0].cpu().numpy()) < 1e-12
+    assert rel(y2[0].cpu().numpy(), y1[0].cpu().numpy()) < 2e-5
+    h1.close(); h2.close()
