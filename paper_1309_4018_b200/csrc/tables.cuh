@@ -202,7 +202,7 @@ static void build_w_table(int P, double kappa, const IndexTables &t, WTable *w)
 // The Laplace form of the series (m2p.cuh, k_m2p_lap): entry p of the stream -- ex, ey, ez DESCENDING with
 // |f| <= P, the order the nested Horner scheme consumes them -- is the coefficient of u^f, u = d / r^2,
 //     C_f = sum_{2i <= f, e = f - 2i, J = |i|} (J! / i!) sum_{|j| = J} (-1)^J (2(|e| + J) - 1)!! / (e! 2^J j!) M^(e + 2j),
-// again a sparse row over the canonical moment index (1293 non-zeros at P = 8).  (-1)!! = 1.
+// again a sparse row over the canonical moment index (1275 non-zeros at P = 8).  (-1)!! = 1.
 static void build_lap_table(int P, const IndexTables &t, WTable *w)
 {
     double fact[PYGBE_PMAX + 1], dfact[2 * PYGBE_PMAX + 2];
