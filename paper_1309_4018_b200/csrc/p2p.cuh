@@ -327,7 +327,11 @@ __device__ __forceinline__ void p2p_quad_tile2(const float4 *__restrict__ sp, co
                                                f2_t Y0, f2_t Z0, f2_t X1, f2_t Y1, f2_t Z1, const P2PQuadConst &kc,
                                                f2_t (&a)[4], f2_t (&b)[4])
 {
-#pragma unroll 1
+#ifndef P2PQ2_UNROLL
+#define P2PQ2_UNROLL 1
+#endif
+    constexpr int UNR2 = P2PQ2_UNROLL;
+#pragma unroll UNR2
     for (int q = 0; q < nq; q++) {
         const float4 px = sp[3 * q], py = sp[3 * q + 1], pz = sp[3 * q + 2];
         const float4 mV = sc[4 * q], mKx = sc[4 * q + 1], mKy = sc[4 * q + 2], mKz = sc[4 * q + 3];
