@@ -126,20 +126,20 @@ def launch_flops(rec, P, kappa):
 
 def profiled_traffic(config, precision, kernel, region):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel` on `region`, from the newest
-    profiles/*_traffic.json (written from an `ncu --set full` capture of this command; the file names the capture and
-    the commit it was taken at).  None if there is no record for this configuration: the run itself measures no DRAM
-    counters."""
+    profiles/*_traffic.csv (columns config, precision, kernel, region, dram_bytes, duration_ms; written from an
+    `ncu --set full` capture of this command, which the *_path.md beside it names together with the commit).  None if
+    there is no record for this configuration: the run itself measures no DRAM counters."""
+    import csv
     import glob
-    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.json")), reverse=True):
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv")), reverse=True):
         try:
-            rec = json.load(open(path))
+            rows = list(csv.DictReader(open(path)))
         except Exception:
             continue
-        if rec.get("config") != config or rec.get("precision") != precision:
-            continue
-        for k in rec.get("kernels", []):
-            if k["kernel"] == kernel and k["region"] == region:
-                return k["dram_bytes"], "%s (%s)" % (os.path.basename(path), rec.get("source", ""))
+        for r in rows:
+            if r["config"] == config and r["precision"] == precision and r["kernel"] == kernel and int(r["region"]) == region:
+                note = os.path.basename(path).replace("_traffic.csv", "_path.md")
+                return float(r["dram_bytes"]), "profiles/%s (capture described in profiles/%s)" % (os.path.basename(path), note)
     return None, None
 
 
