@@ -85,3 +85,36 @@ def test_oracle_on_a_molecule_gauss_identity(oracle_mod):
     y = o.matvec(x)
     # slivers next to a target defeat the centroid-distance near-field rule locally (max), not globally (median)
     assert np.median(np.abs(y[:N])) < 2e-3 and np.max(np.abs(y[:N])) < 0.3
+
+
+def test_cache_is_shared_between_processes(tmp_path, monkeypatch):
+    """workloads.cached: two processes asking for the same problem at once build it once (lock file); the stored
+    .npz reproduces the problem exactly."""
+    import subprocess
+    import sys
+    import textwrap
+    import os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "w.py"
+    script.write_text(textwrap.dedent(f"""
+        import os, sys, time
+        sys.path.insert(0, {root!r})
+        os.environ["PYGBE_WORKLOAD_CACHE"] = {str(tmp_path / "cache")!r}
+        import workloads as W
+        def build():
+            open(os.path.join({str(tmp_path)!r}, "built_%d" % os.getpid()), "w").close()
+            time.sleep(1.0)
+            return W.protein_problem(40, spacing=1.6, seed=3)
+        p = W.cached("t_protein_40", build)
+        print(p.n_panels, float(p.surfaces[0].vertices.sum()))
+    """))
+    procs = [subprocess.Popen([sys.executable, str(script)], stdout=subprocess.PIPE, text=True) for _ in range(3)]
+    outs = [p.communicate(timeout=300)[0].strip() for p in procs]
+    assert all(p.returncode == 0 for p in procs) and len(set(outs)) == 1
+    assert len([f for f in os.listdir(tmp_path) if f.startswith("built_")]) == 1
+    assert not [f for f in os.listdir(tmp_path / "cache") if f.endswith(".lock")]
+    monkeypatch.setenv("PYGBE_WORKLOAD_CACHE", str(tmp_path / "cache"))
+    p = W.cached("t_protein_40", lambda: (_ for _ in ()).throw(AssertionError("must come from the cache")))
+    q = W.protein_problem(40, spacing=1.6, seed=3)
+    assert np.array_equal(p.surfaces[0].vertices, q.surfaces[0].vertices) and np.array_equal(p.charge_q, q.charge_q)
+    assert np.array_equal(p.surfaces[0].triangles, q.surfaces[0].triangles) and list(p.eps) == list(q.eps)

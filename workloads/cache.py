@@ -49,17 +49,60 @@ def load_problem(path):
     return Problem(surfaces, z["eps"], z["kappa"], z["charge_xyz"], z["charge_q"], z["charge_region"], name=str(z["name"]))
 
 
-def cached(tag, build):
-    """Problem `tag` (a string naming builder and arguments) from the cache, else build() and store it."""
+def cached(tag, build, wait_seconds=900.0):
+    """Problem `tag` (a string naming builder and arguments) from the cache, else build() and store it.  When several
+    processes ask at once (one rank per GPU under torchrun), one of them builds -- it holds an exclusive lock file --
+    and the others wait for the .npz to appear (or, if the builder dies, for the lock to go stale) instead of all
+    generating the same mesh side by side."""
+    import time
     path = os.path.join(cache_dir(), "%s_%s.npz" % (tag, _source_hash()))
-    if os.path.exists(path):
+    lock = path + ".lock"
+
+    def try_load():
+        if os.path.exists(path):
+            try:
+                return load_problem(path)
+            except Exception:
+                try:
+                    os.remove(path)
+                except OSError:
+                    pass
+        return None
+
+    p = try_load()
+    if p is not None:
+        return p
+    have_lock = False
+    t0 = time.time()
+    while True:
         try:
-            return load_problem(path)
-        except Exception:
-            os.remove(path)
-    p = build()
+            os.close(os.open(lock, os.O_CREAT | os.O_EXCL | os.O_WRONLY))
+            have_lock = True
+            break
+        except FileExistsError:
+            time.sleep(0.5)
+            p = try_load()
+            if p is not None:
+                return p
+            try:
+                stale = time.time() - os.path.getmtime(lock) > wait_seconds
+            except OSError:
+                stale = False                                   # lock just went away: try to take it
+            if stale or time.time() - t0 > wait_seconds:
+                break                                           # builder died or is too slow: build here, without the lock
+        except OSError:
+            break                                               # cache directory not writable: just build
     try:
-        save_problem(path, p)
-    except OSError:
-        pass
-    return p
+        p = try_load() or build()
+        try:
+            if not os.path.exists(path):
+                save_problem(path, p)
+        except OSError:
+            pass
+        return p
+    finally:
+        if have_lock:
+            try:
+                os.remove(lock)
+            except OSError:
+                pass
